@@ -1,0 +1,168 @@
+/*
+ * lensed.h -- C ABI of the B200-native batched lens likelihood.
+ *
+ * The hot path of Lensed (Tessore, Bellagamba & Metcalf, arXiv:1505.07674): for a batch
+ * of parameter vectors, ray-trace every pixel's quadrature points through the lens
+ * models, evaluate source / foreground surface brightness, integrate to pixel
+ * luminosities, convolve with the PSF and reduce the weighted chi-square to one
+ * log-likelihood per vector.  Citations are "PAPER.md:<line>" of the paper text plus the
+ * section / equation; "R<n>" is a reading listed in DESIGN.md where the paper is silent.
+ *
+ * Every step runs in hand-written CUDA kernels for sm_100a (paper_1505_07674_b200/csrc).
+ * There is no CPU fallback and no other backend: without a CUDA device lensed_create
+ * fails with LENSED_ECUDA.  Plain pointers and sizes only; "host" / "device" is stated
+ * for every pointer.  All device work of a call is enqueued on the given CUDA stream
+ * (a cudaStream_t passed as void*, NULL = the legacy default stream) and is asynchronous
+ * with respect to the host unless stated otherwise.
+ *
+ * Thread-safety: a handle owns its scratch buffers, so calls on ONE handle must not
+ * overlap in time (use one handle per stream / thread); different handles are
+ * independent.
+ */
+#ifndef LENSED_H
+#define LENSED_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lensed_handle lensed_handle;   /* opaque; owns device copies of all inputs */
+
+typedef enum {
+    LENSED_OK = 0,
+    LENSED_EINVAL = 1,        /* bad argument (see each call)                             */
+    LENSED_ENOMEM = 2,        /* host or device allocation failed                         */
+    LENSED_ECUDA = 3,         /* CUDA error; text in lensed_last_error                    */
+    LENSED_EUNSUPPORTED = 4   /* valid request outside the built limits (see LENSED_MAX_*)*/
+} lensed_status;
+
+/* Model kinds.  Lenses deflect (eq. 1, deflections add over lenses,
+ * PAPER.md:37, 357); SRC objects are evaluated at the source-plane point y(x), FG
+ * objects at the image-plane point x (eq. 2).
+ * Parameter layout per kind, in the paper's order:
+ *   SIS    x, y, r                   r = Einstein radius                       (R3)
+ *   SIE    x, y, r, q, pa            Kormann et al. 1994        (R2)
+ *   POINT  x, y, r                   r = Einstein radius of the point mass     (R3)
+ *   SHEAR  g1, g2                    about the image centre                    (R4)
+ *   SERSIC x, y, r, mag, n, q, pa    PAPER.md:244-252 eqs. 22-23; r = half-light (R5, R6)
+ *   GAUSS  x, y, sigma, mag, q, pa                                             (R7)
+ *   SKY    level                     per-pixel constant
+ * Positions and radii in arcsec relative to the image centre (+x = columns, +y = rows,
+ * R1), pa in degrees counter-clockwise from +x to the major axis.  A
+ * vector is the concatenation over the model list, in list order.                       */
+typedef enum {
+    LENSED_LENS_SIS = 0,
+    LENSED_LENS_SIE = 1,
+    LENSED_LENS_POINT = 2,
+    LENSED_LENS_SHEAR = 3,
+    LENSED_SRC_SERSIC = 4,
+    LENSED_SRC_GAUSS = 5,
+    LENSED_FG_SERSIC = 6,
+    LENSED_FG_GAUSS = 7,
+    LENSED_FG_SKY = 8
+} lensed_kind;
+
+#define LENSED_MAX_MODELS 32      /* objects in one model list                            */
+#define LENSED_MAX_QUAD   256     /* points of the pixel quadrature rule (g7k15 = 225)    */
+#define LENSED_MAX_PSF    63      /* PSF rows / columns                                   */
+
+/*
+ * lensed_create -- set up one reconstruction problem (PAPER.md:132-133 steps i-ii,
+ * 159, 182): copies every array to the device; the handle is immutable afterwards.
+ *   H, W        image rows / columns; pixel (i, j) = (row, column) has centre
+ *               x_j = (j-(W-1)/2) s, y_i = (i-(H-1)/2) s                         (R1)
+ *   pixel_scale s, arcsec per pixel, > 0
+ *   image       [H*W] host f32, row-major: observed d_i
+ *   weight      [H*W] host f32, w_i = 1/s_i^2 >= 0 (eq. 17)
+ *   mask        [H*W] host u8 or NULL; 0 = masked => w_i := 0
+ *   psf         [psf_h*psf_w] host f32, odd dims <= LENSED_MAX_PSF, element
+ *               [p+a][q+b] = F_{a,b}, first index = row (R10); divided
+ *               by its sum in double (L159).  NULL or 1x1 = no PSF.  Even dims, a
+ *               non-finite value or a zero sum: LENSED_EINVAL (R11).
+ *   quad        [n_quad][3] host f32 = (xi_k, eta_k, w_k): abscissae as offsets from
+ *               the pixel centre in pixel units, weights renormalised to sum 1
+ *               (eq. 14, R6).  1 <= n_quad <= LENSED_MAX_QUAD.
+ *   models      [n_models] host, 1 <= n_models <= LENSED_MAX_MODELS
+ *   mag_zero_point  zp of F = 10^(-0.4 (mag - zp))                               (R6)
+ *   device      CUDA device ordinal
+ *   out         receives the handle (NULL on failure)
+ * Errors: EINVAL for null pointers, non-positive sizes, negative or non-finite weights,
+ * non-finite image values at unmasked pixels, bad PSF / rule / kind; ECUDA if there is
+ * no usable device.  Synchronous.                                                       */
+lensed_status lensed_create(int H, int W, double pixel_scale,
+                            const float *image, const float *weight,
+                            const unsigned char *mask,
+                            const float *psf, int psf_h, int psf_w,
+                            const float *quad, int n_quad,
+                            const int *models, int n_models,
+                            double mag_zero_point, int device,
+                            lensed_handle **out);
+
+/* P, the length of one parameter vector for the handle's model list; -1 for NULL.       */
+int lensed_num_params(const lensed_handle *h);
+
+/* Pixels lensed_loglike ray-traces per vector: the unmasked set dilated by the PSF
+ * window with border clamping (R8); H*W without a mask.  -1 for NULL.                   */
+int lensed_num_traced(const lensed_handle *h);
+
+/*
+ * lensed_render -- model images L* (PAPER.md:136 step iv; eqs. 14, 15), mask ignored.
+ *   params_dev  [B][P] device f32
+ *   model_dev   [B][H][W] device f32, receives the PSF-convolved pixel luminosities; a
+ *               vector outside the model domain gets NaN everywhere
+ * Errors: EINVAL for null pointers or B < 1; ENOMEM / ECUDA.                            */
+lensed_status lensed_render(lensed_handle *h, const float *params_dev, int B,
+                            float *model_dev, void *cuda_stream);
+
+/*
+ * lensed_loglike -- loglike = -1/2 sum_i w_i (d_i - L*_i)^2 per vector
+ * (PAPER.md:137 step v, 172-182 eqs. 16-17; the normalisation term is dropped as in
+ * the paper).
+ *   params_dev  [B][P] device f32
+ *   logl_dev    [B] device f32; -INFINITY for a vector outside the model domain
+ * Deterministic: the same inputs give bitwise the same output on every call.            */
+lensed_status lensed_loglike(lensed_handle *h, const float *params_dev, int B,
+                             float *logl_dev, void *cuda_stream);
+
+/* The same two calls with HOST buffers: the parameters are copied to the device, the
+ * result is copied back and the stream is synchronised before returning.  Pinned host
+ * memory makes the copies asynchronous until that final synchronisation.                */
+lensed_status lensed_render_host(lensed_handle *h, const float *params_host, int B,
+                                 float *model_host, void *cuda_stream);
+lensed_status lensed_loglike_host(lensed_handle *h, const float *params_host, int B,
+                                  float *logl_host, void *cuda_stream);
+
+/*
+ * Instrumentation (measurement only; never changes results).
+ * lensed_set_profiling(h, 1) brackets every kernel the library launches with CUDA
+ * events on the launching stream.  lensed_get_profile synchronises those events and
+ * returns, since the last lensed_reset_profile: milliseconds and launch counts of the
+ * parameter-prep, ray-trace, convolution(+chi-square) and final-reduction kernels as
+ * ms[4] / launches[4] (host arrays, either may be NULL).  Launch counts are kept even
+ * with profiling off (ms are then 0).                                                   */
+lensed_status lensed_set_profiling(lensed_handle *h, int on);
+lensed_status lensed_get_profile(lensed_handle *h, double *ms, long long *launches);
+lensed_status lensed_reset_profile(lensed_handle *h);
+
+/* Tuning knob: bytes of device scratch the unconvolved images L[b] of one batch chunk
+ * may take (default 64 MiB, so that a chunk stays resident in the 126 MB L2).
+ * EINVAL if bytes < one image.                                                          */
+lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes);
+
+/*
+ * lensed_fma_peak -- FP32 FFMA micro-benchmark used as the measured roofline
+ * denominator: runs `iters` dependent-chain FFMAs per thread on a full grid and returns
+ * the achieved TFLOP/s (2 flops per FFMA) in *tflops.  Synchronous.                     */
+lensed_status lensed_fma_peak(int device, int iters, double *tflops);
+
+/* Text of the last error on this handle (valid until the next call on the handle); for
+ * a failed lensed_create or lensed_fma_peak pass NULL to read the thread-local text.    */
+const char *lensed_last_error(const lensed_handle *h);
+
+/* Frees the handle and its device memory (synchronises the device).  NULL is a no-op.   */
+void lensed_destroy(lensed_handle *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LENSED_H */

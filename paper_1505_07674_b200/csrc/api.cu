@@ -1,0 +1,498 @@
+// api.cu -- the C ABI of include/lensed.h: handle, argument checks, create-time tables
+// (traced-pixel list, active tiles, flipped PSF, padded rule), batch chunking and launches.
+// Host logic only; every step of the path runs in prep.cu / trace.cu / conv.cu.
+#include "../../include/lensed.h"
+#include "lensed_internal.h"
+
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace lensed;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+enum { PH_PREP = 0, PH_TRACE = 1, PH_CONV = 2, PH_FINAL = 3, PH_COUNT = 4 };
+
+struct EventPair { cudaEvent_t a, b; int phase; };
+
+}  // namespace
+
+struct lensed_handle {
+    int device = 0;
+    int H = 0, W = 0;
+    double scale = 0, zp = 0;
+    Program prog{};
+    int n_quad = 0, R = 1, nq_pad = 0;
+    int KH = 1, KW = 1, NC = 1;
+    int tile_w = 0, tile_h = 0;
+
+    // device, immutable after create
+    float *d_image = nullptr, *d_wmask = nullptr, *d_taps = nullptr;
+    float4 *d_quad = nullptr;
+    uint32_t *d_pix_ll = nullptr, *d_pix_all = nullptr, *d_tiles_ll = nullptr, *d_tiles_all = nullptr;
+    int npix_ll = 0, npix_all = 0, ntiles_ll = 0, ntiles_all = 0;
+
+    // device scratch, grown on demand
+    float *d_derived = nullptr; size_t cap_derived = 0;
+    float *d_L = nullptr; size_t cap_L = 0;
+    double *d_partial = nullptr; size_t cap_partial = 0;
+    float *d_stage_in = nullptr; size_t cap_stage_in = 0;
+    float *d_stage_out = nullptr; size_t cap_stage_out = 0;
+    long long chunk_bytes = 64ll << 20;
+
+    // instrumentation
+    bool profiling = false;
+    std::vector<EventPair> used;
+    std::vector<EventPair> pool;
+    double ms[PH_COUNT] = {0, 0, 0, 0};
+    long long launches[PH_COUNT] = {0, 0, 0, 0};
+
+    std::string err;
+};
+
+namespace {
+
+lensed_status fail(lensed_handle *h, lensed_status st, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (h) h->err = buf;
+    g_last_error = buf;
+    return st;
+}
+
+#define CU(h, call)                                                                           \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(h, e_ == cudaErrorMemoryAllocation ? LENSED_ENOMEM : LENSED_ECUDA,    \
+                        "%s: %s", #call, cudaGetErrorString(e_));                             \
+    } while (0)
+
+template <class T>
+lensed_status upload(lensed_handle *h, T **dst, const T *src, size_t n)
+{
+    CU(h, cudaMalloc((void **)dst, std::max<size_t>(n, 1) * sizeof(T)));
+    if (n) CU(h, cudaMemcpy(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice));
+    return LENSED_OK;
+}
+
+template <class T>
+lensed_status grow(lensed_handle *h, T **buf, size_t *cap, size_t need)
+{
+    if (need <= *cap) return LENSED_OK;
+    if (*buf) { CU(h, cudaFree(*buf)); *buf = nullptr; *cap = 0; }   // cudaFree synchronises
+    CU(h, cudaMalloc((void **)buf, need * sizeof(T)));
+    *cap = need;
+    return LENSED_OK;
+}
+
+// Pixels read by the PSF windows of the counted pixels, with border clamping (R8): a
+// counted pixel (i, j) reads rows clamp(i+k), |k| <= p, and columns clamp(j+l), |l| <= q.
+std::vector<uint8_t> dilate(const std::vector<uint8_t> &cnt, int H, int W, int p, int q)
+{
+    std::vector<uint8_t> rows((size_t)H * W, 0), out((size_t)H * W, 0);
+    for (int i = 0; i < H; ++i)
+        for (int k = -p; k <= p; ++k) {
+            const int ii = std::min(std::max(i + k, 0), H - 1);
+            for (int j = 0; j < W; ++j) rows[(size_t)ii * W + j] |= cnt[(size_t)i * W + j];
+        }
+    for (int i = 0; i < H; ++i)
+        for (int j = 0; j < W; ++j) {
+            if (!rows[(size_t)i * W + j]) continue;
+            for (int l = -q; l <= q; ++l) out[(size_t)i * W + std::min(std::max(j + l, 0), W - 1)] = 1;
+        }
+    return out;
+}
+
+void pixel_list(const std::vector<uint8_t> &sel, int H, int W, std::vector<uint32_t> &out)
+{
+    out.clear();
+    for (int i = 0; i < H; ++i)
+        for (int j = 0; j < W; ++j)
+            if (sel[(size_t)i * W + j]) out.push_back(((uint32_t)i << 16) | (uint32_t)j);
+}
+
+void tile_list(const std::vector<uint8_t> &cnt, int H, int W, int tw, int th, std::vector<uint32_t> &out)
+{
+    out.clear();
+    for (int ti = 0; ti * th < H; ++ti)
+        for (int tj = 0; tj * tw < W; ++tj) {
+            bool any = false;
+            for (int i = ti * th; i < std::min(H, (ti + 1) * th) && !any; ++i)
+                for (int j = tj * tw; j < std::min(W, (tj + 1) * tw); ++j)
+                    if (cnt[(size_t)i * W + j]) { any = true; break; }
+            if (any) out.push_back(((uint32_t)ti << 16) | (uint32_t)tj);
+        }
+}
+
+lensed_status timed_begin(lensed_handle *h, int phase, cudaStream_t st)
+{
+    h->launches[phase] += 1;
+    if (!h->profiling) return LENSED_OK;
+    EventPair ep;
+    if (!h->pool.empty()) { ep = h->pool.back(); h->pool.pop_back(); }
+    else { CU(h, cudaEventCreate(&ep.a)); CU(h, cudaEventCreate(&ep.b)); }
+    ep.phase = phase;
+    CU(h, cudaEventRecord(ep.a, st));
+    h->used.push_back(ep);
+    return LENSED_OK;
+}
+
+lensed_status timed_end(lensed_handle *h, cudaStream_t st)
+{
+    if (!h->profiling) return LENSED_OK;
+    CU(h, cudaEventRecord(h->used.back().b, st));
+    return LENSED_OK;
+}
+
+lensed_status collect_profile(lensed_handle *h)
+{
+    for (EventPair &ep : h->used) {
+        CU(h, cudaEventSynchronize(ep.b));
+        float ms = 0.f;
+        CU(h, cudaEventElapsedTime(&ms, ep.a, ep.b));
+        h->ms[ep.phase] += ms;
+        h->pool.push_back(ep);
+    }
+    h->used.clear();
+    return LENSED_OK;
+}
+
+// The whole path for B vectors already on the device.
+lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_dev, bool render,
+                  cudaStream_t st)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (!params_dev || !out_dev) return fail(h, LENSED_EINVAL, "null device pointer");
+    if (B < 1) return fail(h, LENSED_EINVAL, "B = %d < 1", B);
+    CU(h, cudaSetDevice(h->device));
+    const Program &prog = h->prog;
+    const size_t HW = (size_t)h->H * h->W;
+    const int n_tiles = render ? h->ntiles_all : h->ntiles_ll;
+    const int npix = render ? h->npix_all : h->npix_ll;
+
+    long long per_chunk = std::max<long long>(1, h->chunk_bytes / (long long)(HW * sizeof(float)));
+    const int Bc = (int)std::min<long long>(std::min<long long>(per_chunk, 65535), B);
+
+    lensed_status s;
+    if ((s = grow(h, &h->d_derived, &h->cap_derived, (size_t)B * prog.D)) != LENSED_OK) return s;
+    if ((s = grow(h, &h->d_L, &h->cap_L, (size_t)Bc * HW)) != LENSED_OK) return s;
+    if (!render && (s = grow(h, &h->d_partial, &h->cap_partial, (size_t)B * std::max(n_tiles, 1))) != LENSED_OK)
+        return s;
+
+    PrepArgs pa{params_dev, h->d_derived, B, h->scale, h->zp, 0.5 * (h->W - 1), 0.5 * (h->H - 1)};
+    if ((s = timed_begin(h, PH_PREP, st)) != LENSED_OK) return s;
+    CU(h, launch_prep(prog, pa, st));
+    if ((s = timed_end(h, st)) != LENSED_OK) return s;
+
+    for (int b0 = 0; b0 < B; b0 += Bc) {
+        const int nb = std::min(Bc, B - b0);
+        if (npix > 0) {
+            TraceArgs ta{};
+            ta.derived = h->d_derived + (size_t)b0 * prog.D;
+            ta.pix = render ? h->d_pix_all : h->d_pix_ll;
+            ta.quad = h->d_quad;
+            ta.L = h->d_L;
+            ta.l_stride = (long long)HW;
+            ta.npix = npix; ta.nq_pad = h->nq_pad; ta.W = h->W;
+            ta.cxh = 0.5f * (h->W - 1); ta.cyh = 0.5f * (h->H - 1);
+            if ((s = timed_begin(h, PH_TRACE, st)) != LENSED_OK) return s;
+            CU(h, launch_trace(prog, ta, h->R, nb, st));
+            if ((s = timed_end(h, st)) != LENSED_OK) return s;
+        }
+        if (n_tiles > 0) {
+            ConvArgs ca{};
+            ca.L = h->d_L;
+            ca.taps = h->d_taps;
+            ca.image = h->d_image;
+            ca.wmask = h->d_wmask;
+            ca.tiles = render ? h->d_tiles_all : h->d_tiles_ll;
+            ca.partial = render ? nullptr : h->d_partial + (size_t)b0 * n_tiles;
+            ca.model = render ? out_dev + (size_t)b0 * HW : nullptr;
+            ca.derived = h->d_derived + (size_t)b0 * prog.D;
+            ca.l_stride = (long long)HW;
+            ca.D = prog.D;
+            ca.H = h->H; ca.W = h->W; ca.KH = h->KH; ca.KW = h->KW; ca.NC = h->NC; ca.n_tiles = n_tiles;
+            ca.p = (h->KH - 1) / 2; ca.q = (h->KW - 1) / 2;
+            if ((s = timed_begin(h, PH_CONV, st)) != LENSED_OK) return s;
+            CU(h, launch_conv(ca, render, nb, st));
+            if ((s = timed_end(h, st)) != LENSED_OK) return s;
+        }
+    }
+    if (!render) {
+        FinalArgs fa{h->d_partial, h->d_derived, out_dev, B, n_tiles, prog.D};
+        if ((s = timed_begin(h, PH_FINAL, st)) != LENSED_OK) return s;
+        CU(h, launch_final(fa, st));
+        if ((s = timed_end(h, st)) != LENSED_OK) return s;
+    }
+    return LENSED_OK;
+}
+
+lensed_status run_host(lensed_handle *h, const float *params_host, int B, float *out_host, bool render,
+                       cudaStream_t st)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (!params_host || !out_host) return fail(h, LENSED_EINVAL, "null host pointer");
+    if (B < 1) return fail(h, LENSED_EINVAL, "B = %d < 1", B);
+    CU(h, cudaSetDevice(h->device));
+    const size_t n_in = (size_t)B * h->prog.P;
+    const size_t n_out = render ? (size_t)B * h->H * h->W : (size_t)B;
+    lensed_status s;
+    if ((s = grow(h, &h->d_stage_in, &h->cap_stage_in, n_in)) != LENSED_OK) return s;
+    if ((s = grow(h, &h->d_stage_out, &h->cap_stage_out, n_out)) != LENSED_OK) return s;
+    CU(h, cudaMemcpyAsync(h->d_stage_in, params_host, n_in * sizeof(float), cudaMemcpyHostToDevice, st));
+    if ((s = run(h, h->d_stage_in, B, h->d_stage_out, render, st)) != LENSED_OK) return s;
+    CU(h, cudaMemcpyAsync(out_host, h->d_stage_out, n_out * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CU(h, cudaStreamSynchronize(st));
+    return LENSED_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+lensed_status lensed_create(int H, int W, double pixel_scale, const float *image, const float *weight,
+                            const unsigned char *mask, const float *psf, int psf_h, int psf_w,
+                            const float *quad, int n_quad, const int *models, int n_models,
+                            double mag_zero_point, int device, lensed_handle **out)
+{
+    if (!out) return fail(nullptr, LENSED_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (H < 1 || W < 1) return fail(nullptr, LENSED_EINVAL, "image size %d x %d", H, W);
+    if (H > 32767 || W > 32767) return fail(nullptr, LENSED_EUNSUPPORTED, "image side > 32767");
+    if (!(pixel_scale > 0.0) || !isfinite(pixel_scale)) return fail(nullptr, LENSED_EINVAL, "pixel_scale must be > 0");
+    if (!isfinite(mag_zero_point)) return fail(nullptr, LENSED_EINVAL, "mag_zero_point not finite");
+    if (!image || !weight) return fail(nullptr, LENSED_EINVAL, "image / weight is NULL");
+    if (!quad || n_quad < 1) return fail(nullptr, LENSED_EINVAL, "quadrature rule missing (n_quad = %d)", n_quad);
+    if (n_quad > LENSED_MAX_QUAD) return fail(nullptr, LENSED_EUNSUPPORTED, "n_quad %d > %d", n_quad, LENSED_MAX_QUAD);
+    if (!models || n_models < 1) return fail(nullptr, LENSED_EINVAL, "model list missing");
+    if (n_models > LENSED_MAX_MODELS) return fail(nullptr, LENSED_EUNSUPPORTED, "n_models %d > %d", n_models, LENSED_MAX_MODELS);
+    const bool has_psf = psf && !(psf_h == 1 && psf_w == 1);
+    if (psf) {
+        if (psf_h < 1 || psf_w < 1 || psf_h % 2 == 0 || psf_w % 2 == 0)
+            return fail(nullptr, LENSED_EINVAL, "PSF dims %d x %d must be odd (R11)", psf_h, psf_w);
+        if (psf_h > LENSED_MAX_PSF || psf_w > LENSED_MAX_PSF)
+            return fail(nullptr, LENSED_EUNSUPPORTED, "PSF side > %d", LENSED_MAX_PSF);
+    }
+
+    const size_t HW = (size_t)H * W;
+    std::vector<uint8_t> counted(HW), all(HW, 1);
+    std::vector<float> wmask(HW);
+    for (size_t i = 0; i < HW; ++i) {
+        const float w = weight[i];
+        if (!(w >= 0.0f) || !isfinite(w)) return fail(nullptr, LENSED_EINVAL, "weight[%zu] negative or not finite", i);
+        const bool on = (!mask || mask[i]) && w > 0.0f;
+        if (on && !isfinite(image[i])) return fail(nullptr, LENSED_EINVAL, "image[%zu] not finite", i);
+        wmask[i] = on ? w : 0.0f;
+        counted[i] = on;
+    }
+
+    lensed_handle *h = new (std::nothrow) lensed_handle;
+    if (!h) return fail(nullptr, LENSED_ENOMEM, "host allocation failed");
+    lensed_status s = LENSED_OK;
+#define CREATE_FAIL(expr)                                             \
+    do { s = (expr); if (s != LENSED_OK) { g_last_error = h->err.empty() ? g_last_error : h->err; lensed_destroy(h); return s; } } while (0)
+
+    h->device = device; h->H = H; h->W = W; h->scale = pixel_scale; h->zp = mag_zero_point;
+
+    // model list -> program
+    Program &pg = h->prog;
+    pg.n_models = n_models;
+    int P = 0, D = kHeaderFloats;
+    for (int m = 0; m < n_models; ++m) {
+        const int k = models[m];
+        if (k < 0 || k >= K_COUNT) { delete h; return fail(nullptr, LENSED_EINVAL, "models[%d] = %d is not a lensed_kind", m, k); }
+        pg.kind[m] = (uint8_t)k;
+        pg.par_off[m] = (uint16_t)P;
+        pg.der_off[m] = (uint16_t)D;
+        if (k <= K_SHEAR) { pg.lens_kind[pg.n_lens] = (uint8_t)k; pg.lens_off[pg.n_lens++] = (uint16_t)D; }
+        else { pg.light_kind[pg.n_light] = (uint8_t)k; pg.light_off[pg.n_light++] = (uint16_t)D; }
+        P += kind_num_params(k);
+        D += kind_num_derived(k);
+    }
+    pg.P = P; pg.D = D;
+
+    // rule: weights to unit sum in double, padded with zero-weight points to a multiple of R
+    double wsum = 0.0;
+    for (int k = 0; k < n_quad; ++k) {
+        for (int c = 0; c < 3; ++c)
+            if (!isfinite(quad[3 * k + c])) { delete h; return fail(nullptr, LENSED_EINVAL, "quad[%d] not finite", k); }
+        wsum += (double)quad[3 * k + 2];
+    }
+    if (!(fabs(wsum) > 0.0)) { delete h; return fail(nullptr, LENSED_EINVAL, "quadrature weights sum to zero"); }
+    h->n_quad = n_quad;
+    h->R = trace_pick_R(n_quad);
+    h->nq_pad = (n_quad + h->R - 1) / h->R * h->R;
+    std::vector<float4> hq(h->nq_pad, make_float4(0.f, 0.f, 0.f, 0.f));
+    for (int k = 0; k < n_quad; ++k)
+        hq[k] = make_float4(quad[3 * k], quad[3 * k + 1], (float)((double)quad[3 * k + 2] / wsum), 0.f);
+
+    // PSF: normalise in double, flip (eq. 15 uses F_{-k,-l}), pad rows to 4-tap chunks
+    h->KH = has_psf ? psf_h : 1;
+    h->KW = has_psf ? psf_w : 1;
+    h->NC = (h->KW + 3) / 4;
+    std::vector<float> taps((size_t)h->KH * 4 * h->NC, 0.0f);
+    if (has_psf) {
+        double fsum = 0.0;
+        for (int t = 0; t < psf_h * psf_w; ++t) {
+            if (!isfinite(psf[t])) { delete h; return fail(nullptr, LENSED_EINVAL, "psf[%d] not finite", t); }
+            fsum += (double)psf[t];
+        }
+        if (!(fabs(fsum) > 0.0)) { delete h; return fail(nullptr, LENSED_EINVAL, "PSF sums to zero"); }
+        for (int ky = 0; ky < psf_h; ++ky)
+            for (int kx = 0; kx < psf_w; ++kx)
+                taps[(size_t)ky * 4 * h->NC + kx] =
+                    (float)((double)psf[(size_t)(psf_h - 1 - ky) * psf_w + (psf_w - 1 - kx)] / fsum);
+    } else {
+        taps[0] = 1.0f;
+    }
+
+    // pixel lists and tile lists
+    conv_tile_shape(&h->tile_w, &h->tile_h);
+    std::vector<uint32_t> pix_ll, pix_all, tiles_ll, tiles_all;
+    pixel_list(dilate(counted, H, W, (h->KH - 1) / 2, (h->KW - 1) / 2), H, W, pix_ll);
+    pixel_list(all, H, W, pix_all);
+    tile_list(counted, H, W, h->tile_w, h->tile_h, tiles_ll);
+    tile_list(all, H, W, h->tile_w, h->tile_h, tiles_all);
+    h->npix_ll = (int)pix_ll.size(); h->npix_all = (int)pix_all.size();
+    h->ntiles_ll = (int)tiles_ll.size(); h->ntiles_all = (int)tiles_all.size();
+
+    int ndev = 0;
+    cudaError_t ce = cudaGetDeviceCount(&ndev);
+    if (ce != cudaSuccess || ndev < 1) {
+        delete h;
+        return fail(nullptr, LENSED_ECUDA, "no CUDA device (%s); there is no CPU fallback",
+                    ce != cudaSuccess ? cudaGetErrorString(ce) : "device count 0");
+    }
+    if (device < 0 || device >= ndev) { delete h; return fail(nullptr, LENSED_EINVAL, "device %d of %d", device, ndev); }
+    {
+        cudaError_t e1 = cudaSetDevice(device);
+        if (e1 != cudaSuccess) { delete h; return fail(nullptr, LENSED_ECUDA, "cudaSetDevice: %s", cudaGetErrorString(e1)); }
+        cudaDeviceProp prop;
+        e1 = cudaGetDeviceProperties(&prop, device);
+        if (e1 != cudaSuccess) { delete h; return fail(nullptr, LENSED_ECUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e1)); }
+        if (prop.major != 10) {
+            delete h;
+            return fail(nullptr, LENSED_ECUDA, "device %d is sm_%d%d; this library holds sm_100a code only",
+                        device, prop.major, prop.minor);
+        }
+        e1 = conv_setup();
+        if (e1 != cudaSuccess) { delete h; return fail(nullptr, LENSED_ECUDA, "conv_setup: %s", cudaGetErrorString(e1)); }
+    }
+    CREATE_FAIL(upload(h, &h->d_image, image, HW));
+    CREATE_FAIL(upload(h, &h->d_wmask, wmask.data(), HW));
+    CREATE_FAIL(upload(h, &h->d_taps, taps.data(), taps.size()));
+    CREATE_FAIL(upload(h, &h->d_quad, hq.data(), hq.size()));
+    CREATE_FAIL(upload(h, &h->d_pix_ll, pix_ll.data(), pix_ll.size()));
+    CREATE_FAIL(upload(h, &h->d_pix_all, pix_all.data(), pix_all.size()));
+    CREATE_FAIL(upload(h, &h->d_tiles_ll, tiles_ll.data(), tiles_ll.size()));
+    CREATE_FAIL(upload(h, &h->d_tiles_all, tiles_all.data(), tiles_all.size()));
+#undef CREATE_FAIL
+    *out = h;
+    return LENSED_OK;
+}
+
+int lensed_num_params(const lensed_handle *h) { return h ? h->prog.P : -1; }
+int lensed_num_traced(const lensed_handle *h) { return h ? h->npix_ll : -1; }
+
+lensed_status lensed_render(lensed_handle *h, const float *params_dev, int B, float *model_dev, void *stream)
+{
+    return run(h, params_dev, B, model_dev, true, (cudaStream_t)stream);
+}
+
+lensed_status lensed_loglike(lensed_handle *h, const float *params_dev, int B, float *logl_dev, void *stream)
+{
+    return run(h, params_dev, B, logl_dev, false, (cudaStream_t)stream);
+}
+
+lensed_status lensed_render_host(lensed_handle *h, const float *params_host, int B, float *model_host, void *stream)
+{
+    return run_host(h, params_host, B, model_host, true, (cudaStream_t)stream);
+}
+
+lensed_status lensed_loglike_host(lensed_handle *h, const float *params_host, int B, float *logl_host, void *stream)
+{
+    return run_host(h, params_host, B, logl_host, false, (cudaStream_t)stream);
+}
+
+lensed_status lensed_set_profiling(lensed_handle *h, int on)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    h->profiling = on != 0;
+    return LENSED_OK;
+}
+
+lensed_status lensed_get_profile(lensed_handle *h, double *ms, long long *launches)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    lensed_status s = collect_profile(h);
+    if (s != LENSED_OK) return s;
+    for (int i = 0; i < PH_COUNT; ++i) {
+        if (ms) ms[i] = h->ms[i];
+        if (launches) launches[i] = h->launches[i];
+    }
+    return LENSED_OK;
+}
+
+lensed_status lensed_reset_profile(lensed_handle *h)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    lensed_status s = collect_profile(h);
+    if (s != LENSED_OK) return s;
+    for (int i = 0; i < PH_COUNT; ++i) { h->ms[i] = 0.0; h->launches[i] = 0; }
+    return LENSED_OK;
+}
+
+lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (bytes < (long long)((size_t)h->H * h->W * sizeof(float)))
+        return fail(h, LENSED_EINVAL, "chunk of %lld bytes holds less than one image", bytes);
+    h->chunk_bytes = bytes;
+    return LENSED_OK;
+}
+
+lensed_status lensed_fma_peak(int device, int iters, double *tflops)
+{
+    if (!tflops || iters < 1) return fail(nullptr, LENSED_EINVAL, "lensed_fma_peak: bad argument");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev)
+        return fail(nullptr, LENSED_ECUDA, "lensed_fma_peak: no CUDA device %d", device);
+    CU(nullptr, cudaSetDevice(device));
+    CU(nullptr, run_fma_peak(iters, tflops));
+    return LENSED_OK;
+}
+
+const char *lensed_last_error(const lensed_handle *h)
+{
+    return h ? h->err.c_str() : g_last_error.c_str();
+}
+
+void lensed_destroy(lensed_handle *h)
+{
+    if (!h) return;
+    cudaSetDevice(h->device);
+    cudaDeviceSynchronize();
+    for (EventPair &ep : h->used) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+    for (EventPair &ep : h->pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+    cudaFree(h->d_image); cudaFree(h->d_wmask); cudaFree(h->d_taps); cudaFree(h->d_quad);
+    cudaFree(h->d_pix_ll); cudaFree(h->d_pix_all); cudaFree(h->d_tiles_ll); cudaFree(h->d_tiles_all);
+    cudaFree(h->d_derived); cudaFree(h->d_L); cudaFree(h->d_partial);
+    cudaFree(h->d_stage_in); cudaFree(h->d_stage_out);
+    delete h;
+}
+
+}  // extern "C"

@@ -1,0 +1,117 @@
+// lensed_internal.h -- shared declarations of the CUDA path (host side + kernels).
+// Not part of the public ABI (include/lensed.h is); shares nothing with oracle/.
+//
+// Units inside the kernels: PIXELS.  The prep kernel divides every length by the pixel
+// scale, so the ray tracer never multiplies by s; deflections are linear in that scaling
+// for every lens here (SIS, SIE, point mass: alpha(lambda x; lambda b) = lambda alpha(x; b);
+// shear is linear in x).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace lensed {
+
+// ---- derived-constant blocks (floats per model, each a multiple of 4 for LDS.128) ------
+// Every positioned component starts with its centre split as (integer pixel, fraction):
+//   c0 = (cxi, cxf, cyi, cyf),   pixel-frame centre = cxi + cxf, |cxf| <= 1/2,
+// so that the thread forms (float(j) - cxi) - cxf: an exact integer difference followed
+// by ONE rounding at the magnitude of the component-relative offset.
+//
+//  SIS    [c0][b, 0, 0, 0]                                              8
+//  SIE    [c0][cos, sin, q^2, q'][b*sqrt(q), b*sqrt(q)/q', 0, 0]        12
+//  POINT  [c0][thetaE^2, 0, 0, 0]                                       8
+//  SHEAR  [g1, g2, 0, 0]                                                4
+//  SERSIC [c0][a1, a2, a3, a4][log2 I0, b_n*log2(e), 1/(2n), 0]         12
+//         (u', v') = (a1 dx + a2 dy, a3 dx + a4 dy) = rotated, q-stretched offset / r_S,
+//         so that u'^2 + v'^2 = (R / r_S)^2 with R of PAPER.md:250 eq. 23
+//  GAUSS  [c0][a1, a2, a3, a4][log2 I0, log2(e)/2, 0, 0]                12   (offset / sigma)
+//  SKY    [level, 0, 0, 0]                                              4
+// Block 0 of every vector is the header [valid, 0, 0, 0].
+enum Kind : int {
+    K_SIS = 0, K_SIE = 1, K_POINT = 2, K_SHEAR = 3,
+    K_SRC_SERSIC = 4, K_SRC_GAUSS = 5, K_FG_SERSIC = 6, K_FG_GAUSS = 7, K_SKY = 8,
+    K_COUNT = 9
+};
+
+constexpr int kMaxModels = 32;
+constexpr int kMaxQuad = 256;
+constexpr int kMaxPsf = 63;
+constexpr int kHeaderFloats = 4;
+
+__host__ __device__ constexpr int kind_num_params(int k) {
+    return k == K_SIS ? 3 : k == K_SIE ? 5 : k == K_POINT ? 3 : k == K_SHEAR ? 2
+         : (k == K_SRC_SERSIC || k == K_FG_SERSIC) ? 7
+         : (k == K_SRC_GAUSS || k == K_FG_GAUSS) ? 6 : k == K_SKY ? 1 : -1;
+}
+__host__ __device__ constexpr int kind_num_derived(int k) {
+    return k == K_SIS ? 8 : k == K_SIE ? 12 : k == K_POINT ? 8 : k == K_SHEAR ? 4
+         : (k >= K_SRC_SERSIC && k <= K_FG_GAUSS) ? 12 : k == K_SKY ? 4 : -1;
+}
+
+// The model list compiled to two flat programs (lenses first, then lights); passed to the
+// kernels by value, i.e. it sits in the constant bank and is read with uniform loads.
+struct Program {
+    int n_models;                  // list order (prep kernel)
+    int n_lens, n_light;
+    int P, D;                      // floats per parameter vector / per derived vector
+    uint8_t kind[kMaxModels];      // list order
+    uint16_t par_off[kMaxModels];  // list order: offset into the parameter vector
+    uint16_t der_off[kMaxModels];  // list order: offset into the derived vector
+    uint8_t lens_kind[kMaxModels];
+    uint16_t lens_off[kMaxModels];
+    uint8_t light_kind[kMaxModels];   // K_SRC_* / K_FG_* / K_SKY
+    uint16_t light_off[kMaxModels];
+};
+
+struct PrepArgs {
+    const float *params;   // [B][P]
+    float *derived;        // [B][D]
+    int B;
+    double scale, zp;      // arcsec per pixel, magnitude zero point
+    double cxh, cyh;       // (W-1)/2, (H-1)/2
+};
+
+struct TraceArgs {
+    const float *derived;  // [.][D], already offset to the chunk's first vector
+    const uint32_t *pix;   // [npix] packed (row << 16) | column
+    const float4 *quad;    // [nq_pad] (xi, eta, w, 0), zero-weight padding up to a multiple of R
+    float *L;              // [.][H*W], chunk-local
+    long long l_stride;    // H*W
+    int npix, nq_pad, W;
+    float cxh, cyh;
+};
+
+struct ConvArgs {
+    const float *L;        // [.][H*W] chunk-local unconvolved images
+    const float *taps;     // [KH][4*NC] flipped, normalised PSF rows, zero padded columns
+    const float *image;    // [H*W] d
+    const float *wmask;    // [H*W] w_i, 0 where masked
+    const uint32_t *tiles; // [n_tiles] packed (tile row << 16) | tile column (active tiles)
+    double *partial;       // [.][n_tiles] chunk-local chi-square partials   (loglike)
+    float *model;          // [.][H*W] chunk-local output                     (render)
+    const float *derived;  // [.][D] chunk-local (valid flag)                 (render)
+    long long l_stride;
+    int D;
+    int H, W, KH, KW, NC, n_tiles;
+    int p, q;              // (KH-1)/2, (KW-1)/2
+};
+
+struct FinalArgs {
+    const double *partial; // [B][n_tiles]
+    const float *derived;  // [B][D]
+    float *logl;           // [B]
+    int B, n_tiles, D;
+};
+
+// launchers (each returns the cudaGetLastError of its launch)
+cudaError_t launch_prep(const Program &prog, const PrepArgs &a, cudaStream_t st);
+cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nvec, cudaStream_t st);
+cudaError_t launch_conv(const ConvArgs &a, bool render, int nvec, cudaStream_t st);
+cudaError_t launch_final(const FinalArgs &a, cudaStream_t st);
+cudaError_t conv_setup();                 // one-time function attributes
+int trace_pick_R(int n_quad);             // rays per register block for an n_quad-point rule
+void conv_tile_shape(int *tile_w, int *tile_h);
+size_t conv_smem_bytes(int KH, int NC);
+cudaError_t run_fma_peak(int iters, double *tflops);
+
+}  // namespace lensed

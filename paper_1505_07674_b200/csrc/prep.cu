@@ -1,0 +1,175 @@
+// prep.cu -- step a0: parameter vectors xi -> kernel-ready constants, in FP64 on the device.
+//
+// One thread per parameter vector.  Everything the ray tracer would otherwise recompute per
+// ray is evaluated once here, in double, and rounded to FP32 once:
+//   * component centres as (integer pixel, fraction)
+//   * SIE: cos/sin PA, q^2, q' = sqrt(1-q^2), b sqrt(q)        (R2)
+//   * Sersic: b_n from P(2n, b_n) = 1/2 (r_S is the half-light radius; R5),
+//     log2 I_0 from the total magnitude (R6), the rotated, q-stretched,
+//     r_S-scaled frame of eq. 23
+//   * the domain check: outside it the vector is flagged invalid.
+#include "lensed_internal.h"
+#include <math.h>
+
+namespace lensed {
+namespace {
+
+constexpr double kPi = 3.141592653589793238462643383279502884;
+constexpr double kLn2 = 0.693147180559945309417232121458176568;
+constexpr double kLn10 = 2.302585092994045684017991454684364208;
+
+// Regularised lower incomplete gamma P(a, x) by its power series
+//   P = x^a e^-x / Gamma(a+1) * (1 + x/(a+1) + x^2/((a+1)(a+2)) + ...),
+// which converges for every x > 0; near the root of P(2n, x) = 1/2 (x ~ 2n - 1/3 < a + 1)
+// the terms decrease from the start.  Returns ln P.
+__device__ double log_gamma_p_series(double a, double x, double lgam_a1)
+{
+    double term = 1.0, sum = 1.0;
+    for (int k = 1; k < 4000; ++k) {
+        term *= x / (a + k);
+        sum += term;
+        if (term < sum * 1e-17) break;
+    }
+    return a * log(x) - x - lgam_a1 + log(sum);
+}
+
+// b_n: Newton iteration in t = ln b on g(t) = ln P(2n, e^t) - ln(1/2).  ln P is close to
+// linear in t for small b (P ~ b^a / Gamma(a+1)), so the iteration also converges quickly
+// for n << 1 where Newton in b itself crawls.  Start: Ciotti & Bertin's asymptotic series
+// for n >= 0.36, the small-b solution (Gamma(a+1)/2)^(1/a) below.
+__device__ double sersic_bn(double n)
+{
+    const double a = 2.0 * n;
+    const double lgam_a1 = lgamma(a + 1.0);
+    double t;
+    if (n >= 0.36)
+        t = log(a - 1.0 / 3.0 + 4.0 / (405.0 * n) + 46.0 / (25515.0 * n * n));
+    else
+        t = (lgam_a1 - kLn2) / a;
+    for (int it = 0; it < 60; ++it) {
+        const double b = exp(t);
+        const double lp = log_gamma_p_series(a, b, lgam_a1);
+        // d ln P / dt = b * P'(b) / P,   b P'(b) = b^a e^-b / Gamma(a)
+        const double lden = a * t - b - (lgam_a1 - log(a));
+        const double dt = (lp + kLn2) * exp(lp - lden);
+        t -= dt;
+        if (fabs(dt) < 1e-15 * fmax(1.0, fabs(t))) break;
+    }
+    return exp(t);
+}
+
+__device__ inline void put_centre(float *d, double x_arcsec, double y_arcsec, const PrepArgs &a)
+{
+    const double cx = x_arcsec / a.scale + a.cxh, cy = y_arcsec / a.scale + a.cyh;
+    const double ix = rint(cx), iy = rint(cy);
+    d[0] = (float)ix; d[1] = (float)(cx - ix);
+    d[2] = (float)iy; d[3] = (float)(cy - iy);
+}
+
+// frame of eq. 23 scaled by 1/len: (u', v') = (sqrt(q) u, v / sqrt(q)) / len
+__device__ inline void put_frame(float *d, double pa_deg, double q, double len_px)
+{
+    double s, c;
+    sincos(pa_deg * (kPi / 180.0), &s, &c);
+    const double sq = sqrt(q);
+    d[0] = (float)(c * sq / len_px);
+    d[1] = (float)(s * sq / len_px);
+    d[2] = (float)(-s / (sq * len_px));
+    d[3] = (float)(c / (sq * len_px));
+}
+
+__global__ void __launch_bounds__(128) prep_kernel(Program prog, PrepArgs a)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= a.B) return;
+    const float *par = a.params + (size_t)b * prog.P;
+    float *der = a.derived + (size_t)b * prog.D;
+    bool valid = true;
+    for (int i = 0; i < prog.D; ++i) der[i] = 0.0f;
+
+    for (int m = 0; m < prog.n_models; ++m) {
+        const int kind = prog.kind[m];
+        const float *pf = par + prog.par_off[m];
+        float *d = der + prog.der_off[m];
+        double p[7];
+        const int np = kind_num_params(kind);
+        for (int i = 0; i < np; ++i) {
+            p[i] = (double)pf[i];
+            if (!isfinite(p[i])) valid = false;
+        }
+        if (!valid) continue;
+        switch (kind) {
+        case K_SIS:
+            valid = valid && p[2] >= 0.0;
+            put_centre(d, p[0], p[1], a);
+            d[4] = (float)(p[2] / a.scale);
+            break;
+        case K_POINT:
+            valid = valid && p[2] >= 0.0;
+            put_centre(d, p[0], p[1], a);
+            d[4] = (float)((p[2] / a.scale) * (p[2] / a.scale));
+            break;
+        case K_SHEAR:
+            d[0] = (float)p[0]; d[1] = (float)p[1];
+            break;
+        case K_SIE: {
+            const double q = p[3];
+            valid = valid && p[2] >= 0.0 && q > 0.0 && q <= 1.0;
+            if (!valid) break;
+            put_centre(d, p[0], p[1], a);
+            double s, c;
+            sincos(p[4] * (kPi / 180.0), &s, &c);
+            d[4] = (float)c; d[5] = (float)s;
+            d[6] = (float)(q * q);
+            d[7] = (float)sqrt((1.0 - q) * (1.0 + q));
+            const double qp = sqrt((1.0 - q) * (1.0 + q)), bq = p[2] / a.scale * sqrt(q);
+            d[8] = (float)bq;
+            d[9] = (float)(bq / fmax(qp, 0.4));   // only used where q' |v|/psi >= 0.4
+            break;
+        }
+        case K_SRC_SERSIC: case K_FG_SERSIC: {
+            const double rs = p[2] / a.scale, mag = p[3], n = p[4], q = p[5];
+            valid = valid && p[2] > 0.0 && n >= 0.02 && n <= 20.0 && q > 0.0 && q <= 1.0;
+            if (!valid) break;
+            put_centre(d, p[0], p[1], a);
+            put_frame(d + 4, p[6], q, rs);
+            const double bn = sersic_bn(n);
+            // I_0 = F b_n^(2n) / (2 pi n r_S^2 Gamma(2n)), r_S in pixels (R6)
+            const double ln_i0 = -0.4 * (mag - a.zp) * kLn10 + 2.0 * n * log(bn) - lgamma(2.0 * n)
+                                 - log(2.0 * kPi * n * rs * rs);
+            d[8] = (float)(ln_i0 / kLn2);
+            d[9] = (float)(bn / kLn2);
+            d[10] = (float)(0.5 / n);
+            break;
+        }
+        case K_SRC_GAUSS: case K_FG_GAUSS: {
+            const double sg = p[2] / a.scale, mag = p[3], q = p[4];
+            valid = valid && p[2] > 0.0 && q > 0.0 && q <= 1.0;
+            if (!valid) break;
+            put_centre(d, p[0], p[1], a);
+            put_frame(d + 4, p[5], q, sg);
+            const double ln_i0 = -0.4 * (mag - a.zp) * kLn10 - log(2.0 * kPi * sg * sg);
+            d[8] = (float)(ln_i0 / kLn2);
+            d[9] = (float)(0.5 / kLn2);
+            break;
+        }
+        case K_SKY:
+            d[0] = (float)p[0];
+            break;
+        default:
+            valid = false;
+        }
+    }
+    der[0] = valid ? 1.0f : 0.0f;
+}
+
+}  // namespace
+
+cudaError_t launch_prep(const Program &prog, const PrepArgs &a, cudaStream_t st)
+{
+    const int threads = 128;
+    prep_kernel<<<(a.B + threads - 1) / threads, threads, 0, st>>>(prog, a);
+    return cudaGetLastError();
+}
+
+}  // namespace lensed

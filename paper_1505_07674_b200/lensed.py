@@ -1,0 +1,208 @@
+"""Thin binding of the C-ABI library (include/lensed.h): argument marshalling only.
+
+Same names as the C entry points.  Every step of the path runs in the CUDA kernels of
+`liblensed_b200.so`; torch is used for device memory and streams.  There is no CPU
+fallback: if the library is missing it is built with nvcc, and if that fails, or there
+is no CUDA device, the calls raise.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblensed_b200.so")
+
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, 1, 2, 3, 4
+STATUS_NAMES = {0: "LENSED_OK", 1: "LENSED_EINVAL", 2: "LENSED_ENOMEM", 3: "LENSED_ECUDA",
+                4: "LENSED_EUNSUPPORTED"}
+# lensed_kind (include/lensed.h)
+LENS_SIS, LENS_SIE, LENS_POINT, LENS_SHEAR = 0, 1, 2, 3
+SRC_SERSIC, SRC_GAUSS, FG_SERSIC, FG_GAUSS, FG_SKY = 4, 5, 6, 7, 8
+PHASES = ("prep", "trace", "conv", "final")
+
+# every symbol include/lensed.h declares: (restype, argtypes)
+_c, _i, _d, _p, _ll = ctypes.c_char_p, ctypes.c_int, ctypes.c_double, ctypes.c_void_p, ctypes.c_longlong
+SYMBOLS = {
+    "lensed_create": (_i, [_i, _i, _d, _p, _p, _p, _p, _i, _i, _p, _i, _p, _i, _d, _i, _p]),
+    "lensed_num_params": (_i, [_p]),
+    "lensed_num_traced": (_i, [_p]),
+    "lensed_render": (_i, [_p, _p, _i, _p, _p]),
+    "lensed_loglike": (_i, [_p, _p, _i, _p, _p]),
+    "lensed_render_host": (_i, [_p, _p, _i, _p, _p]),
+    "lensed_loglike_host": (_i, [_p, _p, _i, _p, _p]),
+    "lensed_set_profiling": (_i, [_p, _i]),
+    "lensed_get_profile": (_i, [_p, _p, _p]),
+    "lensed_reset_profile": (_i, [_p]),
+    "lensed_set_chunk_bytes": (_i, [_p, _ll]),
+    "lensed_fma_peak": (_i, [_i, _i, _p]),
+    "lensed_last_error": (_c, [_p]),
+    "lensed_destroy": (None, [_p]),
+}
+
+
+class LensedError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__("%s: %s" % (STATUS_NAMES.get(status, status), text))
+        self.status = status
+
+
+_lib = None
+
+
+def lib():
+    """The loaded shared library; built in-tree with nvcc if it is not there."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            from . import build as _build
+            _build.build()
+        L = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _np(a, dtype):
+    return None if a is None else np.ascontiguousarray(a, dtype=dtype)
+
+
+def _hp(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _check(status, handle=None):
+    if status != OK:
+        text = lib().lensed_last_error(handle)
+        raise LensedError(status, text.decode() if text else "")
+
+
+def _stream(stream):
+    if stream is not None:
+        return ctypes.c_void_p(int(stream))
+    import torch
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def lensed_create(image, weight, mask, psf, quad, models, pixel_scale, mag_zero_point=0.0, device=0):
+    """-> opaque handle (ctypes.c_void_p).  Arrays are host numpy arrays; see lensed.h."""
+    image = _np(image, np.float32)
+    H, W = image.shape
+    weight = _np(weight, np.float32)
+    mask = _np(mask, np.uint8)
+    psf = _np(psf, np.float32)
+    ph, pw = (0, 0) if psf is None else psf.shape
+    quad = _np(quad, np.float32).reshape(-1, 3)
+    models = _np(models, np.int32)
+    if weight.shape != image.shape or (mask is not None and mask.shape != image.shape):
+        raise LensedError(EINVAL, "weight / mask shape differs from the image")
+    h = ctypes.c_void_p()
+    st = lib().lensed_create(H, W, float(pixel_scale), _hp(image), _hp(weight), _hp(mask), _hp(psf),
+                             ph, pw, _hp(quad), len(quad), _hp(models), len(models),
+                             float(mag_zero_point), int(device), ctypes.byref(h))
+    _check(st)
+    return h
+
+
+def lensed_num_params(h):
+    return lib().lensed_num_params(h)
+
+
+def lensed_num_traced(h):
+    return lib().lensed_num_traced(h)
+
+
+def lensed_render(h, params_dev, model_dev, stream=None):
+    """params_dev [B][P], model_dev [B][H][W]: contiguous float32 CUDA tensors."""
+    B = _check_dev(h, params_dev)
+    _check_out(model_dev, B)
+    _check(lib().lensed_render(h, params_dev.data_ptr(), B, model_dev.data_ptr(), _stream(stream)), h)
+    return model_dev
+
+
+def lensed_loglike(h, params_dev, logl_dev, stream=None):
+    """params_dev [B][P], logl_dev [B]: contiguous float32 CUDA tensors."""
+    B = _check_dev(h, params_dev)
+    _check_out(logl_dev, B)
+    _check(lib().lensed_loglike(h, params_dev.data_ptr(), B, logl_dev.data_ptr(), _stream(stream)), h)
+    return logl_dev
+
+
+def lensed_render_host(h, params_host, model_host, stream=None):
+    """Host float32 arrays (numpy, or pinned torch CPU tensors); returns after the copy back."""
+    pin, B = _host_ptr(params_host, lensed_num_params(h))
+    pout, _ = _host_ptr(model_host, None)
+    _check(lib().lensed_render_host(h, pin, B, pout, _stream(stream)), h)
+    return model_host
+
+
+def lensed_loglike_host(h, params_host, logl_host, stream=None):
+    pin, B = _host_ptr(params_host, lensed_num_params(h))
+    pout, _ = _host_ptr(logl_host, None)
+    _check(lib().lensed_loglike_host(h, pin, B, pout, _stream(stream)), h)
+    return logl_host
+
+
+def lensed_set_profiling(h, on):
+    _check(lib().lensed_set_profiling(h, int(bool(on))), h)
+
+
+def lensed_get_profile(h):
+    """-> ({phase: ms}, {phase: launches}) since the last reset."""
+    ms = (ctypes.c_double * 4)()
+    n = (ctypes.c_longlong * 4)()
+    _check(lib().lensed_get_profile(h, ms, n), h)
+    return dict(zip(PHASES, ms)), dict(zip(PHASES, n))
+
+
+def lensed_reset_profile(h):
+    _check(lib().lensed_reset_profile(h), h)
+
+
+def lensed_set_chunk_bytes(h, nbytes):
+    _check(lib().lensed_set_chunk_bytes(h, int(nbytes)), h)
+
+
+def lensed_fma_peak(device=0, iters=4096):
+    t = ctypes.c_double()
+    _check(lib().lensed_fma_peak(int(device), int(iters), ctypes.byref(t)))
+    return t.value
+
+
+def lensed_last_error(h=None):
+    t = lib().lensed_last_error(h)
+    return t.decode() if t else ""
+
+
+def lensed_destroy(h):
+    if h is not None and h.value:
+        lib().lensed_destroy(h)
+        h.value = None
+
+
+def _check_dev(h, params_dev):
+    P = lensed_num_params(h)
+    if not (params_dev.is_cuda and params_dev.is_contiguous() and str(params_dev.dtype) == "torch.float32"):
+        raise LensedError(EINVAL, "params must be a contiguous float32 CUDA tensor")
+    if params_dev.dim() != 2 or params_dev.shape[1] != P:
+        raise LensedError(EINVAL, "params must be [B][%d]" % P)
+    return int(params_dev.shape[0])
+
+
+def _check_out(t, B):
+    if not (t.is_cuda and t.is_contiguous() and str(t.dtype) == "torch.float32" and t.shape[0] == B):
+        raise LensedError(EINVAL, "output must be a contiguous float32 CUDA tensor with leading dim B")
+
+
+def _host_ptr(a, P):
+    if isinstance(a, np.ndarray):
+        if a.dtype != np.float32 or not a.flags["C_CONTIGUOUS"]:
+            raise LensedError(EINVAL, "host arrays must be contiguous float32")
+        B = a.shape[0] if P is None else a.size // P
+        return ctypes.c_void_p(a.ctypes.data), int(B)
+    if a.is_cuda or not a.is_contiguous() or str(a.dtype) != "torch.float32":
+        raise LensedError(EINVAL, "host tensors must be contiguous float32 CPU tensors")
+    B = a.shape[0] if P is None else a.numel() // P
+    return ctypes.c_void_p(a.data_ptr()), int(B)

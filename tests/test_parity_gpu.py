@@ -1,0 +1,248 @@
+"""Parity of the CUDA library (through the C ABI) against the CPU oracle, on a B200.
+
+Element by element on seeded inputs at sizes the oracle finishes in seconds (several tiles
+and a ragged tail), then at BASELINE.json's full sizes in the launch configuration
+bench.py times, on sampled vectors the oracle computes one by one.  Tolerances are
+north_star's: 1e-4 relative per rendered pixel above 1e-3 of the image peak, 1e-5 relative
+on logL (tests/cases.py).
+"""
+import numpy as np
+import pytest
+
+from paper_1505_07674_b200 import synth
+from tests.cases import LOGL_RTOL, PIXEL_RTOL, Problem, logl_errors, pixel_errors
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def L():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1505_07674_b200 import lensed
+    lensed.lib()
+    return lensed
+
+
+def _gpu_eval(L, h, params, H, W, render=True):
+    import torch
+    p = torch.from_numpy(np.ascontiguousarray(params, dtype=np.float32)).cuda()
+    logl = torch.empty(p.shape[0], dtype=torch.float32, device="cuda")
+    L.lensed_loglike(h, p, logl)
+    model = None
+    if render:
+        model = torch.empty((p.shape[0], H, W), dtype=torch.float32, device="cuda")
+        L.lensed_render(h, p, model)
+        model = model.cpu().numpy()
+    torch.cuda.synchronize()
+    return logl.cpu().numpy(), model
+
+
+def _check(L, prob, params, render=True):
+    c = prob.cfg
+    h = prob.create()
+    try:
+        logl_g, model_g = _gpu_eval(L, h, params, c.H, c.W, render)
+    finally:
+        L.lensed_destroy(h)
+    logl_o, model_o = prob.oracle_loglike(params, want_model=True)
+    el = logl_errors(logl_g, logl_o)
+    assert np.all(np.isfinite(logl_g))
+    assert el.max() <= LOGL_RTOL, "logL rel err %.3g at vector %d" % (el.max(), el.argmax())
+    if render:
+        ep = pixel_errors(model_g, model_o)
+        assert ep.max() <= PIXEL_RTOL, "pixel rel err %.3g at vector %d" % (ep.max(), ep.argmax())
+    return el.max()
+
+
+# ------------------------------------------------------------------ small, whole batches
+def test_tiny_config_whole_batch(L):
+    cfg = synth.get_config(0)
+    prob = Problem(cfg)
+    _check(L, prob, np.vstack([cfg.batch(), cfg.truth.astype(np.float32)[None]]))
+
+
+@pytest.mark.parametrize("index,H,W,B", [(1, 90, 70, 24), (2, 75, 93, 12), (3, 70, 80, 8), (4, 101, 67, 6)])
+def test_shrunk_configs_span_tiles_and_ragged_tails(L, index, H, W, B):
+    cfg = synth.shrunk(synth.get_config(index), H, W, B)
+    prob = Problem(cfg)
+    _check(L, prob, np.vstack([cfg.batch(), cfg.truth.astype(np.float32)[None]]))
+
+
+def test_paper_mock_scenario_gauss_kronrod_rule(L):
+    """120x120 @ 0.05", SIE + de Vaucouleurs host + Sersic source (18
+    parameters), default g3k7 rule -- 49 points, R = 7 register blocking."""
+    base = synth.get_config(1)
+    models = ("sie", "fg_sersic", "src_sersic")
+    truth = [0.0, 0.0, 1.3624, 0.75, 20.0,
+             0.0, 0.0, 2.0, synth.mag_of_flux(3000.0), 4.0, 0.75, 20.0,
+             0.12, -0.08, 0.2, synth.mag_of_flux(30.0), 2.0, 0.5, 100.0]
+
+    def draw(rng, B):
+        t = np.tile(np.array(truth), (B, 1))
+        t[:, [0, 1, 5, 6, 12, 13]] += rng.uniform(-0.05, 0.05, size=(B, 6))
+        t[:, [2, 7, 14]] *= rng.uniform(0.8, 1.2, size=(B, 3))
+        t[:, 16] = rng.uniform(0.5, 8.0, size=B)
+        t[:, 17] = rng.uniform(0.1, 1.0, size=B)
+        return t
+
+    cfg = synth.Config(1, "mock", 60, 64, 0.05, models, synth.gauss_kronrod_rule(7), base.psf, None,
+                       truth, 6, draw, 0.005, 2000.0)
+    _check(L, Problem(cfg), cfg.batch())
+
+
+# ------------------------------------------------- full sizes, bench launch configuration
+@pytest.mark.parametrize("index,B,n_sample", [(1, 1024, 6), (2, 4096, 3), (3, 4096, 2), (4, 1024, 2)])
+def test_full_size_configs_on_sampled_vectors(L, index, B, n_sample):
+    import torch
+    cfg = synth.get_config(index)
+    prob = Problem(cfg)
+    params = cfg.batch(B)
+    h = prob.create()
+    try:
+        assert L.lensed_num_traced(h) == cfg.n_traced()
+        p = torch.from_numpy(params).cuda()
+        logl = torch.empty(B, dtype=torch.float32, device="cuda")
+        L.lensed_loglike(h, p, logl)
+        logl2 = torch.empty(B, dtype=torch.float32, device="cuda")
+        L.lensed_loglike(h, p, logl2)
+        assert torch.equal(logl, logl2), "loglike is not bitwise reproducible"
+        idx = np.linspace(0, B - 1, n_sample).astype(int)
+        model = torch.empty((n_sample, cfg.H, cfg.W), dtype=torch.float32, device="cuda")
+        L.lensed_render(h, p[torch.from_numpy(idx).cuda()].contiguous(), model)
+        torch.cuda.synchronize()
+        logl_g, model_g = logl.cpu().numpy(), model.cpu().numpy()
+    finally:
+        L.lensed_destroy(h)
+    assert np.all(np.isfinite(logl_g))
+    logl_o, model_o = prob.oracle_loglike(params[idx], want_model=True)
+    assert logl_errors(logl_g[idx], logl_o).max() <= LOGL_RTOL
+    assert pixel_errors(model_g, model_o).max() <= PIXEL_RTOL
+
+
+# ------------------------------------------------------------------------------ edge cases
+def _mini(models, truth, H=24, W=20, psf=None, mask=None, quad=None, scale=0.05):
+    quad = synth.gauss_legendre_rule(2) if quad is None else quad
+    return synth.Config(9, "mini", H, W, scale, models, quad, psf, mask, truth, 1,
+                        lambda rng, B: np.tile(np.array(truth), (B, 1)), 0.01, 0.0)
+
+
+def test_ray_through_the_lens_centre_and_degenerate_lenses(L):
+    """psi = 0 / r = 0 exactly on a rule point (the rule has a point at the pixel centre and
+    the lens sits on a pixel centre); q = 1 SIE; zero-strength lenses."""
+    quad = np.array([[0.0, 0.0, 0.5], [0.25, -0.25, 0.5]])
+    g = [0.1, -0.05, 0.12, synth.mag_of_flux(50.0), 0.8, 30.0]
+    s = 0.05
+    cx, cy = (10 - 9.5) * s, (12 - 11.5) * s          # centre of pixel (row 12, col 10) of 24 x 20
+    for models, lens in ((("sie",), [cx, cy, 0.3, 0.7, 25.0]), (("sis",), [cx, cy, 0.3]),
+                         (("point",), [cx, cy, 0.2]), (("sie",), [cx, cy, 0.3, 1.0, 40.0]),
+                         (("sie",), [0.01, 0.02, 0.3, 0.999999, 40.0]),
+                         (("sie", "sis", "point"), [cx, cy, 0.0, 0.5, 10.0, cx, cy, 0.0, cx, cy, 0.0])):
+        cfg = _mini(models + ("src_gauss",), lens + g, quad=quad)
+        _check(L, Problem(cfg), cfg.truth.astype(np.float32)[None])
+
+
+def test_source_centre_on_a_rule_point(L):
+    """R = 0 exactly: lg2(0) = -inf must give I = I0 (unlensed foreground Sersic on a pixel centre)."""
+    quad = np.array([[0.0, 0.0, 1.0]])
+    s = 0.05
+    cfg = _mini(("fg_sersic", "sky"), [(10 - 9.5) * s, (12 - 11.5) * s, 0.2, synth.mag_of_flux(100.0), 2.5,
+                                        0.6, 15.0, 0.01], quad=quad)
+    _check(L, Problem(cfg), cfg.truth.astype(np.float32)[None])
+
+
+def test_asymmetric_non_square_psf_pins_the_flip_and_axis_order(L):
+    rng = np.random.default_rng(5)
+    psf = rng.uniform(0.0, 1.0, size=(5, 9))
+    psf[0, 8] = 7.0                                   # strongly off-centre tap: F_{-2,+4}
+    cfg = _mini(("sis", "src_gauss", "sky"), [0.0, 0.0, 0.25, 0.05, 0.02, 0.08, synth.mag_of_flux(30.0),
+                                                0.7, 50.0, 0.02], H=70, W=75, psf=psf)
+    _check(L, Problem(cfg), cfg.truth.astype(np.float32)[None])
+
+
+def test_largest_psf_and_one_column_image(L):
+    psf = synth.moffat_psf(63, 3.0, 2.5, e1=0.1)
+    cfg = _mini(("sie", "src_sersic", "sky"), [0.0, 0.0, 0.5, 0.8, 10.0, 0.1, 0.05, 0.1,
+                                                 synth.mag_of_flux(30.0), 1.0, 0.7, 50.0, 0.02],
+                H=66, W=40, psf=psf)
+    _check(L, Problem(cfg), cfg.truth.astype(np.float32)[None])
+    cfg = _mini(("fg_gauss",), [0.0, 0.0, 0.1, synth.mag_of_flux(30.0), 0.7, 50.0], H=37, W=1,
+                psf=synth.gaussian_psf(5, 2.0))
+    _check(L, Problem(cfg), cfg.truth.astype(np.float32)[None])
+
+
+def test_invalid_vectors_give_minus_infinity_and_nan_image(L):
+    import torch
+    cfg = synth.shrunk(synth.get_config(1), 40, 36, 4)
+    prob = Problem(cfg)
+    params = cfg.batch(6)
+    params[1, 3] = 1.5          # SIE q > 1
+    params[2, 9] = -0.1         # Sersic r <= 0
+    params[4, 11] = np.nan      # non-finite
+    params[5, 11] = 25.0        # Sersic n > 20
+    h = prob.create()
+    try:
+        logl_g, model_g = _gpu_eval(L, h, params, cfg.H, cfg.W)
+    finally:
+        L.lensed_destroy(h)
+    logl_o, model_o = prob.oracle_loglike(params)
+    bad = np.array([False, True, True, False, True, True])
+    assert np.array_equal(np.isneginf(logl_g), bad) and np.array_equal(np.isneginf(logl_o), bad)
+    assert np.all(np.isnan(model_g[bad])) and np.all(np.isfinite(model_g[~bad]))
+    assert logl_errors(logl_g[~bad], logl_o[~bad]).max() <= LOGL_RTOL
+
+
+def test_fully_masked_image_and_zero_weights(L):
+    cfg = synth.shrunk(synth.get_config(1), 30, 30, 3)
+    prob = Problem(cfg)
+    cfg.mask = np.zeros((30, 30), dtype=np.uint8)
+    h = prob.create()
+    try:
+        assert L.lensed_num_traced(h) == 0
+        logl_g, _ = _gpu_eval(L, h, cfg.batch(3), 30, 30, render=False)
+    finally:
+        L.lensed_destroy(h)
+    assert np.array_equal(logl_g, np.zeros(3, dtype=np.float32))
+
+
+def test_host_buffer_calls_match_device_calls_and_chunking_does_not_change_results(L):
+    import torch
+    cfg = synth.shrunk(synth.get_config(2), 80, 72, 40)
+    prob = Problem(cfg)
+    params = cfg.batch(40)
+    h = prob.create()
+    try:
+        logl_dev, model_dev = _gpu_eval(L, h, params, cfg.H, cfg.W)
+        logl_host = np.empty(40, dtype=np.float32)
+        L.lensed_loglike_host(h, params, logl_host)
+        pinned = torch.from_numpy(params).pin_memory()
+        out_pinned = torch.empty(40, dtype=torch.float32).pin_memory()
+        L.lensed_loglike_host(h, pinned, out_pinned)
+        model_host = np.empty((40, cfg.H, cfg.W), dtype=np.float32)
+        L.lensed_render_host(h, params, model_host)
+        L.lensed_set_chunk_bytes(h, 3 * cfg.H * cfg.W * 4)       # 3 vectors per chunk, ragged last chunk
+        logl_chunked, model_chunked = _gpu_eval(L, h, params, cfg.H, cfg.W)
+        L.lensed_set_profiling(h, True)
+        L.lensed_reset_profile(h)
+        _gpu_eval(L, h, params, cfg.H, cfg.W, render=False)
+        ms, n = L.lensed_get_profile(h)
+    finally:
+        L.lensed_destroy(h)
+    assert np.array_equal(logl_dev, logl_host) and np.array_equal(logl_dev, out_pinned.numpy())
+    assert np.array_equal(model_dev, model_host)
+    assert np.array_equal(logl_dev, logl_chunked) and np.array_equal(model_dev, model_chunked)
+    assert n == {"prep": 1, "trace": 14, "conv": 14, "final": 1}
+    assert all(v > 0 for v in ms.values())
+
+
+def test_create_rejects_bad_arguments_on_the_gpu_box_too(L):
+    cfg = synth.get_config(0)
+    img = np.zeros((8, 8), np.float32)
+    w = np.ones((8, 8), np.float32)
+    kinds = synth.kind_ids(cfg.models)
+    with pytest.raises(L.LensedError) as e:
+        L.lensed_create(img, w, None, np.ones((4, 3), np.float32), cfg.quad, kinds, 0.05)
+    assert e.value.status == L.EINVAL
+    with pytest.raises(L.LensedError) as e:
+        L.lensed_create(img, -w, None, None, cfg.quad, kinds, 0.05)
+    assert e.value.status == L.EINVAL
