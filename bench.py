@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line: log-likelihood evaluations / s of the batched lens likelihood.
+
+A step = one lensed_loglike call on one batch of B synthetic parameter vectors: prep ->
+fused ray-trace + surface brightness + quadrature -> PSF convolution + chi-square -> logL[B]
+(all rows of SURVEY.md section 8(a)).  Workload at N = 1: BASELINE.json's largest config,
+the Euclid-scale sweep (512x512 @ 0.1"/px, SIE + shear + Sersic source + Sersic lens light
++ sky, 31x31 Moffat PSF, 16-point sub4 rule) at its largest batch, B = 16384 -- the config
+north_star quotes the roofline target on.  `--config 0..4 --batch B` time the other configs
+(parity-test cases, not bench lines).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+N > 1 (under torchrun): every rank holds a replica of the handle and its own B vectors
+(batch sharding, no data-path collective; "weak" scaling); time = max over ranks.
+--impl reference times the CPU oracle (oracle/, test infrastructure, as it stands) on the
+host cores on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1505_07674_b200 import synth  # noqa: E402
+
+METRIC = "loglike_evals_per_sec"
+UNIT = "logL/s"
+DEFAULT_CONFIG = 4
+SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0
+NOMINAL_FP32_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12      # 74.45
+
+# Algorithmic FP32 flops (FMA = 2), SURVEY.md section 8(d) / DESIGN.md "flop model"
+FLOPS_RAY_POS, FLOPS_QUAD = 4, 2
+FLOPS_MODEL = {"sie": 50, "sis": 10, "point": 10, "shear": 8, "src_sersic": 17, "fg_sersic": 17,
+               "src_gauss": 16, "fg_gauss": 16, "sky": 0}
+MUFU_MODEL = {"sie": 4, "sis": 1, "point": 1, "shear": 0, "src_sersic": 3, "fg_sersic": 3,
+              "src_gauss": 1, "fg_gauss": 1, "sky": 0}
+
+
+def flops_per_ray(models):
+    return FLOPS_RAY_POS + FLOPS_QUAD + sum(FLOPS_MODEL[m] for m in models)
+
+
+def flops_per_conv_pixel(cfg):
+    taps = 1 if cfg.psf is None else cfg.psf.size
+    return 2 * taps + 3
+
+
+def workload_name(cfg, B):
+    psf = "delta" if cfg.psf is None else "%dx%d" % cfg.psf.shape
+    return "%s %dx%d @%.2f\"/px, %s, PSF %s, %d-point rule, B=%d" % (
+        cfg.name, cfg.H, cfg.W, cfg.scale, "+".join(cfg.models), psf, len(cfg.quad), B)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons while the timed region runs (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), [c.strip() for c in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for t, r in self.rows if t0 <= t <= t1] or [r for _, r in self.rows[-3:]]
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_problem(cfg, image, weight):
+    """(callable params -> logL) on the CPU oracle; imported here only (cpu_baseline / reference)."""
+    from oracle import lensed_oracle as orc
+    kinds = synth.kind_ids(cfg.models)
+
+    def f(params):
+        return orc.loglike(cfg.H, cfg.W, cfg.scale, image, weight, cfg.mask, cfg.psf, cfg.quad, kinds,
+                           params, zp=cfg.zp)
+    return f, orc.threads()
+
+
+def time_oracle(cfg, image, weight, params, budget_s):
+    """Oracle logL/s on a bounded sample: 1 vector to size it, then about budget_s of work."""
+    f, cores = oracle_problem(cfg, image, weight)
+    t0 = time.perf_counter(); f(params[:1]); t1 = time.perf_counter() - t0
+    n = int(max(1, min(len(params), budget_s / max(t1, 1e-6))))
+    t0 = time.perf_counter(); f(params[:n]); dt = time.perf_counter() - t0
+    return n / dt, cores, n, dt
+
+
+def make_observation_cuda(cfg, device):
+    """Observed image + weights: truth rendered by the CUDA library, seeded noise from synth."""
+    import torch
+    from paper_1505_07674_b200 import lensed
+    kinds = synth.kind_ids(cfg.models)
+    h = lensed.lensed_create(np.zeros((cfg.H, cfg.W), np.float32), np.ones((cfg.H, cfg.W), np.float32),
+                             None, cfg.psf, cfg.quad, kinds, cfg.scale, cfg.zp, device)
+    p = torch.from_numpy(cfg.truth.astype(np.float32)[None]).cuda(device)
+    m = torch.empty((1, cfg.H, cfg.W), dtype=torch.float32, device=p.device)
+    lensed.lensed_render(h, p, m)
+    torch.cuda.synchronize(device)
+    lensed.lensed_destroy(h)
+    return cfg.observe(m[0].cpu().numpy())
+
+
+def make_observation_oracle(cfg):
+    from oracle import lensed_oracle as orc
+    truth = orc.render(cfg.H, cfg.W, cfg.scale, cfg.psf, cfg.quad, synth.kind_ids(cfg.models),
+                       cfg.truth.astype(np.float32), zp=cfg.zp)[0]
+    return cfg.observe(truth)
+
+
+def run_reference(args, cfg, B):
+    """The reference arm of this tier: the CPU oracle, rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    image, weight = make_observation_oracle(cfg)
+    params = cfg.batch(B)
+    f, cores = oracle_problem(cfg, image, weight)
+    t0 = time.perf_counter(); f(params[:1]); t1 = time.perf_counter() - t0
+    total = max(1, args.steps + args.warmup)
+    n = int(max(1, min(B, 120.0 / total / max(t1, 1e-6))))          # whole run within ~2 minutes
+    for _ in range(args.warmup):
+        f(params[:n])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        f(params[:n])
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    sample = "%d of the %d vectors per step, full image" % (n, B)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": workload_name(cfg, B), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--config", type=int, default=DEFAULT_CONFIG)
+    ap.add_argument("--batch", type=int, default=0, help="vectors per GPU per step (0 = the config's)")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the batch sweep of the Euclid config")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    cfg = synth.get_config(args.config)
+    B = args.batch or cfg.B
+    if args.impl == "reference":
+        return run_reference(args, cfg, B)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1505_07674_b200 import lensed
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl ours needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    image, weight = make_observation_cuda(cfg, local)
+    kinds = synth.kind_ids(cfg.models)
+    h = lensed.lensed_create(image, weight, cfg.mask, cfg.psf, cfg.quad, kinds, cfg.scale, cfg.zp, local)
+    n_traced = lensed.lensed_num_traced(h)
+    n_counted = int(cfg.H * cfg.W if cfg.mask is None else cfg.mask.sum())
+
+    params = cfg.batch(B, stream=2 + rank)                 # this rank's shard of the global batch
+    p_dev = torch.from_numpy(params).to(dev)
+    logl = torch.empty(B, dtype=torch.float32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---------------------------------------------------------------- device-resident timing
+    for _ in range(args.warmup):
+        lensed.lensed_loglike(h, p_dev, logl)
+    lensed.lensed_set_profiling(h, True)
+    lensed.lensed_reset_profile(h)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    clocks = ClockSampler(local)
+    t_wall0 = time.perf_counter()
+    for a, b in ev:
+        flush.zero_()                                       # L2 flush between timed iterations (untimed)
+        a.record(stream)
+        lensed.lensed_loglike(h, p_dev, logl)
+        b.record(stream)
+    barrier()
+    t_wall1 = time.perf_counter()
+    clock_info = clocks.stop(t_wall0, t_wall1)
+    ms_steps = [a.elapsed_time(b) for a, b in ev]
+    phase_ms, phase_n = lensed.lensed_get_profile(h)
+    lensed.lensed_set_profiling(h, False)
+    t_dev = torch.tensor([sum(ms_steps)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_dev, op=dist.ReduceOp.MAX)
+    total_ms = float(t_dev.item())
+    value = world * B * args.steps / (total_ms * 1e-3)
+    rays_per_s = value * n_traced * len(cfg.quad)
+
+    # ------------------------------------------------------------- end to end, host buffers
+    p_host = torch.from_numpy(params).pin_memory()
+    l_host = torch.empty(B, dtype=torch.float32).pin_memory()
+    lensed.lensed_loglike_host(h, p_host, l_host)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        lensed.lensed_loglike_host(h, p_host, l_host)       # H2D + path + D2H + stream sync, every step
+    t_e2e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
+    e2e_value = world * B * args.steps / float(t_e2e.item())
+    assert np.array_equal(l_host.numpy(), logl.cpu().numpy())
+
+    # ------------------------------------------------------------------------------ roofline
+    fpr = flops_per_ray(cfg.models)
+    per_launch = {   # algorithmic flops of one launch of each kernel, averaged over its launches
+        "trace": fpr * len(cfg.quad) * n_traced * B * args.steps / max(phase_n["trace"], 1),
+        "conv": flops_per_conv_pixel(cfg) * n_counted * B * args.steps / max(phase_n["conv"], 1),
+    }
+    dom = max(("trace", "conv"), key=lambda k: phase_ms[k])
+    avg_ms = phase_ms[dom] / max(phase_n[dom], 1)
+    achieved = per_launch[dom] / (avg_ms * 1e-3) / 1e12
+    kern = {k: {"ms_per_step": phase_ms[k] / args.steps, "launches_per_step": phase_n[k] / args.steps,
+                "tflops": (per_launch[k] * phase_n[k] / (phase_ms[k] * 1e-3) / 1e12) if k in per_launch and phase_ms[k] > 0 else None}
+            for k in lensed.PHASES}
+    try:
+        measured_ffma = lensed.lensed_fma_peak(local, 2048)
+    except lensed.LensedError:
+        measured_ffma = None
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the ncu capture
+    if os.path.exists(tpath):
+        with open(tpath) as fh:
+            traffic = json.load(fh).get("%s:%d" % (dom, args.config))
+    roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS,
+                "unit": "TFLOP/s", "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": traffic,
+                "peak_source": "nominal 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                "measured_ffma_tflops": measured_ffma,
+                "frac_of_measured_ffma": achieved / measured_ffma if measured_ffma else None,
+                "whole_step_tflops": (per_launch["trace"] * phase_n["trace"] + per_launch["conv"] * phase_n["conv"])
+                / (total_ms * 1e-3) / 1e12 if world == 1 else None,
+                "flops_per_ray": fpr, "flops_per_conv_pixel": flops_per_conv_pixel(cfg), "kernels": kern}
+
+    # -------------------------------------------------------------- batch sweep (config 4 only)
+    sweep = None
+    if args.config == 4 and not args.no_sweep and world == 1:
+        sweep = []
+        for Bs in (256, 1024, 4096, 16384):
+            ps = torch.from_numpy(cfg.batch(Bs)).to(dev)
+            ls = torch.empty(Bs, dtype=torch.float32, device=dev)
+            lensed.lensed_loglike(h, ps, ls)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            flush.zero_()
+            a.record(stream); lensed.lensed_loglike(h, ps, ls); b.record(stream)
+            torch.cuda.synchronize()
+            v = Bs / (a.elapsed_time(b) * 1e-3)
+            sweep.append({"B": Bs, "logl_per_s": v, "rays_per_s": v * n_traced * len(cfg.quad)})
+
+    # ---------------------------------------------------------------------------- cpu baseline
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, cores, n, dt = time_oracle(cfg, image, weight, params, 15.0)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "%d of the %d vectors, full image, %.1f s" % (n, B, dt)}
+
+    lensed.lensed_destroy(h)
+    if rank == 0:
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(cfg, B), "batch_per_gpu": B, "global_batch": B * world,
+                       "traced_pixels": n_traced, "rays_per_step": B * world * n_traced * len(cfg.quad),
+                       "parallelism": "batch-sharded x%d, no collective" % world,
+                       "timing": "CUDA events per step, L2 flushed (256 MB write) between steps, max over ranks"},
+            "rays_per_sec": rays_per_s,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(params.nbytes),
+                    "d2h_bytes_per_step": int(B * 4)},
+            "gpu_launches": int(sum(phase_n.values())),
+            "clocks": clock_info, "roofline": roofline, "cpu_baseline": cpu,
+        }
+        if sweep is not None:
+            out["sweep"] = sweep
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -22,8 +22,8 @@
 // rows are all inside the PSF run branch-free; the first and last ones test each (row, o)
 // pair with block-uniform branches, so no multiply by a padded zero is ever issued in y.
 //
-// Epilogue: loglike -> per-thread FP32 sum over its 4 kTR pixels, warp shuffle tree, then
-// FP64 across the block's warps and one FP64 partial per (vector, tile), summed in a fixed
+// Epilogue: loglike -> per-thread FP32 sum over its 4 kTR pixels, then FP64: warp shuffle
+// tree, the block's warps, and one FP64 partial per (vector, tile), summed in a fixed
 // order by final_kernel: bitwise reproducible, no float atomics.
 #include "lensed_internal.h"
 #include <math.h>
@@ -117,6 +117,8 @@ __global__ void __launch_bounds__(kThreads, 2) conv_kernel(ConvArgs a)
     }
     const bool warp_any = __any_sync(0xffffffffu, any);
 
+    // acc: running sum over tap-column chunks; part: the current chunk (blocked summation:
+    // a chunk adds 4 KH products, the running sum adds NC chunk totals)
     float acc[kTR][4];
 #pragma unroll
     for (int o = 0; o < kTR; ++o)
@@ -130,17 +132,26 @@ __global__ void __launch_bounds__(kThreads, 2) conv_kernel(ConvArgs a)
         const float4 *in_base = reinterpret_cast<const float4 *>(s_in) + (size_t)(ty * kTR) * IW4 + tx;
 #pragma unroll 1
         for (int c = 0; c < a.NC; ++c) {
+            float part[kTR][4];
             float4 T[kTR];
 #pragma unroll
-            for (int s = 0; s < kTR; ++s) T[s] = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int s = 0; s < kTR; ++s) {
+                T[s] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                for (int e = 0; e < 4; ++e) part[s][e] = 0.0f;
+            }
             const float4 *in_c = in_base + c;
             const float4 *tap_c = s_tap + c;
-            super_step<true>(acc, T, in_c, tap_c, 0, a.KH, a.NC, IW4);
+            super_step<true>(part, T, in_c, tap_c, 0, a.KH, a.NC, IW4);
             int g = 1;
 #pragma unroll 1
-            for (; g <= g_hi; ++g) super_step<false>(acc, T, in_c, tap_c, g, a.KH, a.NC, IW4);
+            for (; g <= g_hi; ++g) super_step<false>(part, T, in_c, tap_c, g, a.KH, a.NC, IW4);
 #pragma unroll 1
-            for (; g < G; ++g) super_step<true>(acc, T, in_c, tap_c, g, a.KH, a.NC, IW4);
+            for (; g < G; ++g) super_step<true>(part, T, in_c, tap_c, g, a.KH, a.NC, IW4);
+#pragma unroll
+            for (int o = 0; o < kTR; ++o)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) acc[o][e] += part[o][e];
         }
     }
 
@@ -172,9 +183,10 @@ __global__ void __launch_bounds__(kThreads, 2) conv_kernel(ConvArgs a)
                     }
                 }
         }
+        double dpart = (double)part;
 #pragma unroll
-        for (int sft = 16; sft > 0; sft >>= 1) part += __shfl_xor_sync(0xffffffffu, part, sft);
-        if (lane == 0) s_red[warp] = (double)part;
+        for (int sft = 16; sft > 0; sft >>= 1) dpart += __shfl_xor_sync(0xffffffffu, dpart, sft);
+        if (lane == 0) s_red[warp] = dpart;
         __syncthreads();
         if (threadIdx.x == 0) {
             double s = 0.0;
