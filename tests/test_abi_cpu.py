@@ -1,0 +1,96 @@
+"""CPU-side checks of the boundary: the C-ABI library loads, exports every symbol that
+include/lensed.h declares, validates arguments before touching CUDA, and fails loudly
+(LENSED_ECUDA, no fallback) when there is no device.  No compute calls."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1505_07674_b200 import lensed, synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    text = open(os.path.join(ROOT, "include", "lensed.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return set(re.findall(r"\b(lensed_[a-z_]+)\s*\(", text))
+
+
+def test_library_exports_every_declared_symbol_and_binding_covers_them():
+    declared = _declared()
+    assert len(declared) >= 12
+    dll = ctypes.CDLL(lensed.LIB_PATH) if os.path.exists(lensed.LIB_PATH) else lensed.lib()
+    for name in declared:
+        assert hasattr(dll, name), name
+    assert declared == set(lensed.SYMBOLS), declared ^ set(lensed.SYMBOLS)
+    for name in declared - {"lensed_last_error", "lensed_destroy", "lensed_create"}:
+        assert hasattr(lensed, name)
+
+
+def test_kind_numbering_matches_the_header_and_the_input_generator():
+    text = open(os.path.join(ROOT, "include", "lensed.h")).read()
+    enum = dict((k, int(v)) for k, v in re.findall(r"LENSED_((?:LENS|SRC|FG)_[A-Z]+)\s*=\s*(\d+)", text))
+    assert enum == {"LENS_SIS": 0, "LENS_SIE": 1, "LENS_POINT": 2, "LENS_SHEAR": 3, "SRC_SERSIC": 4,
+                    "SRC_GAUSS": 5, "FG_SERSIC": 6, "FG_GAUSS": 7, "FG_SKY": 8}
+    for name, val in enum.items():
+        assert getattr(lensed, name) == val
+    assert list(synth.kind_ids(synth.KINDS)) == list(range(9))
+
+
+def _args():
+    cfg = synth.get_config(0)
+    return dict(image=np.zeros((8, 6), np.float32), weight=np.ones((8, 6), np.float32), mask=None, psf=None,
+                quad=cfg.quad, models=synth.kind_ids(cfg.models), pixel_scale=0.05)
+
+
+@pytest.mark.parametrize("change,status", [
+    (dict(psf=np.ones((4, 3), np.float32)), lensed.EINVAL),            # even PSF side (R11)
+    (dict(psf=np.zeros((3, 3), np.float32)), lensed.EINVAL),           # PSF sums to zero
+    (dict(psf=np.ones((65, 65), np.float32)), lensed.EUNSUPPORTED),
+    (dict(weight=-np.ones((8, 6), np.float32)), lensed.EINVAL),
+    (dict(weight=np.full((8, 6), np.nan, np.float32)), lensed.EINVAL),
+    (dict(image=np.full((8, 6), np.inf, np.float32)), lensed.EINVAL),
+    (dict(pixel_scale=0.0), lensed.EINVAL),
+    (dict(models=np.array([0, 17], np.int32)), lensed.EINVAL),
+    (dict(models=np.zeros(40, np.int32)), lensed.EUNSUPPORTED),
+    (dict(quad=np.zeros((300, 3), np.float32)), lensed.EUNSUPPORTED),
+    (dict(quad=np.array([[0, 0, 1.0], [0, 0, -1.0]], np.float32)), lensed.EINVAL),   # weights sum to 0
+])
+def test_create_validates_arguments_before_touching_cuda(change, status):
+    a = _args()
+    a.update(change)
+    with pytest.raises(lensed.LensedError) as e:
+        lensed.lensed_create(**a)
+    assert e.value.status == status, str(e.value)
+
+
+def test_null_handles_are_rejected_not_dereferenced():
+    L = lensed.lib()
+    assert L.lensed_num_params(None) == -1 and L.lensed_num_traced(None) == -1
+    assert L.lensed_loglike(None, None, 1, None, None) == lensed.EINVAL
+    assert L.lensed_render_host(None, None, 1, None, None) == lensed.EINVAL
+    assert L.lensed_set_profiling(None, 1) == lensed.EINVAL
+    L.lensed_destroy(None)
+
+
+def test_no_cuda_device_fails_loudly_there_is_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(lensed.LensedError) as e:
+        lensed.lensed_create(**_args())
+    assert e.value.status == lensed.ECUDA and "no CPU fallback" in str(e.value)
+    with pytest.raises(lensed.LensedError):
+        lensed.lensed_fma_peak(0, 16)
+
+
+def test_product_code_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1505_07674_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h", ".cuh")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "lensed_oracle" not in text and "import oracle" not in text and "from oracle" not in text, f
