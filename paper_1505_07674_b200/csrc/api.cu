@@ -208,6 +208,8 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
             ta.L = h->d_L;
             ta.l_stride = (long long)HW;
             ta.npix = npix; ta.nq_pad = h->nq_pad; ta.W = h->W;
+            // a block amortises its prologue (constants + frame tables) over this many pixels
+            ta.pix_per_block = npix >= (1 << 16) ? 2048 : npix >= (1 << 13) ? 1024 : 256;
             ta.cxh = 0.5f * (h->W - 1); ta.cyh = 0.5f * (h->H - 1);
             if ((s = timed_begin(h, PH_TRACE, st)) != LENSED_OK) return s;
             CU(h, launch_trace(prog, ta, h->R, nb, st));
@@ -324,6 +326,15 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
         D += kind_num_derived(k);
     }
     pg.P = P; pg.D = D;
+    // shears to the front of the lens list (stable): the first one initialises alpha in the
+    // tracer; the sum over lenses does not depend on the order beyond rounding
+    {
+        uint8_t kk[kMaxModels]; uint16_t oo[kMaxModels]; int n = 0;
+        for (int pass = 0; pass < 2; ++pass)
+            for (int m = 0; m < pg.n_lens; ++m)
+                if ((pg.lens_kind[m] == K_SHEAR) == (pass == 0)) { kk[n] = pg.lens_kind[m]; oo[n++] = pg.lens_off[m]; }
+        for (int m = 0; m < pg.n_lens; ++m) { pg.lens_kind[m] = kk[m]; pg.lens_off[m] = oo[m]; }
+    }
 
     // rule: weights to unit sum in double, padded with zero-weight points to a multiple of R
     double wsum = 0.0;

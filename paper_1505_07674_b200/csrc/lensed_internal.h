@@ -18,7 +18,8 @@ namespace lensed {
 // by ONE rounding at the magnitude of the component-relative offset.
 //
 //  SIS    [c0][b, 0, 0, 0]                                              8
-//  SIE    [c0][cos, sin, q^2, q'][b*sqrt(q), b*sqrt(q)/q', 0, 0]        12
+//  SIE    [c0][cos, sin, q^2, q'][cos A, sin A, cos A l, -sin A l]      12
+//         A = b sqrt(q)/q' with q' floored at 1e-4, l = ln(2)/2 (trace.cu lens_sie)
 //  POINT  [c0][thetaE^2, 0, 0, 0]                                       8
 //  SHEAR  [g1, g2, 0, 0]                                                4
 //  SERSIC [c0][a1, a2, a3, a4][log2 I0, b_n*log2(e), 1/(2n), 0]         12
@@ -74,10 +75,11 @@ struct PrepArgs {
 struct TraceArgs {
     const float *derived;  // [.][D], already offset to the chunk's first vector
     const uint32_t *pix;   // [npix] packed (row << 16) | column
-    const float4 *quad;    // [nq_pad] (xi, eta, w, 0), zero-weight padding up to a multiple of R
+    const float4 *quad;    // [nq_pad] (xi, eta, w, 0), zero-weight padding up to a multiple of R (even)
     float *L;              // [.][H*W], chunk-local
     long long l_stride;    // H*W
     int npix, nq_pad, W;
+    int pix_per_block;     // pixels of the list one block walks (a multiple of 256)
     float cxh, cyh;
 };
 
@@ -110,6 +112,7 @@ cudaError_t launch_conv(const ConvArgs &a, bool render, int nvec, cudaStream_t s
 cudaError_t launch_final(const FinalArgs &a, cudaStream_t st);
 cudaError_t conv_setup();                 // one-time function attributes
 int trace_pick_R(int n_quad);             // rays per register block for an n_quad-point rule
+size_t trace_smem_bytes(const Program &prog, int nq_pad);
 void conv_tile_shape(int *tile_w, int *tile_h);
 size_t conv_smem_bytes(int KH, int NC);
 cudaError_t run_fma_peak(int iters, double *tflops);

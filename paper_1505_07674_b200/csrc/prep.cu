@@ -3,7 +3,8 @@
 // One thread per parameter vector.  Everything the ray tracer would otherwise recompute per
 // ray is evaluated once here, in double, and rounded to FP32 once:
 //   * component centres as (integer pixel, fraction)
-//   * SIE: cos/sin PA, q^2, q' = sqrt(1-q^2), b sqrt(q)        (R2)
+//   * SIE: cos/sin PA, q^2, q' = sqrt(1-q^2), A = b sqrt(q)/q' folded into the rotation
+//     back to the image frame                                  (R2)
 //   * Sersic: b_n from P(2n, b_n) = 1/2 (r_S is the half-light radius; R5),
 //     log2 I_0 from the total magnitude (R6), the rotated, q-stretched,
 //     r_S-scaled frame of eq. 23
@@ -121,10 +122,13 @@ __global__ void __launch_bounds__(128) prep_kernel(Program prog, PrepArgs a)
             sincos(p[4] * (kPi / 180.0), &s, &c);
             d[4] = (float)c; d[5] = (float)s;
             d[6] = (float)(q * q);
-            d[7] = (float)sqrt((1.0 - q) * (1.0 + q));
-            const double qp = sqrt((1.0 - q) * (1.0 + q)), bq = p[2] / a.scale * sqrt(q);
-            d[8] = (float)bq;
-            d[9] = (float)(bq / fmax(qp, 0.4));   // only used where q' |v|/psi >= 0.4
+            // q' floored: A atan(q' u/psi) -> b sqrt(q) u/psi as q' -> 0 with relative
+            // deviation q'^2/3, so the floor changes nothing above 3e-9 and A stays finite
+            const double qp = fmax(sqrt((1.0 - q) * (1.0 + q)), 1e-4);
+            const double A = p[2] / a.scale * sqrt(q) / qp;
+            d[7] = (float)qp;
+            d[8] = (float)(c * A); d[9] = (float)(s * A);
+            d[10] = (float)(c * A * (0.5 * kLn2)); d[11] = (float)(-s * A * (0.5 * kLn2));
             break;
         }
         case K_SRC_SERSIC: case K_FG_SERSIC: {
