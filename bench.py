@@ -205,7 +205,8 @@ def main():
     image, weight = make_observation_cuda(cfg, local)
     kinds = synth.kind_ids(cfg.models)
     h = lensed.lensed_create(image, weight, cfg.mask, cfg.psf, cfg.quad, kinds, cfg.scale, cfg.zp, local)
-    n_traced = lensed.lensed_num_traced(h)
+    n_traced = cfg.n_traced()                               # m_d, the required set
+    assert n_traced <= lensed.lensed_num_traced(h)
     n_counted = int(cfg.H * cfg.W if cfg.mask is None else cfg.mask.sum())
 
     params = cfg.batch(B, stream=2 + rank)                 # this rank's shard of the global batch

@@ -102,7 +102,9 @@ lensed_status lensed_create(int H, int W, double pixel_scale,
 int lensed_num_params(const lensed_handle *h);
 
 /* Pixels lensed_loglike ray-traces per vector: the unmasked set dilated by the PSF
- * window with border clamping (R8); H*W without a mask.  -1 for NULL.                   */
+ * window with border clamping (R8) plus one guard row above and below every window
+ * (an implementation margin; the result does not depend on it); H*W without a mask.
+ * -1 for NULL.                                                                           */
 int lensed_num_traced(const lensed_handle *h);
 
 /*

@@ -351,11 +351,13 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     for (int k = 0; k < n_quad; ++k)
         hq[k] = make_float4(quad[3 * k], quad[3 * k + 1], (float)((double)quad[3 * k + 2] / wsum), 0.f);
 
-    // PSF: normalise in double, flip (eq. 15 uses F_{-k,-l}), pad rows to 4-tap chunks
+    // PSF: normalise in double, flip (eq. 15 uses F_{-k,-l}) -> G[KH][KW]; the convolution
+    // reads tap PAIRS  Q[j][c][k] = (G[j][4c+k], G[j-1][4c+k]),  j = 0..KH, G[-1] = G[KH] = 0,
+    // columns zero padded to 4-tap chunks (conv.cu "Pairing")
     h->KH = has_psf ? psf_h : 1;
     h->KW = has_psf ? psf_w : 1;
     h->NC = (h->KW + 3) / 4;
-    std::vector<float> taps((size_t)h->KH * 4 * h->NC, 0.0f);
+    std::vector<float> G((size_t)h->KH * h->KW, 1.0f);
     if (has_psf) {
         double fsum = 0.0;
         for (int t = 0; t < psf_h * psf_w; ++t) {
@@ -365,16 +367,23 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
         if (!(fabs(fsum) > 0.0)) { delete h; return fail(nullptr, LENSED_EINVAL, "PSF sums to zero"); }
         for (int ky = 0; ky < psf_h; ++ky)
             for (int kx = 0; kx < psf_w; ++kx)
-                taps[(size_t)ky * 4 * h->NC + kx] =
+                G[(size_t)ky * psf_w + kx] =
                     (float)((double)psf[(size_t)(psf_h - 1 - ky) * psf_w + (psf_w - 1 - kx)] / fsum);
-    } else {
-        taps[0] = 1.0f;
     }
+    std::vector<float> taps((size_t)(h->KH + 1) * h->NC * 8, 0.0f);
+    for (int j = 0; j <= h->KH; ++j)
+        for (int kx = 0; kx < h->KW; ++kx) {
+            float *pair = &taps[((size_t)j * h->NC + kx / 4) * 8 + 2 * (kx % 4)];
+            if (j < h->KH) pair[0] = G[(size_t)j * h->KW + kx];
+            if (j > 0) pair[1] = G[(size_t)(j - 1) * h->KW + kx];
+        }
 
     // pixel lists and tile lists
     conv_tile_shape(&h->tile_w, &h->tile_h);
     std::vector<uint32_t> pix_ll, pix_all, tiles_ll, tiles_all;
-    pixel_list(dilate(counted, H, W, (h->KH - 1) / 2, (h->KW - 1) / 2), H, W, pix_ll);
+    // traced set: the PSF windows of the counted pixels, one more row each way because a
+    // counted row's pair partner multiplies its first / last window row by a zero tap
+    pixel_list(dilate(counted, H, W, (h->KH - 1) / 2 + 1, (h->KW - 1) / 2), H, W, pix_ll);
     pixel_list(all, H, W, pix_all);
     tile_list(counted, H, W, h->tile_w, h->tile_h, tiles_ll);
     tile_list(all, H, W, h->tile_w, h->tile_h, tiles_all);

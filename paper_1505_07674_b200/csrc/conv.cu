@@ -4,65 +4,82 @@
 //   L*_ij = sum_{k=-p..p} sum_{l=-q..q} F_{-k,-l} L_{clamp(i+k), clamp(j+l)}   PAPER.md:159-164 eq. 15
 //   loglike = -1/2 sum_i w_i (d_i - L*_i)^2                                    PAPER.md:178-182 eq. 17
 //
-// FP32 direct convolution on the FMA pipe (not a GEMM: DESIGN.md "why no tensor cores").
+// FP32 direct convolution on the FMA pipe (not a GEMM: DESIGN.md "why no tensor cores"),
+// written on packed pairs (FFMA2, f32x2.cuh): one issue slot per two multiply-adds.
 // blockIdx.y = parameter vector, blockIdx.x = active output tile (tiles with no unmasked
-// pixel are not launched).  A block stages its input tile with the PSF halo in shared
-// memory (border pixels repeated, L164) next to the pre-flipped, normalised taps, then each
-// thread accumulates a kTR x 4 register tile of outputs:
+// pixel are not launched).  A block stages its 64 x 128 input tile with the PSF halo in shared
+// memory (border pixels repeated, L164) next to the tap pairs, then each thread accumulates
+// 4 rows x 8 columns of outputs (two 4-column groups 64 columns apart, so that the 8 lanes
+// of a quarter-warp read consecutive 16-byte words: conflict-free LDS.128).
+//
+// Pairing.  A register pair holds the SAME column of two vertically adjacent output rows
+// (o, o+1).  At input row r they need tap rows r-o and r-o-1, so the pair multiplies the
+// broadcast scalar in[r][x+k] by the tap pair  Q[j][k] = (G[j][k], G[j-1][k]),  j = r-o,
+// G = flipped normalised PSF, G[-1] = G[KH] = 0.  Q is built on the host (api.cu) and sits
+// in shared memory; both operands of the FFMA2 come as they are loaded -- no shuffling of
+// register halves.  The thread's two row pairs (rows 0-1, 2-3) use Q[r] and Q[r-2].
 //
 //   loop over tap-column chunks c (4 taps each)
-//     loop over input rows r of the thread's strip (kTR + KH - 1 of them)
-//       2 x LDS.128  input  in[r][4 tx + 4c .. + 7]          (conflict-free: 8 lanes = 128 B)
-//       1 x LDS.128  taps   G[r][4c .. 4c+3]                 (broadcast)
-//       kTR x 16 FFMA: output row o uses tap row ky = r - o
+//     loop over input rows r of the thread's strip (KH + 3 of them)
+//       4 x LDS.128  input  in[r][4 tx + 4c .. +7]  and  .. + 64        (conflict-free)
+//       4 x LDS.128  taps   Q[r][c], Q[r-2][c]                          (broadcast)
+//       64 x FFMA2
 //
-// The tap row used by output row o at input row r is the one row o+1 uses at r+1, so the
-// tap vectors live in kTR register slots indexed by (ky mod kTR) and the row loop is
-// unrolled by kTR ("super-step") to make every slot index static.  Super-steps whose tap
-// rows are all inside the PSF run branch-free; the first and last ones test each (row, o)
-// pair with block-uniform branches, so no multiply by a padded zero is ever issued in y.
+// Zero padding exists only in the tap columns (KW -> multiple of 4) and in the first / last
+// tap row of each pair; the staged input is zero beyond the KW-1 halo columns, and the traced
+// set is dilated by p+1 rows (api.cu), so a zero tap never meets an untraced value.
+// Summation is blocked (per chunk, then across chunks): FP32 error growth ~ sqrt(4 KH) + sqrt(NC).
 //
-// Epilogue: loglike -> per-thread FP32 sum over its 4 kTR pixels, then FP64: warp shuffle
+// Epilogue: loglike -> per-thread FP32 sum over its 32 pixels, then FP64: warp shuffle
 // tree, the block's warps, and one FP64 partial per (vector, tile), summed in a fixed
 // order by final_kernel: bitwise reproducible, no float atomics.
 #include "lensed_internal.h"
+#include "f32x2.cuh"
 #include <math.h>
 
 namespace lensed {
 namespace {
 
-constexpr int kTR = 4;                 // output rows per thread
+constexpr int kTR = 4;                 // output rows per thread (two pairs)
 constexpr int kNTX = 16, kNTY = 16;    // threads per block in x / y (warps are 8 x 4 threads)
 constexpr int kThreads = kNTX * kNTY;
-constexpr int kTW = 4 * kNTX;          // 64 output columns per tile
+constexpr int kGroup = 4 * kNTX;       // 64: distance of a thread's two column groups
+constexpr int kTW = 2 * kGroup;        // 128 output columns per tile
 constexpr int kTH = kTR * kNTY;        // 64 output rows per tile
 
-__device__ __forceinline__ void fma16(float (&acc)[4], const float4 &t, const float4 &v0, const float4 &v1)
-{
-    const float v[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
-    const float tp[4] = {t.x, t.y, t.z, t.w};
-#pragma unroll
-    for (int k = 0; k < 4; ++k)
-#pragma unroll
-        for (int e = 0; e < 4; ++e) acc[e] = fmaf(tp[k], v[e + k], acc[e]);
-}
+__device__ __forceinline__ f2 as_f2(unsigned long long v) { f2 r; r.v = v; return r; }
 
-// One super-step: input rows r = g kTR + s, s = 0..kTR-1.  EDGE = test the tap rows.
-template <bool EDGE>
-__device__ __forceinline__ void super_step(float (&acc)[kTR][4], float4 (&T)[kTR], const float4 *in_row,
-                                           const float4 *tap_c, int g, int KH, int NC, int IW4)
+// One input row r of the thread's strip against one 4-tap chunk.  P0 / P1: row pair 0 (tap
+// pairs Q[r]) / row pair 1 (Q[r-2]) takes part.  in_r -> in[r][4 tx + 4 c], q0 -> Q[r][c],
+// q1 -> Q[r-2][c].
+template <bool P0, bool P1>
+__device__ __forceinline__ void row_step(f2 (&part)[2][8], const float4 *in_r, const ulonglong2 *q0,
+                                         const ulonglong2 *q1)
 {
+    const float4 a0 = in_r[0], a1 = in_r[1], b0 = in_r[kGroup / 4], b1 = in_r[kGroup / 4 + 1];
+    const float va[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+    const float vb[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+    if (P0) {
+        const ulonglong2 t0 = q0[0], t1 = q0[1];
+        const f2 q[4] = {as_f2(t0.x), as_f2(t0.y), as_f2(t1.x), as_f2(t1.y)};
 #pragma unroll
-    for (int s = 0; s < kTR; ++s) {
-        const int r = g * kTR + s;
-        if (EDGE && r >= KH + kTR - 1) break;
-        const float4 v0 = in_row[(size_t)r * IW4], v1 = in_row[(size_t)r * IW4 + 1];
-        if (!EDGE || r < KH) T[s] = tap_c[r * NC];
+        for (int k = 0; k < 4; ++k)
 #pragma unroll
-        for (int o = 0; o < kTR; ++o) {
-            const int ky = r - o;
-            if (!EDGE || (ky >= 0 && ky < KH)) fma16(acc[o], T[(s - o + kTR) % kTR], v0, v1);
-        }
+            for (int e = 0; e < 4; ++e) {
+                part[0][e] = fma2(q[k], bc(va[e + k]), part[0][e]);
+                part[0][4 + e] = fma2(q[k], bc(vb[e + k]), part[0][4 + e]);
+            }
+    }
+    if (P1) {
+        const ulonglong2 t0 = q1[0], t1 = q1[1];
+        const f2 q[4] = {as_f2(t0.x), as_f2(t0.y), as_f2(t1.x), as_f2(t1.y)};
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                part[1][e] = fma2(q[k], bc(va[e + k]), part[1][e]);
+                part[1][4 + e] = fma2(q[k], bc(vb[e + k]), part[1][4 + e]);
+            }
     }
 }
 
@@ -70,34 +87,34 @@ template <bool RENDER>
 __global__ void __launch_bounds__(kThreads, 2) conv_kernel(ConvArgs a)
 {
     extern __shared__ float4 smem4[];
-    const int IW = kTW + 4 * a.NC, IW4 = IW / 4;
+    const int IW4 = kTW / 4 + a.NC, IW = 4 * IW4;
     const int IH = kTH + a.KH - 1;
-    float *s_in = reinterpret_cast<float *>(smem4);                 // [IH][IW]
-    float4 *s_tap = smem4 + (size_t)IH * IW4;                       // [KH][NC]
+    float *s_in = reinterpret_cast<float *>(smem4);                                    // [IH][IW]
+    ulonglong2 *s_q = reinterpret_cast<ulonglong2 *>(smem4 + (size_t)IH * IW4);        // [KH+1][NC][2]
     __shared__ double s_red[kThreads / 32];
 
     const int bvec = blockIdx.y;
     const uint32_t tile = a.tiles[blockIdx.x];
     const int Y0 = (int)(tile >> 16) * kTH, X0 = (int)(tile & 0xffffu) * kTW;
     const float *Lb = a.L + (size_t)bvec * a.l_stride;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
-    // stage taps and the clamped input tile
+    // stage the tap pairs and the clamped input tile (zero beyond the KW-1 halo columns)
     {
-        const float4 *gt = reinterpret_cast<const float4 *>(a.taps);
-        for (int i = threadIdx.x; i < a.KH * a.NC; i += kThreads) s_tap[i] = gt[i];
-        const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+        const ulonglong2 *gq = reinterpret_cast<const ulonglong2 *>(a.taps);
+        for (int i = threadIdx.x; i < (a.KH + 1) * a.NC * 2; i += kThreads) s_q[i] = gq[i];
+        const int used = kTW + a.KW - 1;
         for (int r = warp; r < IH; r += kThreads / 32) {
             const int y = min(max(Y0 - a.p + r, 0), a.H - 1);
             const float *src = Lb + (size_t)y * a.W;
             for (int c = lane; c < IW; c += 32) {
                 const int x = min(max(X0 - a.q + c, 0), a.W - 1);
-                s_in[r * IW + c] = src[x];
+                s_in[r * IW + c] = c < used ? src[x] : 0.0f;
             }
         }
     }
     __syncthreads();
 
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int tx = (warp & 1) * 8 + (lane & 7);
     const int ty = (warp >> 1) * 4 + (lane >> 3);
     const int oy = Y0 + ty * kTR, ox = X0 + tx * 4;
@@ -110,50 +127,55 @@ __global__ void __launch_bounds__(kThreads, 2) conv_kernel(ConvArgs a)
 #pragma unroll
         for (int o = 0; o < kTR; ++o)
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const int y = oy + o, x = ox + e;
+            for (int e = 0; e < 8; ++e) {
+                const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
                 if (y < a.H && x < a.W) any = any || a.wmask[(size_t)y * a.W + x] != 0.0f;
             }
     }
     const bool warp_any = __any_sync(0xffffffffu, any);
 
-    // acc: running sum over tap-column chunks; part: the current chunk (blocked summation:
-    // a chunk adds 4 KH products, the running sum adds NC chunk totals)
-    float acc[kTR][4];
+    // acc[pair][column]: running sum over tap-column chunks; part: the current chunk
+    f2 acc[2][8];
 #pragma unroll
-    for (int o = 0; o < kTR; ++o)
+    for (int p = 0; p < 2; ++p)
 #pragma unroll
-        for (int e = 0; e < 4; ++e) acc[o][e] = 0.0f;
+        for (int e = 0; e < 8; ++e) acc[p][e] = bc(0.0f);
 
     if (warp_any) {
-        const int S = a.KH + kTR - 1;              // input rows per thread strip
-        const int G = (S + kTR - 1) / kTR;         // super-steps
-        const int g_hi = a.KH / kTR - 1;           // steady super-steps are 1 .. g_hi
+        const int KH = a.KH, NC2 = 2 * a.NC;
         const float4 *in_base = reinterpret_cast<const float4 *>(s_in) + (size_t)(ty * kTR) * IW4 + tx;
 #pragma unroll 1
         for (int c = 0; c < a.NC; ++c) {
-            float part[kTR][4];
-            float4 T[kTR];
+            f2 part[2][8];
 #pragma unroll
-            for (int s = 0; s < kTR; ++s) {
-                T[s] = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int p = 0; p < 2; ++p)
 #pragma unroll
-                for (int e = 0; e < 4; ++e) part[s][e] = 0.0f;
+                for (int e = 0; e < 8; ++e) part[p][e] = bc(0.0f);
+            const float4 *in_r = in_base + c;
+            const ulonglong2 *q_r = s_q + 2 * c;
+            row_step<true, false>(part, in_r, q_r, nullptr);
+            row_step<true, false>(part, in_r + IW4, q_r + NC2, nullptr);
+            in_r += 2 * IW4;
+#pragma unroll 2
+            for (int r = 2; r <= KH; ++r) {
+                row_step<true, true>(part, in_r, q_r + 2 * NC2, q_r);
+                in_r += IW4;
+                q_r += NC2;
             }
-            const float4 *in_c = in_base + c;
-            const float4 *tap_c = s_tap + c;
-            super_step<true>(part, T, in_c, tap_c, 0, a.KH, a.NC, IW4);
-            int g = 1;
-#pragma unroll 1
-            for (; g <= g_hi; ++g) super_step<false>(part, T, in_c, tap_c, g, a.KH, a.NC, IW4);
-#pragma unroll 1
-            for (; g < G; ++g) super_step<true>(part, T, in_c, tap_c, g, a.KH, a.NC, IW4);
+            row_step<false, true>(part, in_r, nullptr, q_r);
+            row_step<false, true>(part, in_r + IW4, nullptr, q_r + NC2);
 #pragma unroll
-            for (int o = 0; o < kTR; ++o)
+            for (int p = 0; p < 2; ++p)
 #pragma unroll
-                for (int e = 0; e < 4; ++e) acc[o][e] += part[o][e];
+                for (int e = 0; e < 8; ++e) acc[p][e] = add2(acc[p][e], part[p][e]);
         }
     }
+
+    float out[kTR][8];
+#pragma unroll
+    for (int p = 0; p < 2; ++p)
+#pragma unroll
+        for (int e = 0; e < 8; ++e) un2(acc[p][e], out[2 * p][e], out[2 * p + 1][e]);
 
     if (RENDER) {
         const bool valid = a.derived[(size_t)bvec * a.D] != 0.0f;
@@ -161,9 +183,9 @@ __global__ void __launch_bounds__(kThreads, 2) conv_kernel(ConvArgs a)
 #pragma unroll
         for (int o = 0; o < kTR; ++o)
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const int y = oy + o, x = ox + e;
-                if (y < a.H && x < a.W) mb[(size_t)y * a.W + x] = valid ? acc[o][e] : nanf("");
+            for (int e = 0; e < 8; ++e) {
+                const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
+                if (y < a.H && x < a.W) mb[(size_t)y * a.W + x] = valid ? out[o][e] : nanf("");
             }
     } else {
         float part = 0.0f;
@@ -171,13 +193,13 @@ __global__ void __launch_bounds__(kThreads, 2) conv_kernel(ConvArgs a)
 #pragma unroll
             for (int o = 0; o < kTR; ++o)
 #pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int y = oy + o, x = ox + e;
+                for (int e = 0; e < 8; ++e) {
+                    const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
                     if (y < a.H && x < a.W) {
                         const size_t i = (size_t)y * a.W + x;
                         const float w = a.wmask[i];
                         if (w != 0.0f) {                   // masked pixels may see untraced L: never touch them
-                            const float diff = a.image[i] - acc[o][e];
+                            const float diff = a.image[i] - out[o][e];
                             part = fmaf(w * diff, diff, part);
                         }
                     }
@@ -215,7 +237,7 @@ void conv_tile_shape(int *tile_w, int *tile_h) { *tile_w = kTW; *tile_h = kTH; }
 size_t conv_smem_bytes(int KH, int NC)
 {
     const size_t IW = kTW + 4 * NC, IH = kTH + KH - 1;
-    return (IH * IW + (size_t)KH * 4 * NC) * sizeof(float);
+    return (IH * IW + (size_t)(KH + 1) * 8 * NC) * sizeof(float);
 }
 
 cudaError_t conv_setup()

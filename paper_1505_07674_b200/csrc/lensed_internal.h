@@ -85,7 +85,7 @@ struct TraceArgs {
 
 struct ConvArgs {
     const float *L;        // [.][H*W] chunk-local unconvolved images
-    const float *taps;     // [KH][4*NC] flipped, normalised PSF rows, zero padded columns
+    const float *taps;     // [KH+1][NC][4][2] tap pairs (G[j][k], G[j-1][k]) of the flipped, normalised PSF (conv.cu)
     const float *image;    // [H*W] d
     const float *wmask;    // [H*W] w_i, 0 where masked
     const uint32_t *tiles; // [n_tiles] packed (tile row << 16) | tile column (active tiles)

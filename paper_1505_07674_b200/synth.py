@@ -206,19 +206,21 @@ class Config:
         w = np.broadcast_to(1.0 / var, t.shape)
         return (t + noise).astype(np.float32), np.ascontiguousarray(w, dtype=np.float32)
 
-    def n_traced(self):
-        """m_d: pixels in the PSF-dilated unmasked set (what loglike must ray-trace)."""
+    def n_traced(self, extra_rows=0):
+        """m_d: pixels in the PSF-dilated unmasked set (what loglike must ray-trace);
+        extra_rows widens every window by that many rows each way."""
         if self.mask is None:
             return self.H * self.W
-        return int(dilate_mask(self.mask, self.psf).sum())
+        return int(dilate_mask(self.mask, self.psf, extra_rows).sum())
 
 
-def dilate_mask(mask, psf):
+def dilate_mask(mask, psf, extra_rows=0):
     """Pixels any unmasked pixel's PSF window (with border clamping) touches."""
     m = np.asarray(mask, dtype=bool)
-    if psf is None:
+    if psf is None and not extra_rows:
         return m
-    p, q = (psf.shape[0] - 1) // 2, (psf.shape[1] - 1) // 2
+    p, q = ((psf.shape[0] - 1) // 2, (psf.shape[1] - 1) // 2) if psf is not None else (0, 0)
+    p += extra_rows
     H, W = m.shape
     rows = np.zeros_like(m)
     for k in range(-p, p + 1):                      # unmasked row i reads row clamp(i + k)
