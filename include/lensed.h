@@ -151,6 +151,16 @@ lensed_status lensed_reset_profile(lensed_handle *h);
  * EINVAL if bytes < one image.                                                          */
 lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes);
 
+/* Tracer selection.  The ray tracer exists as one kernel that interprets any model list
+ * and as kernels specialised at compile time for the model lists of BASELINE.json's
+ * configs (same arithmetic, straight-line code).  lensed_create picks the specialised
+ * kernel when the list has one.  lensed_set_static_tracer(h, 0) forces the interpreting
+ * kernel (tests compare the two); (h, 1) re-enables the specialised one and returns
+ * LENSED_EUNSUPPORTED if the list has none.  lensed_get_static_tracer: 1 / 0 = which one
+ * the next call runs, -1 for NULL.                                                      */
+lensed_status lensed_set_static_tracer(lensed_handle *h, int on);
+int lensed_get_static_tracer(const lensed_handle *h);
+
 /*
  * lensed_fma_peak -- FP32 FFMA micro-benchmark used as the measured roofline
  * denominator: runs `iters` dependent-chain FFMAs per thread on a full grid and returns

@@ -13,9 +13,11 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblensed_b200.so")
-SOURCES = ("api.cu", "prep.cu", "trace.cu", "conv.cu", "peak.cu")
-HEADERS = (os.path.join(CSRC, "lensed_internal.h"),
-           os.path.join(os.path.dirname(HERE), "include", "lensed.h"))
+SOURCES = ("api.cu", "prep.cu", "trace.cu", "trace_sig_a.cu", "trace_sig_b.cu", "trace_sig_c.cu",
+           "trace_sig_d.cu", "conv.cu", "peak.cu")
+HEADERS = tuple(os.path.join(CSRC, f) for f in ("lensed_internal.h", "f32x2.cuh", "trace_math.cuh",
+                                                  "trace_block.cuh", "trace_static.cuh")) + (
+           os.path.join(os.path.dirname(HERE), "include", "lensed.h"),)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

@@ -48,6 +48,7 @@ struct lensed_handle {
     float *d_stage_in = nullptr; size_t cap_stage_in = 0;
     float *d_stage_out = nullptr; size_t cap_stage_out = 0;
     long long chunk_bytes = 64ll << 20;
+    bool static_tracer = false;     // the model list has a compile-time-specialised tracer and may use it
 
     // instrumentation
     bool profiling = false;
@@ -212,7 +213,7 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
             ta.pix_per_block = npix >= (1 << 16) ? 2048 : npix >= (1 << 13) ? 1024 : 256;
             ta.cxh = 0.5f * (h->W - 1); ta.cyh = 0.5f * (h->H - 1);
             if ((s = timed_begin(h, PH_TRACE, st)) != LENSED_OK) return s;
-            CU(h, launch_trace(prog, ta, h->R, nb, st));
+            CU(h, launch_trace(prog, ta, h->R, nb, h->static_tracer, st));
             if ((s = timed_end(h, st)) != LENSED_OK) return s;
         }
         if (n_tiles > 0) {
@@ -326,15 +327,25 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
         D += kind_num_derived(k);
     }
     pg.P = P; pg.D = D;
-    // shears to the front of the lens list (stable): the first one initialises alpha in the
-    // tracer; the sum over lenses does not depend on the order beyond rounding
+    // canonical order (stable within a kind): lenses shear, SIE, SIS, point mass -- the first
+    // shear initialises alpha in the tracer; lights source Sersic, source Gaussian, foreground
+    // Sersic, foreground Gaussian, sky.  The sums over lenses and over lights do not depend on
+    // the order beyond rounding; the static tracer kernels index the lists by it (trace_static.cuh).
     {
+        static const int lens_order[] = {K_SHEAR, K_SIE, K_SIS, K_POINT};
+        static const int light_order[] = {K_SRC_SERSIC, K_SRC_GAUSS, K_FG_SERSIC, K_FG_GAUSS, K_SKY};
         uint8_t kk[kMaxModels]; uint16_t oo[kMaxModels]; int n = 0;
-        for (int pass = 0; pass < 2; ++pass)
+        for (int kind : lens_order)
             for (int m = 0; m < pg.n_lens; ++m)
-                if ((pg.lens_kind[m] == K_SHEAR) == (pass == 0)) { kk[n] = pg.lens_kind[m]; oo[n++] = pg.lens_off[m]; }
+                if (pg.lens_kind[m] == kind) { kk[n] = pg.lens_kind[m]; oo[n++] = pg.lens_off[m]; }
         for (int m = 0; m < pg.n_lens; ++m) { pg.lens_kind[m] = kk[m]; pg.lens_off[m] = oo[m]; }
+        n = 0;
+        for (int kind : light_order)
+            for (int m = 0; m < pg.n_light; ++m)
+                if (pg.light_kind[m] == kind) { kk[n] = pg.light_kind[m]; oo[n++] = pg.light_off[m]; }
+        for (int m = 0; m < pg.n_light; ++m) { pg.light_kind[m] = kk[m]; pg.light_off[m] = oo[m]; }
     }
+    h->static_tracer = trace_has_static(pg);
 
     // rule: weights to unit sum in double, padded with zero-weight points to a multiple of R
     double wsum = 0.0;
@@ -484,6 +495,17 @@ lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes)
     h->chunk_bytes = bytes;
     return LENSED_OK;
 }
+
+lensed_status lensed_set_static_tracer(lensed_handle *h, int on)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (on && !trace_has_static(h->prog))
+        return fail(h, LENSED_EUNSUPPORTED, "no specialised tracer for this model list");
+    h->static_tracer = on != 0;
+    return LENSED_OK;
+}
+
+int lensed_get_static_tracer(const lensed_handle *h) { return h ? (h->static_tracer ? 1 : 0) : -1; }
 
 lensed_status lensed_fma_peak(int device, int iters, double *tflops)
 {

@@ -27,12 +27,20 @@ namespace lensed {
 //         so that u'^2 + v'^2 = (R / r_S)^2 with R of PAPER.md:250 eq. 23
 //  GAUSS  [c0][a1, a2, a3, a4][log2 I0, log2(e)/2, 0, 0]                12   (offset / sigma)
 //  SKY    [level, 0, 0, 0]                                              4
-// Block 0 of every vector is the header [valid, 0, 0, 0].
+// Block 0 of every vector is the header [valid, SIE mode, 0, 0]; the mode (trace_math.cuh
+// "SIE") is the most general one any SIE of the vector needs, 0 without an SIE.
 enum Kind : int {
     K_SIS = 0, K_SIE = 1, K_POINT = 2, K_SHEAR = 3,
     K_SRC_SERSIC = 4, K_SRC_GAUSS = 5, K_FG_SERSIC = 6, K_FG_GAUSS = 7, K_SKY = 8,
     K_COUNT = 9
 };
+
+// SIE mode from the axis ratio (thresholds on q^2; table in trace_math.cuh)
+__host__ __device__ inline int sie_mode(double q)
+{
+    const double q2 = q * q;
+    return q2 >= 0.84 ? 0 : q2 >= 0.64 ? 1 : q2 >= 0.5 ? 2 : q2 >= 1.0 / 3.0 ? 3 : q2 >= 0.25 ? 4 : 5;
+}
 
 constexpr int kMaxModels = 32;
 constexpr int kMaxQuad = 256;
@@ -107,7 +115,9 @@ struct FinalArgs {
 
 // launchers (each returns the cudaGetLastError of its launch)
 cudaError_t launch_prep(const Program &prog, const PrepArgs &a, cudaStream_t st);
-cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nvec, cudaStream_t st);
+// allow_static: use the compile-time-specialised kernel when the list has one (trace.cu)
+cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nvec, bool allow_static, cudaStream_t st);
+bool trace_has_static(const Program &prog);
 cudaError_t launch_conv(const ConvArgs &a, bool render, int nvec, cudaStream_t st);
 cudaError_t launch_final(const FinalArgs &a, cudaStream_t st);
 cudaError_t conv_setup();                 // one-time function attributes

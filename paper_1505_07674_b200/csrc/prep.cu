@@ -86,6 +86,7 @@ __global__ void __launch_bounds__(128) prep_kernel(Program prog, PrepArgs a)
     const float *par = a.params + (size_t)b * prog.P;
     float *der = a.derived + (size_t)b * prog.D;
     bool valid = true;
+    int mode = 0;
     for (int i = 0; i < prog.D; ++i) der[i] = 0.0f;
 
     for (int m = 0; m < prog.n_models; ++m) {
@@ -118,6 +119,7 @@ __global__ void __launch_bounds__(128) prep_kernel(Program prog, PrepArgs a)
             valid = valid && p[2] >= 0.0 && q > 0.0 && q <= 1.0;
             if (!valid) break;
             put_centre(d, p[0], p[1], a);
+            mode = max(mode, sie_mode(q));
             double s, c;
             sincos(p[4] * (kPi / 180.0), &s, &c);
             d[4] = (float)c; d[5] = (float)s;
@@ -165,6 +167,7 @@ __global__ void __launch_bounds__(128) prep_kernel(Program prog, PrepArgs a)
         }
     }
     der[0] = valid ? 1.0f : 0.0f;
+    der[1] = (float)mode;
 }
 
 }  // namespace

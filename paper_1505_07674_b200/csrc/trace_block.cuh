@@ -1,0 +1,75 @@
+// trace_block.cuh -- what every ray-tracer kernel shares: block size, the block prologue
+// (constants of the block's parameter vector and its frame tables into shared memory) and
+// the launch helper.  Included by trace.cu (interpreted model list) and trace_static.cuh
+// (model list fixed at compile time).
+//
+// Shared memory of a block: [D/4] float4 derived constants of its vector, then the frame
+// tables  tab[slot][2][nq_pad]  (slot 0 = identity, 1 + m = lens m, 1 + n_lens + m = light
+// m; lenses and lights in the canonical order of api.cu), then the rule weights [nq_pad].
+#pragma once
+#include "trace_math.cuh"
+
+namespace lensed {
+
+constexpr int kTraceThreads = 256;
+
+struct TraceBlock {
+    const float4 *sder;   // derived constants of the vector
+    const float *stab;    // frame tables
+    const float *sw;      // rule weights
+    float sky;            // summed sky levels
+    bool valid;
+};
+
+// Must be called by all threads of the block; ends with a barrier.
+__device__ __forceinline__ TraceBlock trace_prologue(const Program &prog, const TraceArgs &a, float4 *smem4)
+{
+    float4 *sder = smem4;
+    float *stab = reinterpret_cast<float *>(smem4 + prog.D / 4);
+    const int nq = a.nq_pad;
+    const int n_slots = 1 + prog.n_lens + prog.n_light;
+    float *sw = stab + (size_t)n_slots * 2 * nq;
+    {
+        const float4 *g = reinterpret_cast<const float4 *>(a.derived + (size_t)blockIdx.y * prog.D);
+        for (int i = threadIdx.x; i < prog.D / 4; i += kTraceThreads) sder[i] = g[i];
+    }
+    __syncthreads();
+    TraceBlock tb{sder, stab, sw, 0.0f, sder[0].x != 0.0f};
+    if (!tb.valid) return tb;                     // vector outside the model domain: block-uniform
+    for (int m = 0; m < prog.n_light; ++m)
+        if (prog.light_kind[m] == K_SKY) tb.sky += sder[prog.light_off[m] >> 2].x;
+    for (int i = threadIdx.x; i < n_slots * nq; i += kTraceThreads) {
+        const int slot = i / nq, k = i - slot * nq;
+        const float4 qk = a.quad[k];
+        float m11 = 1.0f, m12 = 0.0f, m21 = 0.0f, m22 = 1.0f;
+        if (slot > 0) {
+            const bool lens = slot <= prog.n_lens;
+            const int m = lens ? slot - 1 : slot - 1 - prog.n_lens;
+            const int kind = lens ? prog.lens_kind[m] : prog.light_kind[m];
+            const float4 *d = sder + ((lens ? prog.lens_off[m] : prog.light_off[m]) >> 2);
+            if (kind == K_SIE) { m11 = d[1].x; m12 = d[1].y; m21 = -d[1].y; m22 = d[1].x; }
+            else if (kind == K_SHEAR) { m11 = d[0].x; m12 = d[0].y; m21 = d[0].y; m22 = -d[0].x; }
+            else if (kind >= K_SRC_SERSIC && kind <= K_FG_GAUSS) { m11 = d[1].x; m12 = d[1].y; m21 = d[1].z; m22 = d[1].w; }
+        }
+        stab[(size_t)(2 * slot) * nq + k] = fmaf(m11, qk.x, m12 * qk.y);
+        stab[(size_t)(2 * slot + 1) * nq + k] = fmaf(m21, qk.x, m22 * qk.y);
+        if (slot == 0) sw[k] = qk.z;
+    }
+    __syncthreads();
+    return tb;
+}
+
+template <class Kernel>
+cudaError_t launch_trace_kernel(Kernel kernel, const Program &prog, const TraceArgs &a, int nvec, cudaStream_t st)
+{
+    const size_t smem = trace_smem_bytes(prog, a.nq_pad);
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    dim3 grid((a.npix + a.pix_per_block - 1) / a.pix_per_block, nvec);
+    kernel<<<grid, kTraceThreads, smem, st>>>(prog, a);
+    return cudaGetLastError();
+}
+
+}  // namespace lensed

@@ -1,0 +1,177 @@
+// trace_static.cuh -- the ray tracer with the model list fixed at compile time.
+//
+// Same computation and layout as trace.cu (steps a1-a4, eqs. 1-2
+// eq. 14), but the lens / light lists are a template signature, so one pass over R rays is
+// straight-line code: no switch per model, no list indexing, and ptxas interleaves the
+// MUFU-heavy light profiles with the FMA-heavy SIE polynomials inside one warp (the
+// interpreted kernel serialises them: profiles/r1c).  Per-pixel frame origins are computed
+// once per pixel, not once per pass.  api.cu sorts the lists into the canonical order
+//   lenses: shear, SIE, SIS, point mass        lights: source Sersic, source Gaussian,
+//                                                      foreground Sersic, foreground Gaussian, sky
+// and trace.cu picks the static kernel whose signature matches, else the interpreted one.
+#pragma once
+#include "trace_block.cuh"
+
+namespace lensed {
+
+template <int NSHEAR, int NSIE, int NSIS, int NPOINT, int NSS, int NSG, int NFS, int NFG>
+struct TraceSig {
+    static_assert(NSHEAR <= 1, "at most one shear in a static signature");
+    static constexpr int n_shear = NSHEAR, n_sie = NSIE, n_sis = NSIS, n_point = NPOINT;
+    static constexpr int n_ss = NSS, n_sg = NSG, n_fs = NFS, n_fg = NFG;
+    static constexpr int n_lens = NSHEAR + NSIE + NSIS + NPOINT;
+    static constexpr int n_pos = NSS + NSG + NFS + NFG;          // positioned lights (sky excluded)
+    static bool matches(const int (&c)[K_COUNT])
+    {
+        return c[K_SHEAR] == NSHEAR && c[K_SIE] == NSIE && c[K_SIS] == NSIS && c[K_POINT] == NPOINT &&
+               c[K_SRC_SERSIC] == NSS && c[K_SRC_GAUSS] == NSG && c[K_FG_SERSIC] == NFS && c[K_FG_GAUSS] == NFG;
+    }
+};
+
+template <int NP, class S, int MODE>
+__device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArgs &a, const TraceBlock &tb, float *Lb)
+{
+    constexpr int R = 2 * NP;
+    constexpr int NL = S::n_lens, NPOS = S::n_pos;
+    constexpr int L_SIE = S::n_shear, L_SIS = L_SIE + S::n_sie, L_PT = L_SIS + S::n_sis;
+    constexpr int G_SG = S::n_ss, G_FS = G_SG + S::n_sg, G_FG = G_FS + S::n_fs;
+    const int nq = a.nq_pad;
+    const float4 *sder = tb.sder;
+    const float *ltab = tb.stab + 2 * nq;                     // lens m: rows 2m, 2m+1
+    const float *gtab = tb.stab + (size_t)(2 * (1 + NL)) * nq; // light m
+
+    const int base = blockIdx.x * a.pix_per_block;
+    const int end = min(base + a.pix_per_block, a.npix);
+#pragma unroll 1
+    for (int ip = base + threadIdx.x; ip < end; ip += kTraceThreads) {
+        const uint32_t rc = a.pix[ip];
+        const int row = (int)(rc >> 16), col = (int)(rc & 0xffffu);
+        const float jf = (float)col, rf = (float)row;
+
+        // frame origins of this pixel
+        float lu[NL > 0 ? NL : 1], lv[NL > 0 ? NL : 1], gu[NPOS > 0 ? NPOS : 1], gv[NPOS > 0 ? NPOS : 1];
+        if (S::n_shear) shear_origin(sder + (prog.lens_off[0] >> 2), jf, rf, a.cxh, a.cyh, lu[0], lv[0]);
+#pragma unroll
+        for (int i = 0; i < S::n_sie; ++i)
+            sie_origin(sder + (prog.lens_off[L_SIE + i] >> 2), jf, rf, lu[L_SIE + i], lv[L_SIE + i]);
+#pragma unroll
+        for (int i = 0; i < S::n_sis + S::n_point; ++i)
+            circular_origin(sder + (prog.lens_off[L_SIS + i] >> 2), jf, rf, lu[L_SIS + i], lv[L_SIS + i]);
+#pragma unroll
+        for (int i = 0; i < NPOS; ++i) light_origin(sder + (prog.light_off[i] >> 2), jf, rf, gu[i], gv[i]);
+
+        f2 acc = bc(0.0f);
+#pragma unroll 1
+        for (int q0 = 0; q0 < nq; q0 += R) {
+            Rays<NP> r;
+            if (S::n_shear) {
+                lens_shear<NP, true>(ltab + q0, ltab + nq + q0, lu[0], lv[0], r);
+            } else {
+#pragma unroll
+                for (int k = 0; k < NP; ++k) { r.ax[k] = bc(0.0f); r.ay[k] = bc(0.0f); }
+            }
+#pragma unroll
+            for (int i = 0; i < S::n_sie; ++i) {
+                const int m = L_SIE + i;
+                lens_sie<NP, MODE>(sder + (prog.lens_off[m] >> 2), ltab + (size_t)(2 * m) * nq + q0,
+                                   ltab + (size_t)(2 * m + 1) * nq + q0, lu[m], lv[m], r);
+            }
+            // SIS / point mass: identity frame = slot 0
+#pragma unroll
+            for (int i = 0; i < S::n_sis; ++i) {
+                const int m = L_SIS + i;
+                lens_circular<NP, false>(sder + (prog.lens_off[m] >> 2), tb.stab + q0, tb.stab + nq + q0, lu[m], lv[m], r);
+            }
+#pragma unroll
+            for (int i = 0; i < S::n_point; ++i) {
+                const int m = L_PT + i;
+                lens_circular<NP, true>(sder + (prog.lens_off[m] >> 2), tb.stab + q0, tb.stab + nq + q0, lu[m], lv[m], r);
+            }
+            if (NPOS == 0) {
+#pragma unroll
+                for (int k = 0; k < NP; ++k) r.I[k] = bc(0.0f);
+            }
+            // foreground lights first: they do not wait for the deflection
+#define LENSED_LIGHT(m, SRC, GAUSS, INIT)                                                                     \
+    light_profile<NP, SRC, GAUSS, INIT>(sder + (prog.light_off[m] >> 2), gtab + (size_t)(2 * (m)) * nq + q0, \
+                                        gtab + (size_t)(2 * (m) + 1) * nq + q0, gu[m], gv[m], r)
+            constexpr bool fg_first = S::n_fs + S::n_fg > 0;
+#pragma unroll
+            for (int i = 0; i < S::n_fs; ++i) {
+                if (i == 0) LENSED_LIGHT(G_FS + i, false, false, true);
+                else LENSED_LIGHT(G_FS + i, false, false, false);
+            }
+#pragma unroll
+            for (int i = 0; i < S::n_fg; ++i) {
+                if (i == 0 && S::n_fs == 0) LENSED_LIGHT(G_FG + i, false, true, true);
+                else LENSED_LIGHT(G_FG + i, false, true, false);
+            }
+#pragma unroll
+            for (int i = 0; i < S::n_ss; ++i) {
+                if (i == 0 && !fg_first) LENSED_LIGHT(i, true, false, true);
+                else LENSED_LIGHT(i, true, false, false);
+            }
+#pragma unroll
+            for (int i = 0; i < S::n_sg; ++i) {
+                if (i == 0 && !fg_first && S::n_ss == 0) LENSED_LIGHT(G_SG + i, true, true, true);
+                else LENSED_LIGHT(G_SG + i, true, true, false);
+            }
+#undef LENSED_LIGHT
+            f2 w[NP];
+            load_pairs<NP>(tb.sw + q0, w);
+#pragma unroll
+            for (int k = 0; k < NP; ++k) acc = fma2(w[k], r.I[k], acc);
+        }
+        Lb[row * a.W + col] = (lo2(acc) + hi2(acc)) + tb.sky;
+    }
+}
+
+template <int NP, class S>
+__global__ void __launch_bounds__(kTraceThreads, 2) trace_static_kernel(Program prog, TraceArgs a)
+{
+    extern __shared__ float4 smem4[];
+    const TraceBlock tb = trace_prologue(prog, a, smem4);
+    if (!tb.valid) return;
+    float *Lb = a.L + (size_t)blockIdx.y * a.l_stride;
+    if constexpr (S::n_sie == 0) {
+        trace_pixels<NP, S, 0>(prog, a, tb, Lb);
+    } else {
+        switch ((int)tb.sder[0].y) {              // SieMode of the vector (prep.cu), block-uniform
+        case 0: trace_pixels<NP, S, 0>(prog, a, tb, Lb); break;
+        case 1: trace_pixels<NP, S, 1>(prog, a, tb, Lb); break;
+        case 2: trace_pixels<NP, S, 2>(prog, a, tb, Lb); break;
+        case 3: trace_pixels<NP, S, 3>(prog, a, tb, Lb); break;
+        case 4: trace_pixels<NP, S, 4>(prog, a, tb, Lb); break;
+        default: trace_pixels<NP, S, 5>(prog, a, tb, Lb); break;
+        }
+    }
+}
+
+// R = rays per register block (2 NP); only the R values trace_pick_R can return
+template <class S>
+cudaError_t launch_trace_static(const Program &prog, const TraceArgs &a, int R, int nvec, cudaStream_t st)
+{
+    switch (R) {
+    case 2: return launch_trace_kernel(trace_static_kernel<1, S>, prog, a, nvec, st);
+    case 4: return launch_trace_kernel(trace_static_kernel<2, S>, prog, a, nvec, st);
+    case 6: return launch_trace_kernel(trace_static_kernel<3, S>, prog, a, nvec, st);
+    case 8: return launch_trace_kernel(trace_static_kernel<4, S>, prog, a, nvec, st);
+    case 10: return launch_trace_kernel(trace_static_kernel<5, S>, prog, a, nvec, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+// Defines  bool NAME(counts, prog, args, R, nvec, stream, &err): false if the signature does
+// not match the list's per-kind counts, else launches and sets err.  One per .cu file, so
+// that the signatures compile in parallel (build.py).
+#define LENSED_DEFINE_STATIC_TRACER(NAME, ...)                                                          \
+    bool NAME(const int (&counts)[K_COUNT], const Program &prog, const TraceArgs &a, int R, int nvec,   \
+              cudaStream_t st, cudaError_t *err)                                                        \
+    {                                                                                                   \
+        using S = TraceSig<__VA_ARGS__>;                                                                \
+        if (!S::matches(counts)) return false;                                                          \
+        *err = launch_trace_static<S>(prog, a, R, nvec, st);                                            \
+        return true;                                                                                    \
+    }
+
+}  // namespace lensed

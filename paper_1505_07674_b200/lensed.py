@@ -35,6 +35,8 @@ SYMBOLS = {
     "lensed_get_profile": (_i, [_p, _p, _p]),
     "lensed_reset_profile": (_i, [_p]),
     "lensed_set_chunk_bytes": (_i, [_p, _ll]),
+    "lensed_set_static_tracer": (_i, [_p, _i]),
+    "lensed_get_static_tracer": (_i, [_p]),
     "lensed_fma_peak": (_i, [_i, _i, _p]),
     "lensed_last_error": (_c, [_p]),
     "lensed_destroy": (None, [_p]),
@@ -163,6 +165,14 @@ def lensed_reset_profile(h):
 
 def lensed_set_chunk_bytes(h, nbytes):
     _check(lib().lensed_set_chunk_bytes(h, int(nbytes)), h)
+
+
+def lensed_set_static_tracer(h, on):
+    _check(lib().lensed_set_static_tracer(h, int(bool(on))), h)
+
+
+def lensed_get_static_tracer(h):
+    return lib().lensed_get_static_tracer(h)
 
 
 def lensed_fma_peak(device=0, iters=4096):

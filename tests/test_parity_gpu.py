@@ -38,10 +38,17 @@ def _gpu_eval(L, h, params, H, W, render=True):
     return logl.cpu().numpy(), model
 
 
-def _check(L, prob, params, render=True):
+def _check(L, prob, params, render=True, static=None):
+    """static: None = whatever lensed_create picked; True = require the compile-time
+    specialised tracer; False = force the interpreting one (include/lensed.h)."""
     c = prob.cfg
     h = prob.create()
     try:
+        if static is True:
+            assert L.lensed_get_static_tracer(h) == 1
+        elif static is False:
+            L.lensed_set_static_tracer(h, 0)
+            assert L.lensed_get_static_tracer(h) == 0
         logl_g, model_g = _gpu_eval(L, h, params, c.H, c.W, render)
     finally:
         L.lensed_destroy(h)
@@ -67,6 +74,31 @@ def test_shrunk_configs_span_tiles_and_ragged_tails(L, index, H, W, B):
     cfg = synth.shrunk(synth.get_config(index), H, W, B)
     prob = Problem(cfg)
     _check(L, prob, np.vstack([cfg.batch(), cfg.truth.astype(np.float32)[None]]))
+
+
+@pytest.mark.parametrize("index,H,W,B", [(0, 32, 32, 16), (1, 90, 70, 24), (2, 75, 93, 12), (3, 70, 80, 8), (4, 101, 67, 6)])
+@pytest.mark.parametrize("static", [True, False])
+def test_both_tracers_on_every_config_list(L, index, H, W, B, static):
+    """The model lists of BASELINE.json's configs have a compile-time specialised tracer; the
+    interpreting kernel must give the same answer (both against the oracle)."""
+    cfg = synth.get_config(index)
+    if index > 0:
+        cfg = synth.shrunk(cfg, H, W, B)
+    _check(L, Problem(cfg), cfg.batch(), static=static)
+
+
+@pytest.mark.parametrize("static", [True, False])
+def test_sie_axis_ratio_sweep_covers_every_polynomial_mode(L, static):
+    """The SIE's atan / atanh approximations are chosen per vector from q (trace_math.cuh):
+    thresholds q^2 = 0.84, 0.64, 0.5, 1/3, 0.25; one vector on each side of each, plus the
+    extremes, in the HST-like list (SIE + shear + Sersic source + Sersic lens light + sky)."""
+    cfg = synth.shrunk(synth.get_config(1), 64, 60, 4)
+    assert cfg.models[0] == "sie"
+    iq = 3                                             # SIE parameters: x, y, theta_E, q, PA
+    qs = [1.0, 0.999, 0.93, 0.9, 0.82, 0.78, 0.72, 0.69, 0.6, 0.56, 0.52, 0.48, 0.3, 0.1, 0.03]
+    params = np.tile(cfg.truth.astype(np.float32), (len(qs), 1))
+    params[:, iq] = qs
+    _check(L, Problem(cfg), params, static=static)
 
 
 def test_paper_mock_scenario_gauss_kronrod_rule(L):
