@@ -88,7 +88,10 @@ typedef enum {
  *   out         receives the handle (NULL on failure)
  * Errors: EINVAL for null pointers, non-positive sizes, negative or non-finite weights,
  * non-finite image values at unmasked pixels, bad PSF / rule / kind; ECUDA if there is
- * no usable device.  Synchronous.                                                       */
+ * no usable device; ENOMEM also when the on-chip tap pool is full: the PSFs of the live
+ * handles of a device share 60 KB of constant memory, (psf_h + 1) * 4 ceil(psf_w / 4) * 8
+ * bytes each (8 KB for 31 x 31, 32 KB for 63 x 63), released by lensed_destroy.
+ * Synchronous.                                                                          */
 lensed_status lensed_create(int H, int W, double pixel_scale,
                             const float *image, const float *weight,
                             const unsigned char *mask,
@@ -147,9 +150,13 @@ lensed_status lensed_get_profile(lensed_handle *h, double *ms, long long *launch
 lensed_status lensed_reset_profile(lensed_handle *h);
 
 /* Tuning knob: bytes of device scratch the unconvolved images L[b] of one batch chunk
- * may take (default 64 MiB, so that a chunk stays resident in the 126 MB L2).
- * EINVAL if bytes < one image.                                                          */
+ * may take (default 1 GiB: the buffer costs ~3.5 bytes of traffic per 3500 flops, so
+ * launches are made long rather than L2-resident).  One vector
+ * takes lensed_frame_bytes(h): its image in a frame padded by the PSF half-widths and
+ * rounded up to whole convolution tiles.  EINVAL if bytes < one frame.
+ * lensed_frame_bytes: -1 for NULL.                                                      */
 lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes);
+long long lensed_frame_bytes(const lensed_handle *h);
 
 /* Tracer selection.  The ray tracer exists as one kernel that interprets any model list
  * and as kernels specialised at compile time for the model lists of BASELINE.json's

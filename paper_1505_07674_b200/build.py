@@ -36,12 +36,14 @@ def _stale(target, deps):
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force=False, verbose=False):
-    """Compile what is out of date; returns the path of the shared library."""
+def build(force=False, verbose=False, defines=(), lib=LIB, objdir=None):
+    """Compile what is out of date; returns the path of the shared library.  `defines`
+    (e.g. ("LENSED_TRACE_MIN_BLOCKS=3",)), `lib` and `objdir` make a differently tuned build
+    beside the default one (load it with LENSED_B200_LIB=<path>)."""
     nvcc = _nvcc()
-    objdir = os.path.join(HERE, "build")
+    objdir = objdir or os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
-    extra = ["-Xptxas", "-v"] if verbose else []
+    extra = (["-Xptxas", "-v"] if verbose else []) + ["-D" + d for d in defines]
     jobs = []
     for src in SOURCES:
         s = os.path.join(CSRC, src)
@@ -60,13 +62,13 @@ def build(force=False, verbose=False):
             if r.returncode != 0:
                 raise RuntimeError("nvcc failed: " + " ".join(cmd))
     objs = [os.path.join(objdir, s[:-3] + ".o") for s in SOURCES]
-    if force or jobs or _stale(LIB, objs):
-        cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs
+    if force or jobs or _stale(lib, objs):
+        cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", lib] + objs
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             sys.stderr.write(r.stdout + r.stderr)
             raise RuntimeError("link failed: " + " ".join(cmd))
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":

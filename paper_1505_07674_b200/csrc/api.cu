@@ -10,6 +10,8 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
+#include <utility>
 #include <new>
 #include <string>
 #include <vector>
@@ -34,9 +36,12 @@ struct lensed_handle {
     int n_quad = 0, R = 1, nq_pad = 0;
     int KH = 1, KW = 1, NC = 1;
     int tile_w = 0, tile_h = 0;
+    int Hp = 0, Wp = 0;             // padded frame of the unconvolved images (conv.cu "Input")
+    int n_sm = 1;
+    int tap_off = -1, tap_pairs = 0; // this handle's range of the constant tap pool
 
     // device, immutable after create
-    float *d_image = nullptr, *d_wmask = nullptr, *d_taps = nullptr;
+    float *d_image = nullptr, *d_wmask = nullptr;
     float4 *d_quad = nullptr;
     uint32_t *d_pix_ll = nullptr, *d_pix_all = nullptr, *d_tiles_ll = nullptr, *d_tiles_all = nullptr;
     int npix_ll = 0, npix_all = 0, ntiles_ll = 0, ntiles_all = 0;
@@ -47,7 +52,7 @@ struct lensed_handle {
     double *d_partial = nullptr; size_t cap_partial = 0;
     float *d_stage_in = nullptr; size_t cap_stage_in = 0;
     float *d_stage_out = nullptr; size_t cap_stage_out = 0;
-    long long chunk_bytes = 64ll << 20;
+    long long chunk_bytes = 1ll << 30;
     bool static_tracer = false;     // the model list has a compile-time-specialised tracer and may use it
 
     // instrumentation
@@ -61,6 +66,33 @@ struct lensed_handle {
 };
 
 namespace {
+
+// Constant tap pool (conv.cu c_taps): first-fit ranges per device, in tap pairs.
+struct TapPool {
+    std::mutex mu;
+    std::vector<std::pair<int, int>> used[64];      // (offset, length), sorted by offset
+    int take(int device, int n)
+    {
+        std::lock_guard<std::mutex> g(mu);
+        auto &u = used[device & 63];
+        int off = 0;
+        size_t at = 0;
+        for (; at < u.size(); ++at) {
+            if (u[at].first - off >= n) break;
+            off = u[at].first + u[at].second;
+        }
+        if (off + n > kTapPoolPairs) return -1;
+        u.insert(u.begin() + at, std::make_pair(off, n));
+        return off;
+    }
+    void give(int device, int off)
+    {
+        std::lock_guard<std::mutex> g(mu);
+        auto &u = used[device & 63];
+        for (size_t i = 0; i < u.size(); ++i)
+            if (u[i].first == off) { u.erase(u.begin() + i); return; }
+    }
+} g_tap_pool;
 
 lensed_status fail(lensed_handle *h, lensed_status st, const char *fmt, ...)
 {
@@ -185,12 +217,17 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
     const int n_tiles = render ? h->ntiles_all : h->ntiles_ll;
     const int npix = render ? h->npix_all : h->npix_ll;
 
-    long long per_chunk = std::max<long long>(1, h->chunk_bytes / (long long)(HW * sizeof(float)));
+    const size_t HWp = (size_t)h->Hp * h->Wp;
+    long long per_chunk = std::max<long long>(1, h->chunk_bytes / (long long)(HWp * sizeof(float)));
     const int Bc = (int)std::min<long long>(std::min<long long>(per_chunk, 65535), B);
 
     lensed_status s;
     if ((s = grow(h, &h->d_derived, &h->cap_derived, (size_t)B * prog.D)) != LENSED_OK) return s;
-    if ((s = grow(h, &h->d_L, &h->cap_L, (size_t)Bc * HW)) != LENSED_OK) return s;
+    if ((size_t)Bc * HWp > h->cap_L) {
+        // pad cells no pixel clamps to (tile overhang) are read, never written: keep them zero
+        if ((s = grow(h, &h->d_L, &h->cap_L, (size_t)Bc * HWp)) != LENSED_OK) return s;
+        CU(h, cudaMemsetAsync(h->d_L, 0, (size_t)Bc * HWp * sizeof(float), st));
+    }
     if (!render && (s = grow(h, &h->d_partial, &h->cap_partial, (size_t)B * std::max(n_tiles, 1))) != LENSED_OK)
         return s;
 
@@ -207,8 +244,9 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
             ta.pix = render ? h->d_pix_all : h->d_pix_ll;
             ta.quad = h->d_quad;
             ta.L = h->d_L;
-            ta.l_stride = (long long)HW;
-            ta.npix = npix; ta.nq_pad = h->nq_pad; ta.W = h->W;
+            ta.l_stride = (long long)HWp;
+            ta.npix = npix; ta.nq_pad = h->nq_pad;
+            ta.H = h->H; ta.W = h->W; ta.Wp = h->Wp; ta.px = (h->KW - 1) / 2; ta.py = (h->KH - 1) / 2;
             // a block amortises its prologue (constants + frame tables) over this many pixels
             ta.pix_per_block = npix >= (1 << 16) ? 2048 : npix >= (1 << 13) ? 1024 : 256;
             ta.cxh = 0.5f * (h->W - 1); ta.cyh = 0.5f * (h->H - 1);
@@ -218,20 +256,19 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
         }
         if (n_tiles > 0) {
             ConvArgs ca{};
-            ca.L = h->d_L;
-            ca.taps = h->d_taps;
+            ca.Lp = h->d_L;
             ca.image = h->d_image;
             ca.wmask = h->d_wmask;
             ca.tiles = render ? h->d_tiles_all : h->d_tiles_ll;
             ca.partial = render ? nullptr : h->d_partial + (size_t)b0 * n_tiles;
             ca.model = render ? out_dev + (size_t)b0 * HW : nullptr;
             ca.derived = h->d_derived + (size_t)b0 * prog.D;
-            ca.l_stride = (long long)HW;
+            ca.lp_stride = (long long)HWp;
             ca.D = prog.D;
-            ca.H = h->H; ca.W = h->W; ca.KH = h->KH; ca.KW = h->KW; ca.NC = h->NC; ca.n_tiles = n_tiles;
-            ca.p = (h->KH - 1) / 2; ca.q = (h->KW - 1) / 2;
+            ca.H = h->H; ca.W = h->W; ca.Wp = h->Wp; ca.KH = h->KH; ca.KW = h->KW; ca.NC = h->NC;
+            ca.n_tiles = n_tiles; ca.nb = nb; ca.tap_off = h->tap_off;
             if ((s = timed_begin(h, PH_CONV, st)) != LENSED_OK) return s;
-            CU(h, launch_conv(ca, render, nb, st));
+            CU(h, launch_conv(ca, render, h->n_sm, st));
             if ((s = timed_end(h, st)) != LENSED_OK) return s;
         }
     }
@@ -391,6 +428,7 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
 
     // pixel lists and tile lists
     conv_tile_shape(&h->tile_w, &h->tile_h);
+    conv_padded_shape(H, W, h->KH, h->NC, &h->Hp, &h->Wp);
     std::vector<uint32_t> pix_ll, pix_all, tiles_ll, tiles_all;
     // traced set: the PSF windows of the counted pixels, one more row each way because a
     // counted row's pair partner multiplies its first / last window row by a zero tap
@@ -420,12 +458,24 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
             return fail(nullptr, LENSED_ECUDA, "device %d is sm_%d%d; this library holds sm_100a code only",
                         device, prop.major, prop.minor);
         }
+        h->n_sm = prop.multiProcessorCount;
         e1 = conv_setup();
         if (e1 != cudaSuccess) { delete h; return fail(nullptr, LENSED_ECUDA, "conv_setup: %s", cudaGetErrorString(e1)); }
     }
     CREATE_FAIL(upload(h, &h->d_image, image, HW));
     CREATE_FAIL(upload(h, &h->d_wmask, wmask.data(), HW));
-    CREATE_FAIL(upload(h, &h->d_taps, taps.data(), taps.size()));
+    {
+        // tap pairs into this handle's range of the constant pool (conv.cu "Taps")
+        h->tap_pairs = (int)(taps.size() / 2);
+        h->tap_off = g_tap_pool.take(device, h->tap_pairs);
+        if (h->tap_off < 0) {
+            lensed_destroy(h);
+            return fail(nullptr, LENSED_ENOMEM, "constant tap pool full: %d pairs wanted, pool of %d shared by the live handles",
+                        (int)(taps.size() / 2), kTapPoolPairs);
+        }
+        cudaError_t e2 = conv_upload_taps(taps.data(), h->tap_pairs, h->tap_off);
+        if (e2 != cudaSuccess) { lensed_destroy(h); return fail(nullptr, LENSED_ECUDA, "tap upload: %s", cudaGetErrorString(e2)); }
+    }
     CREATE_FAIL(upload(h, &h->d_quad, hq.data(), hq.size()));
     CREATE_FAIL(upload(h, &h->d_pix_ll, pix_ll.data(), pix_ll.size()));
     CREATE_FAIL(upload(h, &h->d_pix_all, pix_all.data(), pix_all.size()));
@@ -487,11 +537,17 @@ lensed_status lensed_reset_profile(lensed_handle *h)
     return LENSED_OK;
 }
 
+long long lensed_frame_bytes(const lensed_handle *h)
+{
+    return h ? (long long)((size_t)h->Hp * h->Wp * sizeof(float)) : -1;
+}
+
 lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes)
 {
     if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
-    if (bytes < (long long)((size_t)h->H * h->W * sizeof(float)))
-        return fail(h, LENSED_EINVAL, "chunk of %lld bytes holds less than one image", bytes);
+    if (bytes < lensed_frame_bytes(h))
+        return fail(h, LENSED_EINVAL, "chunk of %lld bytes holds less than one padded frame (%lld bytes)", bytes,
+                    lensed_frame_bytes(h));
     h->chunk_bytes = bytes;
     return LENSED_OK;
 }
@@ -530,7 +586,8 @@ void lensed_destroy(lensed_handle *h)
     cudaDeviceSynchronize();
     for (EventPair &ep : h->used) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (EventPair &ep : h->pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
-    cudaFree(h->d_image); cudaFree(h->d_wmask); cudaFree(h->d_taps); cudaFree(h->d_quad);
+    cudaFree(h->d_image); cudaFree(h->d_wmask); cudaFree(h->d_quad);
+    if (h->tap_off >= 0) g_tap_pool.give(h->device, h->tap_off);
     cudaFree(h->d_pix_ll); cudaFree(h->d_pix_all); cudaFree(h->d_tiles_ll); cudaFree(h->d_tiles_all);
     cudaFree(h->d_derived); cudaFree(h->d_L); cudaFree(h->d_partial);
     cudaFree(h->d_stage_in); cudaFree(h->d_stage_out);

@@ -1,33 +1,50 @@
-// conv.cu -- steps a5-a6: direct PSF convolution with replicate padding and, fused into its
-// epilogue, the weighted chi-square.
+// conv.cu -- steps a5-a6: PSF convolution with replicated borders, fused with the weighted
+// chi-square reduction (loglike) or with the store of the model image (render).
 //
 //   L*_ij = sum_{k=-p..p} sum_{l=-q..q} F_{-k,-l} L_{clamp(i+k), clamp(j+l)}   PAPER.md:159-164 eq. 15
 //   loglike = -1/2 sum_i w_i (d_i - L*_i)^2                                    PAPER.md:178-182 eq. 17
 //
 // FP32 direct convolution on the FMA pipe (not a GEMM: DESIGN.md "why no tensor cores"),
 // written on packed pairs (FFMA2, f32x2.cuh): one issue slot per two multiply-adds.
-// blockIdx.y = parameter vector, blockIdx.x = active output tile (tiles with no unmasked
-// pixel are not launched).  A block stages its 64 x 128 input tile with the PSF halo in shared
-// memory (border pixels repeated, L164) next to the tap pairs, then each thread accumulates
-// 4 rows x 8 columns of outputs (two 4-column groups 64 columns apart, so that the 8 lanes
-// of a quarter-warp read consecutive 16-byte words: conflict-free LDS.128).
+//
+// Input.  The tracer writes the unconvolved images into a PADDED buffer: pixel (i, j) sits at
+// (i + p, j + q) of a [Hp][Wp] frame and border pixels are replicated into the pad (L164), so
+// a tile with its PSF halo is a plain rectangle of that frame -- no clamping here.
+// Hp = 64 tiles_y + KH - 1, Wp = 128 tiles_x + 4 NC (NC = ceil(KW / 4)): tiles that overhang
+// the image read zeros / stale finite values whose outputs are dropped.
+//
+// Work.  One persistent block of 256 threads per SM.  A work item is (output tile of 64 x 128
+// pixels, parameter vector); items are ordered tile-major and split evenly over the blocks,
+// so a block stays on one tile position for many vectors: the tile's data d and weights w
+// are staged in shared memory once per position.  The input tile (64 + KH - 1 rows of
+// 128 + 4 NC floats) comes in with cp.async, double buffered: item i+1 loads while item i is
+// convolved (single buffer when two do not fit: PSFs beyond ~45 x 45).
+//
+// Thread tile: 4 rows x 8 columns of outputs (two 4-column groups 64 columns apart, so that
+// the 8 lanes of a quarter-warp read consecutive 16-byte words: conflict-free LDS.128).
 //
 // Pairing.  A register pair holds the SAME column of two vertically adjacent output rows
 // (o, o+1).  At input row r they need tap rows r-o and r-o-1, so the pair multiplies the
 // broadcast scalar in[r][x+k] by the tap pair  Q[j][k] = (G[j][k], G[j-1][k]),  j = r-o,
-// G = flipped normalised PSF, G[-1] = G[KH] = 0.  Q is built on the host (api.cu) and sits
-// in shared memory; both operands of the FFMA2 come as they are loaded -- no shuffling of
-// register halves.  The thread's two row pairs (rows 0-1, 2-3) use Q[r] and Q[r-2].
+// G = flipped normalised PSF, G[-1] = G[KH] = 0.  Q is built on the host (api.cu).  At step
+// j = 0..KH the thread's two row pairs (rows 0-1, 2-3) both use Q[j]: pair 0 against input
+// row j of the thread's strip, pair 1 against row j + 2.  Four staged rows live in registers
+// and change roles every two steps, so each staged row is loaded once per chunk.
+//
+// Taps.  Q is block-uniform, so it is read through the UNIFORM datapath: it lives in the
+// constant bank (c_taps, a pool shared by the live handles) and FFMA2 takes the pair straight
+// from a uniform register (FFMA2 R, R.F32, UR.F32x2, R): no shared-memory traffic, no vector
+// registers for taps.
 //
 //   loop over tap-column chunks c (4 taps each)
-//     loop over input rows r of the thread's strip (KH + 3 of them)
-//       4 x LDS.128  input  in[r][4 tx + 4c .. +7]  and  .. + 64        (conflict-free)
-//       4 x LDS.128  taps   Q[r][c], Q[r-2][c]                          (broadcast)
+//     loop over steps j = 0 .. KH
+//       4 x LDS.128   input  in[j + 4][4 tx + 4c .. +7]  and  .. + 64    (conflict-free)
+//       4 x LDCU.64   taps   Q[j][c][0..3]                               (uniform datapath)
 //       64 x FFMA2
 //
 // Zero padding exists only in the tap columns (KW -> multiple of 4) and in the first / last
-// tap row of each pair; the staged input is zero beyond the KW-1 halo columns, and the traced
-// set is dilated by p+1 rows (api.cu), so a zero tap never meets an untraced value.
+// tap row of each pair; the traced set is dilated by p+1 rows (api.cu) and the padded frame
+// is zero-initialised, so a zero tap never meets a non-finite stale value.
 // Summation is blocked (per chunk, then across chunks): FP32 error growth ~ sqrt(4 KH) + sqrt(NC).
 //
 // Epilogue: loglike -> per-thread FP32 sum over its 32 pixels, then FP64: warp shuffle
@@ -38,6 +55,10 @@
 #include <math.h>
 
 namespace lensed {
+
+// tap pairs of all live handles (api.cu allocates ranges); 60 KB of the 64 KB constant bank
+__constant__ unsigned long long c_taps[kTapPoolPairs];
+
 namespace {
 
 constexpr int kTR = 4;                 // output rows per thread (two pairs)
@@ -46,212 +67,298 @@ constexpr int kThreads = kNTX * kNTY;
 constexpr int kGroup = 4 * kNTX;       // 64: distance of a thread's two column groups
 constexpr int kTW = 2 * kGroup;        // 128 output columns per tile
 constexpr int kTH = kTR * kNTY;        // 64 output rows per tile
+constexpr int kSlackRows = 2;          // rows past a staged tile the last loop body loads but never uses
 
 __device__ __forceinline__ f2 as_f2(unsigned long long v) { f2 r; r.v = v; return r; }
 
-// One input row r of the thread's strip against one 4-tap chunk.  P0 / P1: row pair 0 (tap
-// pairs Q[r]) / row pair 1 (Q[r-2]) takes part.  in_r -> in[r][4 tx + 4 c], q0 -> Q[r][c],
-// q1 -> Q[r-2][c].
-template <bool P0, bool P1>
-__device__ __forceinline__ void row_step(f2 (&part)[2][8], const float4 *in_r, const ulonglong2 *q0,
-                                         const ulonglong2 *q1)
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
 {
-    const float4 a0 = in_r[0], a1 = in_r[1], b0 = in_r[kGroup / 4], b1 = in_r[kGroup / 4 + 1];
-    const float va[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
-    const float vb[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
-    if (P0) {
-        const ulonglong2 t0 = q0[0], t1 = q0[1];
-        const f2 q[4] = {as_f2(t0.x), as_f2(t0.y), as_f2(t1.x), as_f2(t1.y)};
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// The 16 input floats a thread needs from one staged row for one 4-tap chunk: columns
+// 4 tx + 4 c .. + 7 of both column groups.
+struct InRow { float4 a0, a1, b0, b1; };
+
+__device__ __forceinline__ void load_row(InRow &x, const float4 *p)
+{
+    x.a0 = p[0]; x.a1 = p[1]; x.b0 = p[kGroup / 4]; x.b1 = p[kGroup / 4 + 1];
+}
+
+// One step j of a 4-tap chunk: both row pairs against the SAME tap pairs Q[j][c][0..3]
+// (iq = their index in c_taps).  Pair 0 (output rows 0-1) takes input row j of the strip
+// (x0), pair 1 (rows 2-3) takes input row j + 2 (x1).
+__device__ __forceinline__ void tap_step(f2 (&part)[2][8], const InRow &x0, const InRow &x1, int iq)
+{
+    const float va0[8] = {x0.a0.x, x0.a0.y, x0.a0.z, x0.a0.w, x0.a1.x, x0.a1.y, x0.a1.z, x0.a1.w};
+    const float vb0[8] = {x0.b0.x, x0.b0.y, x0.b0.z, x0.b0.w, x0.b1.x, x0.b1.y, x0.b1.z, x0.b1.w};
+    const float va1[8] = {x1.a0.x, x1.a0.y, x1.a0.z, x1.a0.w, x1.a1.x, x1.a1.y, x1.a1.z, x1.a1.w};
+    const float vb1[8] = {x1.b0.x, x1.b0.y, x1.b0.z, x1.b0.w, x1.b1.x, x1.b1.y, x1.b1.z, x1.b1.w};
 #pragma unroll
-        for (int k = 0; k < 4; ++k)
+    for (int k = 0; k < 4; ++k) {
+        const f2 q = as_f2(c_taps[iq + k]);
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                part[0][e] = fma2(q[k], bc(va[e + k]), part[0][e]);
-                part[0][4 + e] = fma2(q[k], bc(vb[e + k]), part[0][4 + e]);
-            }
-    }
-    if (P1) {
-        const ulonglong2 t0 = q1[0], t1 = q1[1];
-        const f2 q[4] = {as_f2(t0.x), as_f2(t0.y), as_f2(t1.x), as_f2(t1.y)};
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                part[1][e] = fma2(q[k], bc(va[e + k]), part[1][e]);
-                part[1][4 + e] = fma2(q[k], bc(vb[e + k]), part[1][4 + e]);
-            }
+        for (int e = 0; e < 4; ++e) {
+            part[0][e] = fma2(q, bc(va0[e + k]), part[0][e]);
+            part[0][4 + e] = fma2(q, bc(vb0[e + k]), part[0][4 + e]);
+            part[1][e] = fma2(q, bc(va1[e + k]), part[1][e]);
+            part[1][4 + e] = fma2(q, bc(vb1[e + k]), part[1][4 + e]);
+        }
     }
 }
 
 template <bool RENDER>
-__global__ void __launch_bounds__(kThreads, 2) conv_kernel(ConvArgs a)
+__global__ void __launch_bounds__(kThreads, 1) conv_kernel(ConvArgs a)
 {
     extern __shared__ float4 smem4[];
     const int IW4 = kTW / 4 + a.NC, IW = 4 * IW4;
-    const int IH = kTH + a.KH - 1;
-    float *s_in = reinterpret_cast<float *>(smem4);                                    // [IH][IW]
-    ulonglong2 *s_q = reinterpret_cast<ulonglong2 *>(smem4 + (size_t)IH * IW4);        // [KH+1][NC][2]
+    const int IH = kTH + a.KH - 1 + kSlackRows;
+    float *s_stage = reinterpret_cast<float *>(smem4);                    // [n_stages][IH][IW]
+    float *s_d = s_stage + (size_t)a.n_stages * IH * IW;                  // [kTH][kTW] data      (loglike)
+    float *s_w = s_d + kTH * kTW;                                         // [kTH][kTW] weights   (loglike)
     __shared__ double s_red[kThreads / 32];
 
-    const int bvec = blockIdx.y;
-    const uint32_t tile = a.tiles[blockIdx.x];
-    const int Y0 = (int)(tile >> 16) * kTH, X0 = (int)(tile & 0xffffu) * kTW;
-    const float *Lb = a.L + (size_t)bvec * a.l_stride;
+    // this block's share of the (tile, vector) items, tile-major
+    const long long n_items = (long long)a.n_tiles * a.nb;
+    const int lo = (int)(n_items * blockIdx.x / gridDim.x), hi = (int)(n_items * (blockIdx.x + 1) / gridDim.x);
+    if (lo >= hi) return;
+
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-
-    // stage the tap pairs and the clamped input tile (zero beyond the KW-1 halo columns)
-    {
-        const ulonglong2 *gq = reinterpret_cast<const ulonglong2 *>(a.taps);
-        for (int i = threadIdx.x; i < (a.KH + 1) * a.NC * 2; i += kThreads) s_q[i] = gq[i];
-        const int used = kTW + a.KW - 1;
-        for (int r = warp; r < IH; r += kThreads / 32) {
-            const int y = min(max(Y0 - a.p + r, 0), a.H - 1);
-            const float *src = Lb + (size_t)y * a.W;
-            for (int c = lane; c < IW; c += 32) {
-                const int x = min(max(X0 - a.q + c, 0), a.W - 1);
-                s_in[r * IW + c] = c < used ? src[x] : 0.0f;
-            }
-        }
-    }
-    __syncthreads();
-
     const int tx = (warp & 1) * 8 + (lane & 7);
     const int ty = (warp >> 1) * 4 + (lane >> 3);
-    const int oy = Y0 + ty * kTR, ox = X0 + tx * 4;
 
-    // does this warp own any pixel that counts?  (uniform per warp: skipping is free)
-    bool any = false;
-    if (RENDER) {
-        any = oy < a.H && ox < a.W;
-    } else {
-#pragma unroll
-        for (int o = 0; o < kTR; ++o)
-#pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
-                if (y < a.H && x < a.W) any = any || a.wmask[(size_t)y * a.W + x] != 0.0f;
-            }
-    }
-    const bool warp_any = __any_sync(0xffffffffu, any);
-
-    // acc[pair][column]: running sum over tap-column chunks; part: the current chunk
-    f2 acc[2][8];
-#pragma unroll
-    for (int p = 0; p < 2; ++p)
-#pragma unroll
-        for (int e = 0; e < 8; ++e) acc[p][e] = bc(0.0f);
-
-    if (warp_any) {
-        const int KH = a.KH, NC2 = 2 * a.NC;
-        const float4 *in_base = reinterpret_cast<const float4 *>(s_in) + (size_t)(ty * kTR) * IW4 + tx;
-#pragma unroll 1
-        for (int c = 0; c < a.NC; ++c) {
-            f2 part[2][8];
-#pragma unroll
-            for (int p = 0; p < 2; ++p)
-#pragma unroll
-                for (int e = 0; e < 8; ++e) part[p][e] = bc(0.0f);
-            const float4 *in_r = in_base + c;
-            const ulonglong2 *q_r = s_q + 2 * c;
-            row_step<true, false>(part, in_r, q_r, nullptr);
-            row_step<true, false>(part, in_r + IW4, q_r + NC2, nullptr);
-            in_r += 2 * IW4;
-#pragma unroll 2
-            for (int r = 2; r <= KH; ++r) {
-                row_step<true, true>(part, in_r, q_r + 2 * NC2, q_r);
-                in_r += IW4;
-                q_r += NC2;
-            }
-            row_step<false, true>(part, in_r, nullptr, q_r);
-            row_step<false, true>(part, in_r + IW4, nullptr, q_r + NC2);
-#pragma unroll
-            for (int p = 0; p < 2; ++p)
-#pragma unroll
-                for (int e = 0; e < 8; ++e) acc[p][e] = add2(acc[p][e], part[p][e]);
+    // input tile of an item -> stage s (all threads; one commit group)
+    auto issue = [&](int item, int s) {
+        const int t = item / a.nb, b = item - t * a.nb;
+        const uint32_t tile = a.tiles[t];
+        const int Y0 = (int)(tile >> 16) * kTH, X0 = (int)(tile & 0xffffu) * kTW;
+        const float *src = a.Lp + (size_t)b * a.lp_stride + (size_t)Y0 * a.Wp + X0;
+        float *dst = s_stage + (size_t)s * IH * IW;
+        for (int i = threadIdx.x; i < (IH - kSlackRows) * IW4; i += kThreads) {
+            const int r = i / IW4, c4 = i - r * IW4;
+            cp_async16(dst + r * IW + 4 * c4, src + (size_t)r * a.Wp + 4 * c4);
         }
-    }
+        cp_async_commit();
+    };
 
-    float out[kTR][8];
-#pragma unroll
-    for (int p = 0; p < 2; ++p)
-#pragma unroll
-        for (int e = 0; e < 8; ++e) un2(acc[p][e], out[2 * p][e], out[2 * p + 1][e]);
+    issue(lo, 0);
+    int cur_t = -1;
+    bool warp_any = true;
+    const int NC4 = 4 * a.NC;
+    const int n4 = (a.KH + 1) >> 2;                 // KH + 1 steps (KH is odd): n4 bodies of four
+    const bool tail2 = ((a.KH + 1) & 2) != 0;       // + two more
 
-    if (RENDER) {
-        const bool valid = a.derived[(size_t)bvec * a.D] != 0.0f;
-        float *mb = a.model + (size_t)bvec * a.l_stride;
+#pragma unroll 1
+    for (int item = lo; item < hi; ++item) {
+        const int s = a.n_stages == 2 ? ((item - lo) & 1) : 0;
+        const int t = item / a.nb, b = item - t * a.nb;
+        const uint32_t tile = a.tiles[t];
+        const int Y0 = (int)(tile >> 16) * kTH, X0 = (int)(tile & 0xffffu) * kTW;
+        const bool more = item + 1 < hi;
+        if (a.n_stages == 2 && more) issue(item + 1, s ^ 1);
+
+        if (!RENDER && t != cur_t) {
+            // data and weights of this tile position (the previous item's epilogue is done:
+            // barrier at the end of the loop body); w = 0 outside the image
+            for (int i = threadIdx.x; i < kTH * kTW / 4; i += kThreads) {
+                const int r = i / (kTW / 4), c = 4 * (i - r * (kTW / 4));
+                const int y = Y0 + r;
+                float dv[4], wv[4];
 #pragma unroll
-        for (int o = 0; o < kTR; ++o)
-#pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
-                if (y < a.H && x < a.W) mb[(size_t)y * a.W + x] = valid ? out[o][e] : nanf("");
+                for (int e = 0; e < 4; ++e) {
+                    const int x = X0 + c + e;
+                    const bool in = y < a.H && x < a.W;
+                    dv[e] = in ? a.image[(size_t)y * a.W + x] : 0.0f;
+                    wv[e] = in ? a.wmask[(size_t)y * a.W + x] : 0.0f;
+                }
+                *reinterpret_cast<float4 *>(s_d + r * kTW + c) = make_float4(dv[0], dv[1], dv[2], dv[3]);
+                *reinterpret_cast<float4 *>(s_w + r * kTW + c) = make_float4(wv[0], wv[1], wv[2], wv[3]);
             }
-    } else {
-        float part = 0.0f;
+        }
+        if (a.n_stages == 2 && more) cp_async_wait<1>(); else cp_async_wait<0>();
+        __syncthreads();
+
+        if (t != cur_t) {
+            cur_t = t;
+            if (!RENDER) {
+                // warps whose 16 x 64 outputs are all masked skip the convolution
+                bool any = false;
+#pragma unroll
+                for (int o = 0; o < kTR; ++o)
+#pragma unroll
+                    for (int g = 0; g < 2; ++g) {
+                        const float4 w4 = *reinterpret_cast<const float4 *>(s_w + (ty * kTR + o) * kTW + 4 * tx + g * kGroup);
+                        any = any || w4.x != 0.0f || w4.y != 0.0f || w4.z != 0.0f || w4.w != 0.0f;
+                    }
+                warp_any = __any_sync(0xffffffffu, any);
+            }
+        }
+
+        // acc[pair][column]: running sum over tap-column chunks; part: the current chunk
+        f2 acc[2][8];
+#pragma unroll
+        for (int p = 0; p < 2; ++p)
+#pragma unroll
+            for (int e = 0; e < 8; ++e) acc[p][e] = bc(0.0f);
+
         if (warp_any) {
+            const float4 *in_base = reinterpret_cast<const float4 *>(s_stage + (size_t)s * IH * IW) +
+                                    (size_t)(ty * kTR) * IW4 + tx;
+#pragma unroll 1
+            for (int c = 0; c < a.NC; ++c) {
+                f2 part[2][8];
+#pragma unroll
+                for (int p = 0; p < 2; ++p)
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) part[p][e] = bc(0.0f);
+                // steps j = 0 .. KH (tap pair rows Q[j]); four input rows live in registers and
+                // rotate A -> C's partner etc. without moves: the loop body is four steps
+                const float4 *in_r = in_base + c;
+                int iq = a.tap_off + 4 * c;                 // Q[j][c][0]
+                InRow A, B, C, D;
+                load_row(A, in_r);
+                load_row(B, in_r + IW4);
+                load_row(C, in_r + 2 * IW4);
+                load_row(D, in_r + 3 * IW4);
+                in_r += 4 * IW4;
+#pragma unroll 1
+                for (int j4 = 0; j4 < n4; ++j4) {
+                    tap_step(part, A, C, iq);
+                    load_row(A, in_r);
+                    tap_step(part, B, D, iq + NC4);
+                    load_row(B, in_r + IW4);
+                    tap_step(part, C, A, iq + 2 * NC4);
+                    load_row(C, in_r + 2 * IW4);
+                    tap_step(part, D, B, iq + 3 * NC4);
+                    load_row(D, in_r + 3 * IW4);
+                    in_r += 4 * IW4;
+                    iq += 4 * NC4;
+                }
+                if (tail2) {
+                    tap_step(part, A, C, iq);
+                    tap_step(part, B, D, iq + NC4);
+                }
+#pragma unroll
+                for (int p = 0; p < 2; ++p)
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) acc[p][e] = add2(acc[p][e], part[p][e]);
+            }
+        }
+
+        float out[kTR][8];
+#pragma unroll
+        for (int p = 0; p < 2; ++p)
+#pragma unroll
+            for (int e = 0; e < 8; ++e) un2(acc[p][e], out[2 * p][e], out[2 * p + 1][e]);
+
+        const int oy = Y0 + ty * kTR, ox = X0 + tx * 4;
+        if (RENDER) {
+            const bool valid = a.derived[(size_t)b * a.D] != 0.0f;
+            float *mb = a.model + (size_t)b * a.H * a.W;
 #pragma unroll
             for (int o = 0; o < kTR; ++o)
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
                     const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
-                    if (y < a.H && x < a.W) {
-                        const size_t i = (size_t)y * a.W + x;
-                        const float w = a.wmask[i];
-                        if (w != 0.0f) {                   // masked pixels may see untraced L: never touch them
-                            const float diff = a.image[i] - out[o][e];
-                            part = fmaf(w * diff, diff, part);
-                        }
-                    }
+                    if (y < a.H && x < a.W) mb[(size_t)y * a.W + x] = valid ? out[o][e] : nanf("");
                 }
-        }
-        double dpart = (double)part;
+        } else {
+            float part = 0.0f;
+            if (warp_any) {
 #pragma unroll
-        for (int sft = 16; sft > 0; sft >>= 1) dpart += __shfl_xor_sync(0xffffffffu, dpart, sft);
-        if (lane == 0) s_red[warp] = dpart;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double s = 0.0;
+                for (int o = 0; o < kTR; ++o)
 #pragma unroll
-            for (int i = 0; i < kThreads / 32; ++i) s += s_red[i];
-            a.partial[(size_t)bvec * a.n_tiles + blockIdx.x] = s;
+                    for (int g = 0; g < 2; ++g) {
+                        const int off = (ty * kTR + o) * kTW + 4 * tx + g * kGroup;
+                        const float4 w4 = *reinterpret_cast<const float4 *>(s_w + off);
+                        const float4 d4 = *reinterpret_cast<const float4 *>(s_d + off);
+                        const float wv[4] = {w4.x, w4.y, w4.z, w4.w}, dv[4] = {d4.x, d4.y, d4.z, d4.w};
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            if (wv[e] != 0.0f) {           // masked pixels may see untraced L: never touch them
+                                const float diff = dv[e] - out[o][4 * g + e];
+                                part = fmaf(wv[e] * diff, diff, part);
+                            }
+                    }
+            }
+            double sum = (double)part;
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
+            if (lane == 0) s_red[warp] = sum;
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                double tot = 0.0;
+                for (int i = 0; i < kThreads / 32; ++i) tot += s_red[i];
+                a.partial[(size_t)b * a.n_tiles + t] = tot;
+            }
         }
+        __syncthreads();           // stage s and s_red are free again
+        if (a.n_stages == 1 && more) issue(item + 1, 0);
     }
 }
 
-__global__ void __launch_bounds__(128) final_kernel(FinalArgs a)
+// logL[b] = -1/2 sum over tiles, in tile order; -inf for vectors outside the model domain
+__global__ void final_kernel(FinalArgs a)
 {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= a.B) return;
-    double s = 0.0;
-    const double *p = a.partial + (size_t)b * a.n_tiles;
-    for (int t = 0; t < a.n_tiles; ++t) s += p[t];
-    const bool valid = a.derived[(size_t)b * a.D] != 0.0f;
-    a.logl[b] = valid ? (float)(-0.5 * s) : -INFINITY;
+    if (a.derived[(size_t)b * a.D] == 0.0f) { a.logl[b] = -INFINITY; return; }
+    double chi2 = 0.0;
+    for (int t = 0; t < a.n_tiles; ++t) chi2 += a.partial[(size_t)b * a.n_tiles + t];
+    a.logl[b] = (float)(-0.5 * chi2);
 }
 
 }  // namespace
 
 void conv_tile_shape(int *tile_w, int *tile_h) { *tile_w = kTW; *tile_h = kTH; }
 
-size_t conv_smem_bytes(int KH, int NC)
+void conv_padded_shape(int H, int W, int KH, int NC, int *Hp, int *Wp)
 {
-    const size_t IW = kTW + 4 * NC, IH = kTH + KH - 1;
-    return (IH * IW + (size_t)(KH + 1) * 8 * NC) * sizeof(float);
+    *Hp = (H + kTH - 1) / kTH * kTH + KH - 1;
+    *Wp = (W + kTW - 1) / kTW * kTW + 4 * NC;
+}
+
+namespace {
+constexpr size_t kSmemLimit = 226 * 1024;   // dynamic part; 227 KB per block minus the static s_red
+size_t stage_bytes(int KH, int NC) { return (size_t)(kTH + KH - 1 + kSlackRows) * (kTW + 4 * NC) * sizeof(float); }
+size_t dw_bytes(bool render) { return render ? 0 : (size_t)2 * kTH * kTW * sizeof(float); }
+}  // namespace
+
+int conv_num_stages(int KH, int NC, bool render)
+{
+    return 2 * stage_bytes(KH, NC) + dw_bytes(render) <= kSmemLimit ? 2 : 1;
+}
+
+size_t conv_smem_bytes(int KH, int NC, bool render)
+{
+    return conv_num_stages(KH, NC, render) * stage_bytes(KH, NC) + dw_bytes(render);
 }
 
 cudaError_t conv_setup()
 {
-    const int max_smem = (int)conv_smem_bytes(kMaxPsf, (kMaxPsf + 3) / 4);
-    cudaError_t e = cudaFuncSetAttribute(conv_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+    cudaError_t e = cudaFuncSetAttribute(conv_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(conv_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+    return cudaFuncSetAttribute(conv_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit);
 }
 
-cudaError_t launch_conv(const ConvArgs &a, bool render, int nvec, cudaStream_t st)
+cudaError_t conv_upload_taps(const float *pairs, int n_pairs, int pool_offset)
 {
-    const size_t smem = conv_smem_bytes(a.KH, a.NC);
-    dim3 grid(a.n_tiles, nvec);
+    return cudaMemcpyToSymbol(c_taps, pairs, (size_t)n_pairs * sizeof(unsigned long long),
+                              (size_t)pool_offset * sizeof(unsigned long long), cudaMemcpyHostToDevice);
+}
+
+// n_blocks: persistent blocks to launch (the SM count; fewer when there are fewer items)
+cudaError_t launch_conv(ConvArgs a, bool render, int n_blocks, cudaStream_t st)
+{
+    a.n_stages = conv_num_stages(a.KH, a.NC, render);
+    const size_t smem = conv_smem_bytes(a.KH, a.NC, render);
+    const long long n_items = (long long)a.n_tiles * a.nb;
+    const int grid = (int)(n_items < n_blocks ? n_items : n_blocks);
+    if (grid < 1) return cudaSuccess;
     if (render) conv_kernel<true><<<grid, kThreads, smem, st>>>(a);
     else conv_kernel<false><<<grid, kThreads, smem, st>>>(a);
     return cudaGetLastError();

@@ -46,6 +46,7 @@ constexpr int kMaxModels = 32;
 constexpr int kMaxQuad = 256;
 constexpr int kMaxPsf = 63;
 constexpr int kHeaderFloats = 4;
+constexpr int kTapPoolPairs = 7680;   // conv.cu c_taps: 60 KB of constant bank shared by the live handles
 
 __host__ __device__ constexpr int kind_num_params(int k) {
     return k == K_SIS ? 3 : k == K_SIE ? 5 : k == K_POINT ? 3 : k == K_SHEAR ? 2
@@ -84,26 +85,30 @@ struct TraceArgs {
     const float *derived;  // [.][D], already offset to the chunk's first vector
     const uint32_t *pix;   // [npix] packed (row << 16) | column
     const float4 *quad;    // [nq_pad] (xi, eta, w, 0), zero-weight padding up to a multiple of R (even)
-    float *L;              // [.][H*W], chunk-local
-    long long l_stride;    // H*W
-    int npix, nq_pad, W;
+    float *L;              // [.][Hp*Wp], chunk-local PADDED frames: pixel (i, j) at (i + py, j + px),
+                           // border pixels replicated into the pad (conv.cu "Input")
+    long long l_stride;    // Hp*Wp
+    int npix, nq_pad;
+    int H, W, Wp, px, py;
     int pix_per_block;     // pixels of the list one block walks (a multiple of 256)
     float cxh, cyh;
 };
 
 struct ConvArgs {
-    const float *L;        // [.][H*W] chunk-local unconvolved images
-    const float *taps;     // [KH+1][NC][4][2] tap pairs (G[j][k], G[j-1][k]) of the flipped, normalised PSF (conv.cu)
+    const float *Lp;       // [nb][Hp*Wp] chunk-local padded unconvolved images (TraceArgs::L)
     const float *image;    // [H*W] d
     const float *wmask;    // [H*W] w_i, 0 where masked
     const uint32_t *tiles; // [n_tiles] packed (tile row << 16) | tile column (active tiles)
-    double *partial;       // [.][n_tiles] chunk-local chi-square partials   (loglike)
-    float *model;          // [.][H*W] chunk-local output                     (render)
-    const float *derived;  // [.][D] chunk-local (valid flag)                 (render)
-    long long l_stride;
+    double *partial;       // [nb][n_tiles] chunk-local chi-square partials   (loglike)
+    float *model;          // [nb][H*W] chunk-local output                    (render)
+    const float *derived;  // [nb][D] chunk-local (valid flag)                (render)
+    long long lp_stride;   // Hp*Wp
     int D;
-    int H, W, KH, KW, NC, n_tiles;
-    int p, q;              // (KH-1)/2, (KW-1)/2
+    int H, W, Wp, KH, KW, NC, n_tiles;
+    int nb;                // vectors in this launch
+    int tap_off;           // first tap pair of this handle in c_taps: Q[j][c][k] at tap_off + (j NC + c) 4 + k,
+                           // Q[j][c][k] = (G[j][4c+k], G[j-1][4c+k]), j = 0..KH, G = flipped normalised PSF
+    int n_stages;          // input-tile buffers in shared memory (set by launch_conv)
 };
 
 struct FinalArgs {
@@ -118,13 +123,15 @@ cudaError_t launch_prep(const Program &prog, const PrepArgs &a, cudaStream_t st)
 // allow_static: use the compile-time-specialised kernel when the list has one (trace.cu)
 cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nvec, bool allow_static, cudaStream_t st);
 bool trace_has_static(const Program &prog);
-cudaError_t launch_conv(const ConvArgs &a, bool render, int nvec, cudaStream_t st);
+cudaError_t launch_conv(ConvArgs a, bool render, int n_blocks, cudaStream_t st);
+cudaError_t conv_upload_taps(const float *pairs, int n_pairs, int pool_offset);
+void conv_padded_shape(int H, int W, int KH, int NC, int *Hp, int *Wp);
 cudaError_t launch_final(const FinalArgs &a, cudaStream_t st);
 cudaError_t conv_setup();                 // one-time function attributes
 int trace_pick_R(int n_quad);             // rays per register block for an n_quad-point rule
 size_t trace_smem_bytes(const Program &prog, int nq_pad);
 void conv_tile_shape(int *tile_w, int *tile_h);
-size_t conv_smem_bytes(int KH, int NC);
+size_t conv_smem_bytes(int KH, int NC, bool render);
 cudaError_t run_fma_peak(int iters, double *tflops);
 
 }  // namespace lensed

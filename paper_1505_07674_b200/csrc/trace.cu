@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(kTraceThreads, 2) trace_kernel(Program prog, T
 #pragma unroll
             for (int k = 0; k < NP; ++k) acc = fma2(w[k], r.I[k], acc);
         }
-        Lb[row * a.W + col] = (lo2(acc) + hi2(acc)) + tb.sky;
+        store_pixel(a, Lb, row, col, (lo2(acc) + hi2(acc)) + tb.sky);
     }
 }
 

@@ -59,6 +59,20 @@ __device__ __forceinline__ TraceBlock trace_prologue(const Program &prog, const 
     return tb;
 }
 
+// L_i into the padded frame the convolution reads (conv.cu "Input"): pixel (row, col) at
+// (row + py, col + px); a border pixel also fills the pad cells that clamp to it
+// ("border pixels are repeated").
+__device__ __forceinline__ void store_pixel(const TraceArgs &a, float *Lb, int row, int col, float v)
+{
+    Lb[(size_t)(row + a.py) * a.Wp + col + a.px] = v;
+    if (row == 0 || col == 0 || row == a.H - 1 || col == a.W - 1) {
+        const int r0 = row == 0 ? 0 : row + a.py, r1 = row == a.H - 1 ? a.H - 1 + 2 * a.py : row + a.py;
+        const int c0 = col == 0 ? 0 : col + a.px, c1 = col == a.W - 1 ? a.W - 1 + 2 * a.px : col + a.px;
+        for (int r = r0; r <= r1; ++r)
+            for (int c = c0; c <= c1; ++c) Lb[(size_t)r * a.Wp + c] = v;
+    }
+}
+
 template <class Kernel>
 cudaError_t launch_trace_kernel(Kernel kernel, const Program &prog, const TraceArgs &a, int nvec, cudaStream_t st)
 {

@@ -122,12 +122,16 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
 #pragma unroll
             for (int k = 0; k < NP; ++k) acc = fma2(w[k], r.I[k], acc);
         }
-        Lb[row * a.W + col] = (lo2(acc) + hi2(acc)) + tb.sky;
+        store_pixel(a, Lb, row, col, (lo2(acc) + hi2(acc)) + tb.sky);
     }
 }
 
+#ifndef LENSED_TRACE_MIN_BLOCKS
+#define LENSED_TRACE_MIN_BLOCKS 2      // resident blocks per SM the register budget is cut for
+#endif
+
 template <int NP, class S>
-__global__ void __launch_bounds__(kTraceThreads, 2) trace_static_kernel(Program prog, TraceArgs a)
+__global__ void __launch_bounds__(kTraceThreads, LENSED_TRACE_MIN_BLOCKS) trace_static_kernel(Program prog, TraceArgs a)
 {
     extern __shared__ float4 smem4[];
     const TraceBlock tb = trace_prologue(prog, a, smem4);

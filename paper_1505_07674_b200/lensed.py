@@ -35,6 +35,7 @@ SYMBOLS = {
     "lensed_get_profile": (_i, [_p, _p, _p]),
     "lensed_reset_profile": (_i, [_p]),
     "lensed_set_chunk_bytes": (_i, [_p, _ll]),
+    "lensed_frame_bytes": (_ll, [_p]),
     "lensed_set_static_tracer": (_i, [_p, _i]),
     "lensed_get_static_tracer": (_i, [_p]),
     "lensed_fma_peak": (_i, [_i, _i, _p]),
@@ -56,10 +57,11 @@ def lib():
     """The loaded shared library; built in-tree with nvcc if it is not there."""
     global _lib
     if _lib is None:
-        if not os.path.exists(LIB_PATH):
+        path = os.environ.get("LENSED_B200_LIB") or LIB_PATH     # override: a differently tuned build
+        if path == LIB_PATH and not os.path.exists(LIB_PATH):
             from . import build as _build
             _build.build()
-        L = ctypes.CDLL(LIB_PATH)
+        L = ctypes.CDLL(path)
         for name, (res, args) in SYMBOLS.items():
             fn = getattr(L, name)
             fn.restype, fn.argtypes = res, args
@@ -165,6 +167,10 @@ def lensed_reset_profile(h):
 
 def lensed_set_chunk_bytes(h, nbytes):
     _check(lib().lensed_set_chunk_bytes(h, int(nbytes)), h)
+
+
+def lensed_frame_bytes(h):
+    return lib().lensed_frame_bytes(h)
 
 
 def lensed_set_static_tracer(h, on):

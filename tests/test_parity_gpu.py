@@ -253,7 +253,7 @@ def test_host_buffer_calls_match_device_calls_and_chunking_does_not_change_resul
         L.lensed_loglike_host(h, pinned, out_pinned)
         model_host = np.empty((40, cfg.H, cfg.W), dtype=np.float32)
         L.lensed_render_host(h, params, model_host)
-        L.lensed_set_chunk_bytes(h, 3 * cfg.H * cfg.W * 4)       # 3 vectors per chunk, ragged last chunk
+        L.lensed_set_chunk_bytes(h, 3 * L.lensed_frame_bytes(h))  # 3 vectors per chunk, ragged last chunk
         logl_chunked, model_chunked = _gpu_eval(L, h, params, cfg.H, cfg.W)
         L.lensed_set_profiling(h, True)
         L.lensed_reset_profile(h)
