@@ -127,7 +127,7 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
 }
 
 #ifndef LENSED_TRACE_MIN_BLOCKS
-#define LENSED_TRACE_MIN_BLOCKS 2      // resident blocks per SM the register budget is cut for
+#define LENSED_TRACE_MIN_BLOCKS 3      // resident blocks per SM the register budget is cut for
 #endif
 
 template <int NP, class S>
