@@ -279,10 +279,12 @@ def main():
     except lensed.LensedError:
         measured_ffma = None
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the ncu capture
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per vector from the ncu capture
     if os.path.exists(tpath):
         with open(tpath) as fh:
-            traffic = json.load(fh).get("%s:%d" % (dom, args.config))
+            t = json.load(fh).get("%s:%d" % (dom, args.config))
+            if t:                                            # per vector in the capture -> per launch of this run
+                traffic = int(t["bytes_per_vector"] * B * args.steps / max(phase_n[dom], 1))
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS,
                 "unit": "TFLOP/s", "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": traffic,
                 "peak_source": "nominal 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)",
