@@ -91,7 +91,9 @@ __device__ __forceinline__ void load_row(InRow &x, const float4 *p)
 
 // One step j of a 4-tap chunk: both row pairs against the SAME tap pairs Q[j][c][0..3]
 // (iq = their index in c_taps).  Pair 0 (output rows 0-1) takes input row j of the strip
-// (x0), pair 1 (rows 2-3) takes input row j + 2 (x1).
+// (x0), pair 1 (rows 2-3) takes input row j + 2 (x1).  NT = taps of the chunk (4, or the
+// 1-3 of the last chunk when KW is not a multiple of 4: no multiply by a padded zero column).
+template <int NT>
 __device__ __forceinline__ void tap_step(f2 (&part)[2][8], const InRow &x0, const InRow &x1, int iq)
 {
     const float va0[8] = {x0.a0.x, x0.a0.y, x0.a0.z, x0.a0.w, x0.a1.x, x0.a1.y, x0.a1.z, x0.a1.w};
@@ -99,7 +101,7 @@ __device__ __forceinline__ void tap_step(f2 (&part)[2][8], const InRow &x0, cons
     const float va1[8] = {x1.a0.x, x1.a0.y, x1.a0.z, x1.a0.w, x1.a1.x, x1.a1.y, x1.a1.z, x1.a1.w};
     const float vb1[8] = {x1.b0.x, x1.b0.y, x1.b0.z, x1.b0.w, x1.b1.x, x1.b1.y, x1.b1.z, x1.b1.w};
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < NT; ++k) {
         const f2 q = as_f2(c_taps[iq + k]);
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
@@ -109,6 +111,47 @@ __device__ __forceinline__ void tap_step(f2 (&part)[2][8], const InRow &x0, cons
             part[1][4 + e] = fma2(q, bc(vb1[e + k]), part[1][4 + e]);
         }
     }
+}
+
+// One 4-tap chunk: steps j = 0 .. KH (tap pair rows Q[j], first pair at c_taps[iq]) into
+// `part`, then `acc += part`.  Four staged rows live in registers and change roles every two
+// steps without moves: the loop body is four steps.  in_r -> in[strip row 0][4 tx + 4 c].
+template <int NT>
+__device__ __forceinline__ void conv_chunk(f2 (&acc)[2][8], const float4 *in_r, int iq, int n4, bool tail2, int IW4,
+                                           int NC4)
+{
+    f2 part[2][8];
+#pragma unroll
+    for (int p = 0; p < 2; ++p)
+#pragma unroll
+        for (int e = 0; e < 8; ++e) part[p][e] = bc(0.0f);
+    InRow A, B, C, D;
+    load_row(A, in_r);
+    load_row(B, in_r + IW4);
+    load_row(C, in_r + 2 * IW4);
+    load_row(D, in_r + 3 * IW4);
+    in_r += 4 * IW4;
+#pragma unroll 1
+    for (int j4 = 0; j4 < n4; ++j4) {
+        tap_step<NT>(part, A, C, iq);
+        load_row(A, in_r);
+        tap_step<NT>(part, B, D, iq + NC4);
+        load_row(B, in_r + IW4);
+        tap_step<NT>(part, C, A, iq + 2 * NC4);
+        load_row(C, in_r + 2 * IW4);
+        tap_step<NT>(part, D, B, iq + 3 * NC4);
+        load_row(D, in_r + 3 * IW4);
+        in_r += 4 * IW4;
+        iq += 4 * NC4;
+    }
+    if (tail2) {
+        tap_step<NT>(part, A, C, iq);
+        tap_step<NT>(part, B, D, iq + NC4);
+    }
+#pragma unroll
+    for (int p = 0; p < 2; ++p)
+#pragma unroll
+        for (int e = 0; e < 8; ++e) acc[p][e] = add2(acc[p][e], part[p][e]);
 }
 
 template <bool RENDER>
@@ -208,44 +251,17 @@ __global__ void __launch_bounds__(kThreads, 1) conv_kernel(ConvArgs a)
         if (warp_any) {
             const float4 *in_base = reinterpret_cast<const float4 *>(s_stage + (size_t)s * IH * IW) +
                                     (size_t)(ty * kTR) * IW4 + tx;
+            const int last_taps = a.KW - 4 * (a.NC - 1);          // taps of the last chunk, 1..4
+            const int n_full = last_taps == 4 ? a.NC : a.NC - 1;
 #pragma unroll 1
-            for (int c = 0; c < a.NC; ++c) {
-                f2 part[2][8];
-#pragma unroll
-                for (int p = 0; p < 2; ++p)
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) part[p][e] = bc(0.0f);
-                // steps j = 0 .. KH (tap pair rows Q[j]); four input rows live in registers and
-                // rotate A -> C's partner etc. without moves: the loop body is four steps
-                const float4 *in_r = in_base + c;
-                int iq = a.tap_off + 4 * c;                 // Q[j][c][0]
-                InRow A, B, C, D;
-                load_row(A, in_r);
-                load_row(B, in_r + IW4);
-                load_row(C, in_r + 2 * IW4);
-                load_row(D, in_r + 3 * IW4);
-                in_r += 4 * IW4;
-#pragma unroll 1
-                for (int j4 = 0; j4 < n4; ++j4) {
-                    tap_step(part, A, C, iq);
-                    load_row(A, in_r);
-                    tap_step(part, B, D, iq + NC4);
-                    load_row(B, in_r + IW4);
-                    tap_step(part, C, A, iq + 2 * NC4);
-                    load_row(C, in_r + 2 * IW4);
-                    tap_step(part, D, B, iq + 3 * NC4);
-                    load_row(D, in_r + 3 * IW4);
-                    in_r += 4 * IW4;
-                    iq += 4 * NC4;
-                }
-                if (tail2) {
-                    tap_step(part, A, C, iq);
-                    tap_step(part, B, D, iq + NC4);
-                }
-#pragma unroll
-                for (int p = 0; p < 2; ++p)
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) acc[p][e] = add2(acc[p][e], part[p][e]);
+            for (int c = 0; c < n_full; ++c)
+                conv_chunk<4>(acc, in_base + c, a.tap_off + 4 * c, n4, tail2, IW4, NC4);
+            if (last_taps != 4) {
+                const float4 *in_r = in_base + n_full;
+                const int iq = a.tap_off + 4 * n_full;
+                if (last_taps == 3) conv_chunk<3>(acc, in_r, iq, n4, tail2, IW4, NC4);
+                else if (last_taps == 2) conv_chunk<2>(acc, in_r, iq, n4, tail2, IW4, NC4);
+                else conv_chunk<1>(acc, in_r, iq, n4, tail2, IW4, NC4);
             }
         }
 

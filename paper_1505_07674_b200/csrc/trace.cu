@@ -150,6 +150,9 @@ size_t trace_smem_bytes(const Program &prog, int nq_pad)
 // by a per-block overhead that shrinks with R (4 -> 4, 9 -> 10, 16 -> 8, 25 -> 10, 49 -> 10).
 int trace_pick_R(int n_quad)
 {
+#ifdef LENSED_TRACE_FORCE_R            // tuning builds (build.py defines=...)
+    return LENSED_TRACE_FORCE_R;
+#endif
     int best = 2;
     double best_cost = 1e300;
     for (int R = 2; R <= 10; R += 2) {

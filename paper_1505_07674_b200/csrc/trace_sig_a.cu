@@ -4,5 +4,8 @@
 #include "trace_static.cuh"
 
 namespace lensed {
-LENSED_DEFINE_STATIC_TRACER(trace_static_a, 0, 0, 1, 0, 0, 1, 0, 0)
+#ifndef LENSED_MINB_A
+#define LENSED_MINB_A 3
+#endif
+LENSED_DEFINE_STATIC_TRACER(trace_static_a, LENSED_MINB_A, 0, 0, 1, 0, 0, 1, 0, 0)
 }  // namespace lensed

@@ -4,5 +4,8 @@
 #include "trace_static.cuh"
 
 namespace lensed {
-LENSED_DEFINE_STATIC_TRACER(trace_static_b, 1, 1, 0, 0, 1, 0, 1, 0)
+#ifndef LENSED_MINB_B
+#define LENSED_MINB_B 3
+#endif
+LENSED_DEFINE_STATIC_TRACER(trace_static_b, LENSED_MINB_B, 1, 1, 0, 0, 1, 0, 1, 0)
 }  // namespace lensed

@@ -4,5 +4,8 @@
 #include "trace_static.cuh"
 
 namespace lensed {
-LENSED_DEFINE_STATIC_TRACER(trace_static_c, 1, 1, 0, 0, 2, 0, 1, 0)
+#ifndef LENSED_MINB_C
+#define LENSED_MINB_C 3
+#endif
+LENSED_DEFINE_STATIC_TRACER(trace_static_c, LENSED_MINB_C, 1, 1, 0, 0, 2, 0, 1, 0)
 }  // namespace lensed

@@ -4,5 +4,8 @@
 #include "trace_static.cuh"
 
 namespace lensed {
-LENSED_DEFINE_STATIC_TRACER(trace_static_d, 1, 2, 0, 1, 2, 1, 1, 0)
+#ifndef LENSED_MINB_D
+#define LENSED_MINB_D 2
+#endif
+LENSED_DEFINE_STATIC_TRACER(trace_static_d, LENSED_MINB_D, 1, 2, 0, 1, 2, 1, 1, 0)
 }  // namespace lensed

@@ -126,12 +126,10 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
     }
 }
 
-#ifndef LENSED_TRACE_MIN_BLOCKS
-#define LENSED_TRACE_MIN_BLOCKS 3      // resident blocks per SM the register budget is cut for
-#endif
-
-template <int NP, class S>
-__global__ void __launch_bounds__(kTraceThreads, LENSED_TRACE_MIN_BLOCKS) trace_static_kernel(Program prog, TraceArgs a)
+// MINB = resident blocks per SM the register budget is cut for (3 -> 80 registers, 2 -> 128):
+// chosen per signature where it was measured (profiles/r1f.md)
+template <int NP, class S, int MINB>
+__global__ void __launch_bounds__(kTraceThreads, MINB) trace_static_kernel(Program prog, TraceArgs a)
 {
     extern __shared__ float4 smem4[];
     const TraceBlock tb = trace_prologue(prog, a, smem4);
@@ -152,15 +150,15 @@ __global__ void __launch_bounds__(kTraceThreads, LENSED_TRACE_MIN_BLOCKS) trace_
 }
 
 // R = rays per register block (2 NP); only the R values trace_pick_R can return
-template <class S>
+template <class S, int MINB>
 cudaError_t launch_trace_static(const Program &prog, const TraceArgs &a, int R, int nvec, cudaStream_t st)
 {
     switch (R) {
-    case 2: return launch_trace_kernel(trace_static_kernel<1, S>, prog, a, nvec, st);
-    case 4: return launch_trace_kernel(trace_static_kernel<2, S>, prog, a, nvec, st);
-    case 6: return launch_trace_kernel(trace_static_kernel<3, S>, prog, a, nvec, st);
-    case 8: return launch_trace_kernel(trace_static_kernel<4, S>, prog, a, nvec, st);
-    case 10: return launch_trace_kernel(trace_static_kernel<5, S>, prog, a, nvec, st);
+    case 2: return launch_trace_kernel(trace_static_kernel<1, S, MINB>, prog, a, nvec, st);
+    case 4: return launch_trace_kernel(trace_static_kernel<2, S, MINB>, prog, a, nvec, st);
+    case 6: return launch_trace_kernel(trace_static_kernel<3, S, MINB>, prog, a, nvec, st);
+    case 8: return launch_trace_kernel(trace_static_kernel<4, S, MINB>, prog, a, nvec, st);
+    case 10: return launch_trace_kernel(trace_static_kernel<5, S, MINB>, prog, a, nvec, st);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -168,13 +166,13 @@ cudaError_t launch_trace_static(const Program &prog, const TraceArgs &a, int R, 
 // Defines  bool NAME(counts, prog, args, R, nvec, stream, &err): false if the signature does
 // not match the list's per-kind counts, else launches and sets err.  One per .cu file, so
 // that the signatures compile in parallel (build.py).
-#define LENSED_DEFINE_STATIC_TRACER(NAME, ...)                                                          \
+#define LENSED_DEFINE_STATIC_TRACER(NAME, MINB, ...)                                                         \
     bool NAME(const int (&counts)[K_COUNT], const Program &prog, const TraceArgs &a, int R, int nvec,   \
               cudaStream_t st, cudaError_t *err)                                                        \
     {                                                                                                   \
         using S = TraceSig<__VA_ARGS__>;                                                                \
         if (!S::matches(counts)) return false;                                                          \
-        *err = launch_trace_static<S>(prog, a, R, nvec, st);                                            \
+        *err = launch_trace_static<S, MINB>(prog, a, R, nvec, st);                                           \
         return true;                                                                                    \
     }
 
