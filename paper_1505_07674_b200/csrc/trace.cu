@@ -147,7 +147,8 @@ size_t trace_smem_bytes(const Program &prog, int nq_pad)
 }
 
 // Rays carried per thread, R = 2 NP in {2, 4, 6, 8, 10}: least padded rule length, weighted
-// by a per-block overhead that shrinks with R (4 -> 4, 9 -> 10, 16 -> 8, 25 -> 10, 49 -> 10).
+// by a per-pass overhead that shrinks with R (4 -> 4, 9 -> 10, 16 -> 8, 25 -> 4, 49 -> 10;
+// measured on the multi-lens config, 25 points: R = 4 / 6 / 8 / 10 -> 34.8 / 37.3 / 38.9 / 38.8 ms).
 int trace_pick_R(int n_quad)
 {
 #ifdef LENSED_TRACE_FORCE_R            // tuning builds (build.py defines=...)
@@ -157,7 +158,7 @@ int trace_pick_R(int n_quad)
     double best_cost = 1e300;
     for (int R = 2; R <= 10; R += 2) {
         const int pad = (n_quad + R - 1) / R * R;
-        const double cost = pad * (1.0 + 0.6 / R);
+        const double cost = pad * (1.0 + 0.4 / R);
         if (cost < best_cost - 1e-12) { best = R; best_cost = cost; }
     }
     return best;
