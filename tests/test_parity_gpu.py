@@ -124,7 +124,7 @@ def test_paper_mock_scenario_gauss_kronrod_rule(L):
 
 
 # ------------------------------------------------- full sizes, bench launch configuration
-@pytest.mark.parametrize("index,B,n_sample", [(1, 1024, 6), (2, 4096, 3), (3, 4096, 2), (4, 1024, 2)])
+@pytest.mark.parametrize("index,B,n_sample", [(1, 1024, 6), (2, 4096, 3), (3, 4096, 2), (4, 16384, 3)])
 def test_full_size_configs_on_sampled_vectors(L, index, B, n_sample):
     import torch
     cfg = synth.get_config(index)
