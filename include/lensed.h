@@ -169,6 +169,22 @@ lensed_status lensed_set_static_tracer(lensed_handle *h, int on);
 int lensed_get_static_tracer(const lensed_handle *h);
 
 /*
+ * Quadrature error estimate ("an embedded three-point rule estimates the error
+ * of the integration for each pixel, which is saved with the output").
+ * lensed_set_error_rule: w_embedded [n_quad] host f32 = weights of the embedded lower-order
+ * rule at the abscissae given to lensed_create (0 at the points it does not use; for the
+ * Cartesian square of a Gauss-Kronrod rule: the products of the embedded Gauss weights),
+ * renormalised to sum 1.  EINVAL for NULL, non-finite values or a zero sum.  Synchronises
+ * the device.
+ * lensed_render_error: err_dev [B][H*W] device f32 receives, for every pixel (mask ignored),
+ *   | sum_k w_k I(x_k) - sum_k w'_k I(x_k) |
+ * of the UNCONVOLVED pixel luminosity (eq. 14, before the PSF); NaN for parameter vectors
+ * outside the model domain.  Asynchronous on `stream`.  EINVAL before an embedded rule is set.
+ * A diagnostic, not on the likelihood path: it runs the interpreting tracer.              */
+lensed_status lensed_set_error_rule(lensed_handle *h, const float *w_embedded);
+lensed_status lensed_render_error(lensed_handle *h, const float *params_dev, int B, float *err_dev, void *stream);
+
+/*
  * lensed_fma_peak -- FP32 FFMA micro-benchmark used as the measured roofline
  * denominator: runs `iters` dependent-chain FFMAs per thread on a full grid and returns
  * the achieved TFLOP/s (2 flops per FFMA) in *tflops.  Synchronous.                     */

@@ -119,6 +119,17 @@ def render_raw(H, W, scale, quad, kinds, params, zp=0.0):
     return out
 
 
+def error_map(H, W, scale, quad, w_embedded, kinds, params, zp=0.0):
+    """Per-pixel error estimate of the pixel quadrature: the definition written
+    out with render_raw,  | sum_k w_k I(x_k) - sum_k w'_k I(x_k) |,  w' = the embedded rule's
+    weights at the same abscissae (render_raw renormalises each weight set to sum 1, R6)."""
+    quad = _f64(quad).reshape(-1, 3)
+    emb = quad.copy()
+    emb[:, 2] = _f64(w_embedded)
+    return np.abs(render_raw(H, W, scale, quad, kinds, params, zp)
+                  - render_raw(H, W, scale, emb, kinds, params, zp))
+
+
 def convolve(L, psf):
     """eq. 15 with replicate padding and automatic PSF normalisation."""
     L = _f64(L)

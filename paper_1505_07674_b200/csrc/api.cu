@@ -34,6 +34,8 @@ struct lensed_handle {
     double scale = 0, zp = 0;
     Program prog{};
     int n_quad = 0, R = 1, nq_pad = 0;
+    std::vector<float4> h_quad;     // host copy of d_quad (lensed_set_error_rule rewrites .w)
+    bool has_error_rule = false;
     int KH = 1, KW = 1, NC = 1;
     int tile_w = 0, tile_h = 0;
     int Hp = 0, Wp = 0;             // padded frame of the unconvolved images (conv.cu "Input")
@@ -477,6 +479,7 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
         if (e2 != cudaSuccess) { lensed_destroy(h); return fail(nullptr, LENSED_ECUDA, "tap upload: %s", cudaGetErrorString(e2)); }
     }
     CREATE_FAIL(upload(h, &h->d_quad, hq.data(), hq.size()));
+    h->h_quad = hq;
     CREATE_FAIL(upload(h, &h->d_pix_ll, pix_ll.data(), pix_ll.size()));
     CREATE_FAIL(upload(h, &h->d_pix_all, pix_all.data(), pix_all.size()));
     CREATE_FAIL(upload(h, &h->d_tiles_ll, tiles_ll.data(), tiles_ll.size()));
@@ -488,6 +491,59 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
 
 int lensed_num_params(const lensed_handle *h) { return h ? h->prog.P : -1; }
 int lensed_num_traced(const lensed_handle *h) { return h ? h->npix_ll : -1; }
+
+lensed_status lensed_set_error_rule(lensed_handle *h, const float *w_embedded)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (!w_embedded) return fail(h, LENSED_EINVAL, "w_embedded is NULL");
+    double sum = 0.0;
+    for (int k = 0; k < h->n_quad; ++k) {
+        if (!isfinite(w_embedded[k])) return fail(h, LENSED_EINVAL, "w_embedded[%d] not finite", k);
+        sum += (double)w_embedded[k];
+    }
+    if (!(fabs(sum) > 0.0)) return fail(h, LENSED_EINVAL, "embedded weights sum to zero");
+    CU(h, cudaSetDevice(h->device));
+    CU(h, cudaDeviceSynchronize());                // no call of this handle may still read d_quad
+    for (int k = 0; k < h->n_quad; ++k)
+        h->h_quad[k].w = (float)((double)h->h_quad[k].z - (double)w_embedded[k] / sum);
+    CU(h, cudaMemcpy(h->d_quad, h->h_quad.data(), h->h_quad.size() * sizeof(float4), cudaMemcpyHostToDevice));
+    h->has_error_rule = true;
+    return LENSED_OK;
+}
+
+lensed_status lensed_render_error(lensed_handle *h, const float *params_dev, int B, float *err_dev, void *stream)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (!params_dev || !err_dev) return fail(h, LENSED_EINVAL, "null device pointer");
+    if (B < 1) return fail(h, LENSED_EINVAL, "B = %d < 1", B);
+    if (!h->has_error_rule) return fail(h, LENSED_EINVAL, "no embedded rule: call lensed_set_error_rule first");
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(h, cudaSetDevice(h->device));
+    const Program &prog = h->prog;
+    lensed_status s;
+    if ((s = grow(h, &h->d_derived, &h->cap_derived, (size_t)B * prog.D)) != LENSED_OK) return s;
+    PrepArgs pa{params_dev, h->d_derived, B, h->scale, h->zp, 0.5 * (h->W - 1), 0.5 * (h->H - 1)};
+    if ((s = timed_begin(h, PH_PREP, st)) != LENSED_OK) return s;
+    CU(h, launch_prep(prog, pa, st));
+    if ((s = timed_end(h, st)) != LENSED_OK) return s;
+    const size_t HW = (size_t)h->H * h->W;
+    for (int b0 = 0; b0 < B; b0 += 65535) {
+        const int nb = std::min(65535, B - b0);
+        TraceArgs ta{};
+        ta.derived = h->d_derived + (size_t)b0 * prog.D;
+        ta.pix = h->d_pix_all;
+        ta.quad = h->d_quad;
+        ta.err = err_dev + (size_t)b0 * HW;
+        ta.npix = h->npix_all; ta.nq_pad = h->nq_pad;
+        ta.H = h->H; ta.W = h->W;
+        ta.pix_per_block = ta.npix >= (1 << 16) ? 2048 : ta.npix >= (1 << 13) ? 1024 : 256;
+        ta.cxh = 0.5f * (h->W - 1); ta.cyh = 0.5f * (h->H - 1);
+        if ((s = timed_begin(h, PH_TRACE, st)) != LENSED_OK) return s;
+        CU(h, launch_trace(prog, ta, h->R, nb, false, st));
+        if ((s = timed_end(h, st)) != LENSED_OK) return s;
+    }
+    return LENSED_OK;
+}
 
 lensed_status lensed_render(lensed_handle *h, const float *params_dev, int B, float *model_dev, void *stream)
 {

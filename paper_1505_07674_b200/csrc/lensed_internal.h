@@ -84,7 +84,9 @@ struct PrepArgs {
 struct TraceArgs {
     const float *derived;  // [.][D], already offset to the chunk's first vector
     const uint32_t *pix;   // [npix] packed (row << 16) | column
-    const float4 *quad;    // [nq_pad] (xi, eta, w, 0), zero-weight padding up to a multiple of R (even)
+    const float4 *quad;    // [nq_pad] (xi, eta, w, w - w'), zero-weight padding up to a multiple of R (even);
+                           // w' = embedded rule of lensed_set_error_rule (0 before it is set)
+    float *err;            // [.][H*W] quadrature error estimates instead of L (trace.cu ERR), or NULL
     float *L;              // [.][Hp*Wp], chunk-local PADDED frames: pixel (i, j) at (i + py, j + px),
                            // border pixels replicated into the pad (conv.cu "Input")
     long long l_stride;    // Hp*Wp

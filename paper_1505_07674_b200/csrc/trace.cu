@@ -56,13 +56,26 @@ __device__ __forceinline__ void sie_by_mode(int mode, const float4 *d, const flo
     }
 }
 
-template <int NP>
+// ERR: instead of L_i, write the error estimate of the pixel quadrature
+//   | sum_k w_k I(x_k) - sum_k w'_k I(x_k) |,   w' = embedded lower-order rule,
+// accumulated as sum_k (w_k - w'_k) I(x_k), into a.err[vector][H][W] (NaN for vectors outside
+// the model domain).  A diagnostic output, not on the likelihood path: interpreter only.
+template <int NP, bool ERR>
 __global__ void __launch_bounds__(kTraceThreads, 2) trace_kernel(Program prog, TraceArgs a)
 {
     constexpr int R = 2 * NP;
     extern __shared__ float4 smem4[];
     const TraceBlock tb = trace_prologue(prog, a, smem4);
-    if (!tb.valid) return;
+    if (!tb.valid) {
+        if (ERR) {
+            const int base = blockIdx.x * a.pix_per_block, end = min(base + a.pix_per_block, a.npix);
+            for (int ip = base + threadIdx.x; ip < end; ip += kTraceThreads) {
+                const uint32_t rc = a.pix[ip];
+                a.err[(size_t)blockIdx.y * a.H * a.W + (size_t)(rc >> 16) * a.W + (rc & 0xffffu)] = nanf("");
+            }
+        }
+        return;
+    }
     const float4 *sder = tb.sder;
     const float *stab = tb.stab;
     const int nq = a.nq_pad;
@@ -130,11 +143,12 @@ __global__ void __launch_bounds__(kTraceThreads, 2) trace_kernel(Program prog, T
                 }
             }
             f2 w[NP];
-            load_pairs<NP>(tb.sw + q0, w);
+            load_pairs<NP>((ERR ? tb.sdw : tb.sw) + q0, w);
 #pragma unroll
             for (int k = 0; k < NP; ++k) acc = fma2(w[k], r.I[k], acc);
         }
-        store_pixel(a, Lb, row, col, (lo2(acc) + hi2(acc)) + tb.sky);
+        if (ERR) a.err[(size_t)blockIdx.y * a.H * a.W + (size_t)row * a.W + col] = fabsf(lo2(acc) + hi2(acc));
+        else store_pixel(a, Lb, row, col, (lo2(acc) + hi2(acc)) + tb.sky);
     }
 }
 
@@ -143,7 +157,7 @@ __global__ void __launch_bounds__(kTraceThreads, 2) trace_kernel(Program prog, T
 size_t trace_smem_bytes(const Program &prog, int nq_pad)
 {
     const size_t n_slots = 1 + prog.n_lens + prog.n_light;
-    return (size_t)prog.D * sizeof(float) + (n_slots * 2 + 1) * (size_t)nq_pad * sizeof(float);
+    return (size_t)prog.D * sizeof(float) + (n_slots * 2 + 2) * (size_t)nq_pad * sizeof(float);
 }
 
 // Rays carried per thread, R = 2 NP in {2, 4, 6, 8, 10}: least padded rule length, weighted
@@ -180,7 +194,7 @@ bool trace_has_static(const Program &prog)
 
 cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nvec, bool allow_static, cudaStream_t st)
 {
-    if (allow_static) {
+    if (allow_static && a.err == nullptr) {
         int counts[K_COUNT] = {0};
         for (int m = 0; m < prog.n_models; ++m) counts[prog.kind[m]] += 1;
         cudaError_t err = cudaSuccess;
@@ -188,12 +202,18 @@ cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nve
             trace_static_c(counts, prog, a, R, nvec, st, &err) || trace_static_d(counts, prog, a, R, nvec, st, &err))
             return err;
     }
+    const bool err = a.err != nullptr;
     switch (R) {
-    case 2: return launch_trace_kernel(trace_kernel<1>, prog, a, nvec, st);
-    case 4: return launch_trace_kernel(trace_kernel<2>, prog, a, nvec, st);
-    case 6: return launch_trace_kernel(trace_kernel<3>, prog, a, nvec, st);
-    case 8: return launch_trace_kernel(trace_kernel<4>, prog, a, nvec, st);
-    case 10: return launch_trace_kernel(trace_kernel<5>, prog, a, nvec, st);
+#define LENSED_CASE(NP)                                                                      \
+    case 2 * NP:                                                                             \
+        return err ? launch_trace_kernel(trace_kernel<NP, true>, prog, a, nvec, st)          \
+                   : launch_trace_kernel(trace_kernel<NP, false>, prog, a, nvec, st);
+        LENSED_CASE(1)
+        LENSED_CASE(2)
+        LENSED_CASE(3)
+        LENSED_CASE(4)
+        LENSED_CASE(5)
+#undef LENSED_CASE
     default: return cudaErrorInvalidValue;
     }
 }

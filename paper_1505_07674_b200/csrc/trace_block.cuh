@@ -5,7 +5,8 @@
 //
 // Shared memory of a block: [D/4] float4 derived constants of its vector, then the frame
 // tables  tab[slot][2][nq_pad]  (slot 0 = identity, 1 + m = lens m, 1 + n_lens + m = light
-// m; lenses and lights in the canonical order of api.cu), then the rule weights [nq_pad].
+// m; lenses and lights in the canonical order of api.cu), then the rule weights [nq_pad] and
+// the difference weights of the embedded rule [nq_pad].
 #pragma once
 #include "trace_math.cuh"
 
@@ -17,6 +18,7 @@ struct TraceBlock {
     const float4 *sder;   // derived constants of the vector
     const float *stab;    // frame tables
     const float *sw;      // rule weights
+    const float *sdw;     // rule weights minus the embedded rule's (error estimate, trace.cu)
     float sky;            // summed sky levels
     bool valid;
 };
@@ -34,7 +36,8 @@ __device__ __forceinline__ TraceBlock trace_prologue(const Program &prog, const 
         for (int i = threadIdx.x; i < prog.D / 4; i += kTraceThreads) sder[i] = g[i];
     }
     __syncthreads();
-    TraceBlock tb{sder, stab, sw, 0.0f, sder[0].x != 0.0f};
+    float *sdw = sw + nq;
+    TraceBlock tb{sder, stab, sw, sdw, 0.0f, sder[0].x != 0.0f};
     if (!tb.valid) return tb;                     // vector outside the model domain: block-uniform
     for (int m = 0; m < prog.n_light; ++m)
         if (prog.light_kind[m] == K_SKY) tb.sky += sder[prog.light_off[m] >> 2].x;
@@ -53,7 +56,7 @@ __device__ __forceinline__ TraceBlock trace_prologue(const Program &prog, const 
         }
         stab[(size_t)(2 * slot) * nq + k] = fmaf(m11, qk.x, m12 * qk.y);
         stab[(size_t)(2 * slot + 1) * nq + k] = fmaf(m21, qk.x, m22 * qk.y);
-        if (slot == 0) sw[k] = qk.z;
+        if (slot == 0) { sw[k] = qk.z; sdw[k] = qk.w; }
     }
     __syncthreads();
     return tb;

@@ -30,6 +30,8 @@ SYMBOLS = {
     "lensed_render": (_i, [_p, _p, _i, _p, _p]),
     "lensed_loglike": (_i, [_p, _p, _i, _p, _p]),
     "lensed_render_host": (_i, [_p, _p, _i, _p, _p]),
+    "lensed_set_error_rule": (_i, [_p, _p]),
+    "lensed_render_error": (_i, [_p, _p, _i, _p, _p]),
     "lensed_loglike_host": (_i, [_p, _p, _i, _p, _p]),
     "lensed_set_profiling": (_i, [_p, _i]),
     "lensed_get_profile": (_i, [_p, _p, _p]),
@@ -124,6 +126,20 @@ def lensed_render(h, params_dev, model_dev, stream=None):
     _check_out(model_dev, B)
     _check(lib().lensed_render(h, params_dev.data_ptr(), B, model_dev.data_ptr(), _stream(stream)), h)
     return model_dev
+
+
+def lensed_set_error_rule(h, w_embedded):
+    """w_embedded [n_quad]: weights of the embedded lower-order rule (host array)."""
+    w = _np(w_embedded, np.float32)
+    _check(lib().lensed_set_error_rule(h, _hp(w)), h)
+
+
+def lensed_render_error(h, params_dev, err_dev, stream=None):
+    """params_dev [B][P], err_dev [B][H][W]: contiguous float32 CUDA tensors."""
+    B = _check_dev(h, params_dev)
+    _check_out(err_dev, B)
+    _check(lib().lensed_render_error(h, params_dev.data_ptr(), B, err_dev.data_ptr(), _stream(stream)), h)
+    return err_dev
 
 
 def lensed_loglike(h, params_dev, logl_dev, stream=None):

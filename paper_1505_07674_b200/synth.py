@@ -49,20 +49,31 @@ def subsample_rule(n):
     return np.array(q, dtype=np.float64)
 
 
-_GK = {  # Gauss-Kronrod (Patterson 1968) nodes / Kronrod weights on [-1, 1]
+_GK = {  # Gauss-Kronrod (Patterson 1968) nodes / Kronrod weights / embedded Gauss weights on
+    # [-1, 1] (0 at the nodes the Gauss rule does not use)
     7: ([0.0, 0.434243749346802, 0.774596669241483, 0.960491268708020],
-        [0.450916538658474, 0.401397414775962, 0.268488089868333, 0.104656226026467]),
+        [0.450916538658474, 0.401397414775962, 0.268488089868333, 0.104656226026467],
+        [8.0 / 9.0, 0.0, 5.0 / 9.0, 0.0]),
 }
 
 
 def gauss_kronrod_rule(n=7):
     """Cartesian square of the n-point Kronrod rule (the paper's default g3k7 for n = 7)."""
-    xs, ws = _GK[n]
+    xs, ws, _ = _GK[n]
     x = np.array([-v for v in xs[:0:-1]] + xs)
     w = np.array(ws[:0:-1] + ws)
     x, w = 0.5 * x, 0.5 * w
     q = [(x[a], x[b], w[a] * w[b]) for b in range(n) for a in range(n)]
     return np.array(q, dtype=np.float64)
+
+
+def gauss_kronrod_embedded_weights(n=7):
+    """Weights of the embedded Gauss rule (3-point for n = 7) at the abscissae of
+    gauss_kronrod_rule(n), same order, summing to 1: the rule whose difference from the Kronrod
+    sum is the per-pixel error estimate of PAPER.md:166."""
+    _, _, gs = _GK[n]
+    g = 0.5 * np.array(gs[:0:-1] + gs)
+    return np.array([g[a] * g[b] for b in range(n) for a in range(n)], dtype=np.float64)
 
 
 # ------------------------------------------------------------------------------ PSFs

@@ -541,3 +541,74 @@ def test_chi2_per_dof_is_about_one_at_the_truth():
     d, w = cfg.observe(truth)
     ll = orc.loglike(cfg.H, cfg.W, cfg.scale, d, w, None, cfg.psf, cfg.quad, kinds, cfg.truth)[0]
     assert 0.85 < -2 * ll / (cfg.H * cfg.W) < 1.15
+
+
+# ------------------------------------------------- quadrature error estimate
+def test_embedded_gauss_weights_are_the_three_point_rule_on_the_kronrod_nodes():
+    quad = synth.gauss_kronrod_rule(7)
+    emb = synth.gauss_kronrod_embedded_weights(7)
+    assert emb.sum() == pytest.approx(1.0, abs=1e-15) and np.count_nonzero(emb) == 9
+    # the nonzero points are the 3 x 3 Gauss-Legendre rule on the pixel, weights included
+    gl = synth.gauss_legendre_rule(3)
+    mine = sorted((round(x, 12), round(y, 12), round(w, 12)) for (x, y, _), w in zip(quad, emb) if w != 0)
+    ref = sorted((round(x, 12), round(y, 12), round(w, 12)) for x, y, w in gl)
+    assert np.allclose(mine, ref, atol=1e-11)
+
+
+def test_error_map_vanishes_for_what_both_rules_integrate_exactly():
+    # constant sky: both weight sets sum to one -> the estimate is zero up to rounding
+    quad, emb = synth.gauss_kronrod_rule(7), synth.gauss_kronrod_embedded_weights(7)
+    e = orc.error_map(6, 5, 0.05, quad, emb, [orc.FG_SKY], [0.37])
+    assert np.all(e <= 1e-15)
+
+
+def test_error_map_of_a_separable_gaussian_is_the_product_of_one_dimensional_rules():
+    """A circular Gaussian is exp(-x^2/2s^2) exp(-y^2/2s^2): on a pixel the Cartesian-square
+    rule gives K1(x) K1(y) and the embedded rule G1(x) G1(y), K1 / G1 = the one-dimensional
+    7-point Kronrod / 3-point Gauss sums, evaluated here from the node table of the paper's
+    reference (Patterson 1968) without the oracle."""
+    kx = np.array([0.0, 0.434243749346802, 0.774596669241483, 0.960491268708020])
+    kw = np.array([0.450916538658474, 0.401397414775962, 0.268488089868333, 0.104656226026467])
+    x1 = 0.5 * np.concatenate([-kx[:0:-1], kx])
+    w1 = 0.5 * np.concatenate([kw[:0:-1], kw])
+    g1x, g1w = 0.5 * np.array([-math.sqrt(0.6), 0.0, math.sqrt(0.6)]), 0.5 * np.array([5 / 9, 8 / 9, 5 / 9])
+    H, W, s, sig = 7, 6, 0.05, 0.02                  # sigma = 0.4 px: badly resolved on purpose
+    cx, cy = 0.013, -0.021
+    F = 3.0
+    i0 = F / (2 * math.pi * sig * sig) * s * s       # brightness per pixel area (R6, R7)
+    quad, emb = synth.gauss_kronrod_rule(7), synth.gauss_kronrod_embedded_weights(7)
+    e = orc.error_map(H, W, s, quad, emb, [orc.FG_GAUSS], [cx, cy, sig, synth.mag_of_flux(F), 1.0, 0.0])
+
+    def rule(nodes, weights, c):
+        return np.sum(weights * np.exp(-((c + nodes * s) ** 2) / (2 * sig * sig)))
+
+    expect = np.empty((H, W))
+    for i in range(H):
+        for j in range(W):
+            xc, yc = (j - 0.5 * (W - 1)) * s - cx, (i - 0.5 * (H - 1)) * s - cy
+            expect[i, j] = i0 * abs(rule(x1, w1, xc) * rule(x1, w1, yc) - rule(g1x, g1w, xc) * rule(g1x, g1w, yc))
+    assert e.max() > 1e-4 * i0                       # the estimate is not trivially small here
+    assert np.allclose(e, expect, rtol=1e-10, atol=1e-14 * i0)
+
+
+def test_error_map_tracks_the_true_error_of_the_embedded_rule():
+    """The Kronrod sum is far more accurate than the embedded Gauss sum, so |K - G| must be
+    the Gauss rule's true error; the exact pixel integral of a circular Gaussian is a product
+    of erf differences."""
+    H, W, s, sig = 5, 5, 0.05, 0.04
+    cx, cy, F = 0.004, 0.009, 1.0
+    p = [cx, cy, sig, synth.mag_of_flux(F), 1.0, 0.0]
+    quad, emb = synth.gauss_kronrod_rule(7), synth.gauss_kronrod_embedded_weights(7)
+    e = orc.error_map(H, W, s, quad, emb, [orc.FG_GAUSS], p)
+    gq = quad.copy(); gq[:, 2] = emb
+    g = orc.render_raw(H, W, s, gq, [orc.FG_GAUSS], p)
+
+    def cdf(c):                                       # integral over one pixel side, centre offset c
+        r = sig * math.sqrt(2.0)
+        return 0.5 * (math.erf((c + 0.5 * s) / r) - math.erf((c - 0.5 * s) / r))
+
+    exact = np.array([[F * cdf((j - 0.5 * (W - 1)) * s - cx) * cdf((i - 0.5 * (H - 1)) * s - cy)
+                       for j in range(W)] for i in range(H)])
+    true_err = np.abs(exact - g)
+    assert true_err.max() > 1e-5 * exact.max()
+    assert np.allclose(e, true_err, rtol=0.02, atol=1e-3 * true_err.max())

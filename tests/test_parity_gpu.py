@@ -279,3 +279,42 @@ def test_create_rejects_bad_arguments_on_the_gpu_box_too(L):
     with pytest.raises(L.LensedError) as e:
         L.lensed_create(img, -w, None, None, cfg.quad, kinds, 0.05)
     assert e.value.status == L.EINVAL
+
+
+# --------------------------------------------------- quadrature error estimate
+def test_quadrature_error_map_of_the_gauss_kronrod_rule(L):
+    """lensed_render_error against the oracle's |K - G| on the paper-mock list with the default
+    g3k7 rule; the estimate is a small difference of two FP32 sums, so the bound is absolute:
+    1e-5 of the pixel's own luminosity (floored at 1e-3 of the image peak)."""
+    import torch
+    from oracle import lensed_oracle as orc
+    models = ("sie", "shear", "src_sersic", "fg_sersic", "sky")
+    base = synth.shrunk(synth.get_config(1), 40, 44, 5)
+    quad, emb = synth.gauss_kronrod_rule(7), synth.gauss_kronrod_embedded_weights(7)
+    cfg = synth.Config(1, "gk", base.H, base.W, base.scale, models, quad, base.psf, None, base.truth, 5,
+                       base._draw, 0.005, 2000.0)
+    params = cfg.batch()
+    params[4, 3] = 1.5                                   # q > 1: outside the domain -> NaN map
+    h = Problem(cfg).create()
+    try:
+        p = torch.from_numpy(params).cuda()
+        err = torch.empty((len(params), cfg.H, cfg.W), dtype=torch.float32, device="cuda")
+        with pytest.raises(L.LensedError):
+            L.lensed_render_error(h, p, err)             # no embedded rule yet
+        L.lensed_set_error_rule(h, emb)
+        L.lensed_render_error(h, p, err)
+        logl = torch.empty(len(params), dtype=torch.float32, device="cuda")
+        L.lensed_loglike(h, p, logl)                     # the likelihood path is untouched by the rule
+        torch.cuda.synchronize()
+        err = err.cpu().numpy()
+    finally:
+        L.lensed_destroy(h)
+    kinds = synth.kind_ids(models)
+    assert np.all(np.isnan(err[4])) and np.isneginf(logl[4].item())
+    for b in range(4):
+        ref = orc.error_map(cfg.H, cfg.W, cfg.scale, quad, emb, kinds, params[b], zp=cfg.zp)
+        raw = orc.render_raw(cfg.H, cfg.W, cfg.scale, quad, kinds, params[b], zp=cfg.zp)
+        bound = 1e-5 * np.maximum(raw, 1e-3 * raw.max())
+        assert ref.max() > 10 * bound.max()              # the map is well above the bound somewhere
+        assert np.all(np.abs(err[b] - ref) <= bound), "error map off by %.3g of the bound" % (
+            np.abs(err[b] - ref) / bound).max()
