@@ -169,6 +169,24 @@ lensed_status lensed_set_static_tracer(lensed_handle *h, int on);
 int lensed_get_static_tracer(const lensed_handle *h);
 
 /*
+ * lensed_estimate_weights -- create-time variance estimation from the data (PAPER.md:190-212
+ * eqs. 18-21), for observations without an independent variance map: photon counts
+ * k_i = g_i (d_i + b_i) are Poisson, so  s_i^2 = (d_i + b_i) / g_i  and
+ *   w_i = x_i / s_i^2 = x_i g_i / (d_i + b_i).
+ *   image   [n] host f32, d_i
+ *   gain    [n] host f32 or NULL (then gain0 for every pixel): effective gain g_i > 0 (eq. 19)
+ *   offset  [n] host f32 or NULL (then offset0): b_i, what was subtracted from the data
+ *   extra   [n] host f32 or NULL (then 1): the multiplicative extra weight factor x_i >= 0
+ *   weight  [n] host f32, receives w_i, ready for lensed_create
+ * Pixels whose estimated counts are not positive (d_i + b_i <= 0) cannot be given a Poisson
+ * variance and get w_i = 0, i.e. they are masked (reading R15).  Host arithmetic in
+ * double; no device is touched.  EINVAL for NULL image / weight, n < 1, a gain <= 0, a
+ * negative extra factor or a non-finite input.                                            */
+lensed_status lensed_estimate_weights(long long n, const float *image, const float *gain, double gain0,
+                                      const float *offset, double offset0, const float *extra,
+                                      float *weight);
+
+/*
  * Quadrature error estimate ("an embedded three-point rule estimates the error
  * of the integration for each pixel, which is saved with the output").
  * lensed_set_error_rule: w_embedded [n_quad] host f32 = weights of the embedded lower-order

@@ -492,6 +492,24 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
 int lensed_num_params(const lensed_handle *h) { return h ? h->prog.P : -1; }
 int lensed_num_traced(const lensed_handle *h) { return h ? h->npix_ll : -1; }
 
+lensed_status lensed_estimate_weights(long long n, const float *image, const float *gain, double gain0,
+                                      const float *offset, double offset0, const float *extra, float *weight)
+{
+    if (!image || !weight) return fail(nullptr, LENSED_EINVAL, "image / weight is NULL");
+    if (n < 1) return fail(nullptr, LENSED_EINVAL, "n = %lld < 1", n);
+    for (long long i = 0; i < n; ++i) {
+        const double d = image[i], g = gain ? (double)gain[i] : gain0, b = offset ? (double)offset[i] : offset0;
+        const double x = extra ? (double)extra[i] : 1.0;
+        if (!isfinite(d) || !isfinite(g) || !isfinite(b) || !isfinite(x))
+            return fail(nullptr, LENSED_EINVAL, "non-finite input at pixel %lld", i);
+        if (!(g > 0.0)) return fail(nullptr, LENSED_EINVAL, "gain %g at pixel %lld is not > 0", g, i);
+        if (x < 0.0) return fail(nullptr, LENSED_EINVAL, "extra weight %g at pixel %lld is negative", x, i);
+        const double counts_over_g2 = (d + b) / g;           // s_i^2, eq. 21
+        weight[i] = counts_over_g2 > 0.0 ? (float)(x / counts_over_g2) : 0.0f;
+    }
+    return LENSED_OK;
+}
+
 lensed_status lensed_set_error_rule(lensed_handle *h, const float *w_embedded)
 {
     if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");

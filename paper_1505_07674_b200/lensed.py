@@ -30,6 +30,7 @@ SYMBOLS = {
     "lensed_render": (_i, [_p, _p, _i, _p, _p]),
     "lensed_loglike": (_i, [_p, _p, _i, _p, _p]),
     "lensed_render_host": (_i, [_p, _p, _i, _p, _p]),
+    "lensed_estimate_weights": (_i, [_ll, _p, _p, _d, _p, _d, _p, _p]),
     "lensed_set_error_rule": (_i, [_p, _p]),
     "lensed_render_error": (_i, [_p, _p, _i, _p, _p]),
     "lensed_loglike_host": (_i, [_p, _p, _i, _p, _p]),
@@ -126,6 +127,18 @@ def lensed_render(h, params_dev, model_dev, stream=None):
     _check_out(model_dev, B)
     _check(lib().lensed_render(h, params_dev.data_ptr(), B, model_dev.data_ptr(), _stream(stream)), h)
     return model_dev
+
+
+def lensed_estimate_weights(image, gain, offset=0.0, extra=None):
+    """w = extra * gain / (image + offset) (eqs. 18-21); gain / offset: scalars or maps."""
+    img = _np(image, np.float32)
+    g = None if np.isscalar(gain) else _np(gain, np.float32)
+    b = None if np.isscalar(offset) else _np(offset, np.float32)
+    x = _np(extra, np.float32)
+    out = np.empty(img.shape, dtype=np.float32)
+    _check(lib().lensed_estimate_weights(img.size, _hp(img), _hp(g), float(gain) if g is None else 0.0,
+                                         _hp(b), float(offset) if b is None else 0.0, _hp(x), _hp(out)))
+    return out
 
 
 def lensed_set_error_rule(h, w_embedded):

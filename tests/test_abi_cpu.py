@@ -94,3 +94,41 @@ def test_product_code_never_imports_the_oracle():
             if f.endswith((".py", ".cu", ".h", ".cuh")):
                 text = open(os.path.join(dirpath, f)).read()
                 assert "lensed_oracle" not in text and "import oracle" not in text and "from oracle" not in text, f
+
+
+# ------------------------------------------- create-time variance estimation (eqs. 18-21)
+def test_estimate_weights_is_gain_over_counts_with_scalars_or_maps():
+    from paper_1505_07674_b200 import lensed
+    d = np.array([3.0, 0.5, 10.0, -0.25], dtype=np.float32)
+    w = lensed.lensed_estimate_weights(d, 2.0, 0.25)
+    # s^2 = (d + b) / g  ->  w = g / (d + b); hand-computed: 2/3.25, 2/0.75, 2/10.25; d + b = 0 -> masked
+    assert np.allclose(w, [0.6153846, 2.6666667, 0.19512195, 0.0], rtol=1e-6)
+    gmap, bmap = np.full(4, 2.0, np.float32), np.full(4, 0.25, np.float32)
+    assert np.array_equal(w, lensed.lensed_estimate_weights(d, gmap, bmap))
+    x = np.array([1.0, 0.5, 0.0, 2.0], dtype=np.float32)
+    assert np.allclose(lensed.lensed_estimate_weights(d, gmap, bmap, x), w * x, rtol=1e-7)
+
+
+def test_estimated_weights_normalise_poisson_residuals():
+    """d = k/g - b with k ~ Poisson(mu): Var(d) = mu/g^2, and eq. 21 estimates it by (d + b)/g =
+    k/g^2, so sum_i w_i (d_i - E d_i)^2 / n -> E[(k - mu)^2 / k] ~ 1 for large mu."""
+    from paper_1505_07674_b200 import lensed
+    rng = np.random.default_rng(150507674)
+    mu, g, b = 400.0, 3.0, 20.0
+    k = rng.poisson(mu, size=200000)
+    d = (k / g - b).astype(np.float32)
+    w = lensed.lensed_estimate_weights(d, g, b)
+    chi2_per_pixel = np.mean(w.astype(np.float64) * (d.astype(np.float64) - (mu / g - b)) ** 2)
+    assert abs(chi2_per_pixel - 1.0) < 0.02
+
+
+@pytest.mark.parametrize("kwargs", [dict(gain=0.0), dict(gain=-1.0), dict(gain=float("nan")),
+                                    dict(extra=np.array([1.0, -0.1], np.float32)),
+                                    dict(offset=float("inf"))])
+def test_estimate_weights_rejects_bad_arguments(kwargs):
+    from paper_1505_07674_b200 import lensed
+    args = dict(image=np.array([1.0, 2.0], np.float32), gain=1.0, offset=0.0, extra=None)
+    args.update(kwargs)
+    with pytest.raises(lensed.LensedError) as e:
+        lensed.lensed_estimate_weights(**args)
+    assert e.value.status == lensed.EINVAL
