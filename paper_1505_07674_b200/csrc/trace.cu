@@ -39,6 +39,7 @@ LENSED_DECLARE_STATIC_TRACER(trace_static_a)
 LENSED_DECLARE_STATIC_TRACER(trace_static_b)
 LENSED_DECLARE_STATIC_TRACER(trace_static_c)
 LENSED_DECLARE_STATIC_TRACER(trace_static_d)
+LENSED_DECLARE_STATIC_TRACER(trace_static_e)
 
 namespace {
 
@@ -183,7 +184,7 @@ bool trace_has_static(const Program &prog)
     int counts[K_COUNT] = {0};
     for (int m = 0; m < prog.n_models; ++m) counts[prog.kind[m]] += 1;
     // the same list as in launch_trace
-    const int sigs[][8] = {{0, 0, 1, 0, 0, 1, 0, 0}, {1, 1, 0, 0, 1, 0, 1, 0}, {1, 1, 0, 0, 2, 0, 1, 0}, {1, 2, 0, 1, 2, 1, 1, 0}};
+    const int sigs[][8] = {{0, 0, 1, 0, 0, 1, 0, 0}, {1, 1, 0, 0, 1, 0, 1, 0}, {1, 1, 0, 0, 2, 0, 1, 0}, {1, 2, 0, 1, 2, 1, 1, 0}, {0, 1, 0, 0, 1, 0, 1, 0}};
     for (const auto &s : sigs)
         if (counts[K_SHEAR] == s[0] && counts[K_SIE] == s[1] && counts[K_SIS] == s[2] && counts[K_POINT] == s[3] &&
             counts[K_SRC_SERSIC] == s[4] && counts[K_SRC_GAUSS] == s[5] && counts[K_FG_SERSIC] == s[6] &&
@@ -199,7 +200,8 @@ cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nve
         for (int m = 0; m < prog.n_models; ++m) counts[prog.kind[m]] += 1;
         cudaError_t err = cudaSuccess;
         if (trace_static_a(counts, prog, a, R, nvec, st, &err) || trace_static_b(counts, prog, a, R, nvec, st, &err) ||
-            trace_static_c(counts, prog, a, R, nvec, st, &err) || trace_static_d(counts, prog, a, R, nvec, st, &err))
+            trace_static_c(counts, prog, a, R, nvec, st, &err) || trace_static_d(counts, prog, a, R, nvec, st, &err) ||
+            trace_static_e(counts, prog, a, R, nvec, st, &err))
             return err;
     }
     const bool err = a.err != nullptr;

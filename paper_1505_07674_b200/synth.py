@@ -170,6 +170,30 @@ SLACS_MODELS = ("sie", "shear", "src_sersic", "src_sersic", "fg_sersic", "sky")
 MULTI_MODELS = ("sie", "sie", "point", "shear", "src_sersic", "src_sersic", "src_gauss",
                 "fg_sersic", "sky")
 
+MOCK_MODELS = ("sie", "fg_sersic", "src_sersic")
+_MOCK_TRUTH = [0.0, 0.0, 1.3624, 0.75, 20.0,
+               0.0, 0.0, 2.0, mag_of_flux(3000.0), 4.0, 0.75, 20.0,
+               0.12, -0.08, 0.2, mag_of_flux(30.0), 2.0, 0.5, 100.0]
+
+
+def _draw_mock(rng, B):
+    """lens fixed type, sources with n in [0.5, 8], q in [0.1, 1],
+    r in [0.1, 0.4]", placed in a disc about the caustic; host n = 4 (de Vaucouleurs, R12)."""
+    t = np.tile(np.array(_MOCK_TRUTH), (B, 1))
+    t[:, [0, 1, 5, 6]] += rng.uniform(-0.05, 0.05, size=(B, 4))
+    t[:, 2] = rng.uniform(1.0, 1.5, size=B)
+    t[:, 3] = rng.uniform(0.5, 1.0, size=B)
+    t[:, 4] = rng.uniform(0.0, 180.0, size=B)
+    t[:, 7] *= rng.uniform(0.8, 1.2, size=B)
+    sx, sy = _disc(rng, 0.5, B)
+    t[:, 12], t[:, 13] = sx, sy
+    t[:, 14] = rng.uniform(0.1, 0.4, size=B)
+    t[:, 16] = rng.uniform(0.5, 8.0, size=B)
+    t[:, 17] = rng.uniform(0.1, 1.0, size=B)
+    t[:, 18] = rng.uniform(0.0, 180.0, size=B)
+    return t
+
+
 _HST_TRUTH = [0.02, -0.03, 1.2, 0.75, 35.0, 0.03, -0.02,
               0.15, 0.10, 0.15, mag_of_flux(20.0), 1.5, 0.6, 70.0,
               0.02, -0.03, 1.0, mag_of_flux(2000.0), 4.0, 0.8, 30.0, 0.01]
@@ -282,7 +306,15 @@ def get_config(index):
     if index == 4:
         return Config(4, "euclid", 512, 512, 0.1, HST_MODELS, subsample_rule(4),
                       moffat_psf(31, 1.8, 2.5), None, _HST_TRUTH, 16384, _draw_hst, 0.005, 2000.0)
-    raise ValueError("config index 0..4")
+    if index == 5:
+        # The paper's own mock scenario: 120x120 at
+        # 0.05"/px, SIE + de Vaucouleurs host + Sersic source (18 parameters), default g3k7 rule
+        # (PAPER.md:166).  Context for "thousands of individual parameter settings per second"
+        # (PAPER.md:445), not one of BASELINE.json's configs.  The TinyTim PSF is not in the
+        # container: a 15x15 Moffat (beta = 3, FWHM 0.1") stands in for it.
+        return Config(5, "mock", 120, 120, 0.05, MOCK_MODELS, gauss_kronrod_rule(7),
+                      moffat_psf(15, 2.0, 3.0), None, _MOCK_TRUTH, 4096, _draw_mock, 0.005, 2000.0)
+    raise ValueError("config index 0..5")
 
 
 def shrunk(cfg, H, W, B):

@@ -76,7 +76,8 @@ def test_shrunk_configs_span_tiles_and_ragged_tails(L, index, H, W, B):
     _check(L, prob, np.vstack([cfg.batch(), cfg.truth.astype(np.float32)[None]]))
 
 
-@pytest.mark.parametrize("index,H,W,B", [(0, 32, 32, 16), (1, 90, 70, 24), (2, 75, 93, 12), (3, 70, 80, 8), (4, 101, 67, 6)])
+@pytest.mark.parametrize("index,H,W,B", [(0, 32, 32, 16), (1, 90, 70, 24), (2, 75, 93, 12), (3, 70, 80, 8), (4, 101, 67, 6),
+                                         (5, 60, 64, 6)])
 @pytest.mark.parametrize("static", [True, False])
 def test_both_tracers_on_every_config_list(L, index, H, W, B, static):
     """The model lists of BASELINE.json's configs have a compile-time specialised tracer; the
@@ -124,7 +125,7 @@ def test_paper_mock_scenario_gauss_kronrod_rule(L):
 
 
 # ------------------------------------------------- full sizes, bench launch configuration
-@pytest.mark.parametrize("index,B,n_sample", [(1, 1024, 6), (2, 4096, 3), (3, 4096, 2), (4, 16384, 3)])
+@pytest.mark.parametrize("index,B,n_sample", [(1, 1024, 6), (2, 4096, 3), (3, 4096, 2), (4, 16384, 3), (5, 4096, 3)])
 def test_full_size_configs_on_sampled_vectors(L, index, B, n_sample):
     import torch
     cfg = synth.get_config(index)

@@ -6,7 +6,8 @@ from paper_1505_07674_b200 import synth
 
 def test_configs_have_the_baseline_shapes():
     want = [(32, 32, 9, 4, None, 16), (100, 100, 22, 9, (9, 9), 1024), (200, 200, 29, 16, (21, 21), 4096),
-            (256, 256, 43, 25, (15, 15), 4096), (512, 512, 22, 16, (31, 31), 16384)]
+            (256, 256, 43, 25, (15, 15), 4096), (512, 512, 22, 16, (31, 31), 16384),
+            (120, 120, 19, 49, (15, 15), 4096)]                 # 5 = the paper's mock scenario (context)
     for c, (H, W, P, N, psf, B) in enumerate(want):
         cfg = synth.get_config(c)
         assert (cfg.H, cfg.W, cfg.P, len(cfg.quad), cfg.B) == (H, W, P, N, B)
