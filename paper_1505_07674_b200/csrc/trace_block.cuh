@@ -19,6 +19,7 @@ struct TraceBlock {
     const float *stab;    // frame tables
     const float *sw;      // rule weights
     const float *sdw;     // rule weights minus the embedded rule's (error estimate, trace.cu)
+    float4 *smat;         // [n_light] scratch matrices (trace_static.cuh "direct frames")
     float sky;            // summed sky levels
     bool valid;
 };
@@ -37,7 +38,8 @@ __device__ __forceinline__ TraceBlock trace_prologue(const Program &prog, const 
     }
     __syncthreads();
     float *sdw = sw + nq;
-    TraceBlock tb{sder, stab, sw, sdw, 0.0f, sder[0].x != 0.0f};
+    float4 *smat = reinterpret_cast<float4 *>(sdw + nq);      // nq is even and the tables are 16-byte aligned
+    TraceBlock tb{sder, stab, sw, sdw, smat, 0.0f, sder[0].x != 0.0f};
     if (!tb.valid) return tb;                     // vector outside the model domain: block-uniform
     for (int m = 0; m < prog.n_light; ++m)
         if (prog.light_kind[m] == K_SKY) tb.sky += sder[prog.light_off[m] >> 2].x;

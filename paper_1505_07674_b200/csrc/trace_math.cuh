@@ -158,7 +158,10 @@ __device__ __forceinline__ void sie_origin(const float4 *d, float jf, float rf, 
     v0 = fmaf(c1.x, dy, -c1.y * dx);
 }
 
-template <int NP, int MODE>
+// RAW: leave (atan, atanh-in-lg2-units) themselves in (r.ax, r.ay) instead of accumulating the
+// deflection: the sources then subtract B (atan, atanh), B = M_source x [amplitudes, rotation]
+// (trace_static.cuh "direct frames").
+template <int NP, int MODE, bool RAW = false>
 __device__ __forceinline__ void lens_sie(const float4 *d, const float *tu, const float *tv, float u0, float v0,
                                          Rays<NP> &r)
 {
@@ -174,8 +177,13 @@ __device__ __forceinline__ void lens_sie(const float4 *d, const float *tu, const
         const f2 s = mul2(ipsi, bc(c1.w));
         const f2 at = sie_atan2x<MODE>(mul2(u, s));
         const f2 lv = sie_atanh2x<MODE>(v, s);
-        r.ax[k] = fma2(lv, bc(c2.w), fma2(at, bc(c2.x), r.ax[k]));
-        r.ay[k] = fma2(lv, bc(c2.z), fma2(at, bc(c2.y), r.ay[k]));
+        if (RAW) {
+            r.ax[k] = at;
+            r.ay[k] = lv;
+        } else {
+            r.ax[k] = fma2(lv, bc(c2.w), fma2(at, bc(c2.x), r.ax[k]));
+            r.ay[k] = fma2(lv, bc(c2.z), fma2(at, bc(c2.y), r.ay[k]));
+        }
     }
 }
 
@@ -247,11 +255,13 @@ __device__ __forceinline__ void light_origin(const float4 *d, float jf, float rf
     v0 = fmaf(c1.z, dx, c1.w * dy);
 }
 
+// cm: the 2 x 2 matrix applied to (r.ax, r.ay) of a source -- the frame M itself (d[1]) when
+// they hold the deflection, B when they hold the SIE's raw functions.
 template <int NP, bool SRC, bool GAUSS, bool INIT>
 __device__ __forceinline__ void light_profile(const float4 *d, const float *tu, const float *tv, float u0, float v0,
-                                              Rays<NP> &r)
+                                              Rays<NP> &r, const float4 *cm = nullptr)
 {
-    const float4 c1 = d[1], c2 = d[2];
+    const float4 c1 = cm ? cm[0] : d[1], c2 = d[2];
     const float nk = -c2.y;
     f2 pu[NP], pv[NP];
     load_pairs<NP>(tu, pu);

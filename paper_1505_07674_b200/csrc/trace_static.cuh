@@ -21,6 +21,14 @@ struct TraceSig {
     static constexpr int n_ss = NSS, n_sg = NSG, n_fs = NFS, n_fg = NFG;
     static constexpr int n_lens = NSHEAR + NSIE + NSIS + NPOINT;
     static constexpr int n_pos = NSS + NSG + NFS + NFG;          // positioned lights (sky excluded)
+    static constexpr int n_src = NSS + NSG;
+    // "Direct frames": with one SIE and no other non-linear lens, the deflection is never
+    // formed.  alpha = Gamma (x - x_c) + R diag(A, A l) (atan, atanh), so in a source frame
+    //   M (x - c - alpha) = [M (x - c) - M Gamma (x - x_c)]  -  B (atan, atanh),   B = M R diag(A, A l):
+    // the bracket is linear in x -- the source's table and per-pixel origin absorb the shear --
+    // and the SIE leaves its two raw functions in (ax, ay).  Saves the two packed adds of the
+    // shear and the four packed FMAs of the SIE's accumulation per pair of rays.
+    static constexpr bool direct = NSIE == 1 && NSIS == 0 && NPOINT == 0 && NSS + NSG >= 1;
     static bool matches(const int (&c)[K_COUNT])
     {
         return c[K_SHEAR] == NSHEAR && c[K_SIE] == NSIE && c[K_SIS] == NSIS && c[K_POINT] == NPOINT &&
@@ -59,12 +67,22 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
             circular_origin(sder + (prog.lens_off[L_SIS + i] >> 2), jf, rf, lu[L_SIS + i], lv[L_SIS + i]);
 #pragma unroll
         for (int i = 0; i < NPOS; ++i) light_origin(sder + (prog.light_off[i] >> 2), jf, rf, gu[i], gv[i]);
+        if (S::direct && S::n_shear) {
+#pragma unroll
+            for (int i = 0; i < S::n_src; ++i) {              // sources come first among the lights
+                const float4 M = sder[(prog.light_off[i] >> 2) + 1];
+                gu[i] -= fmaf(M.x, lu[0], M.y * lv[0]);
+                gv[i] -= fmaf(M.z, lu[0], M.w * lv[0]);
+            }
+        }
 
         f2 acc = bc(0.0f);
 #pragma unroll 1
         for (int q0 = 0; q0 < nq; q0 += R) {
             Rays<NP> r;
-            if (S::n_shear) {
+            if (S::direct) {
+                // (ax, ay) are set by the SIE below
+            } else if (S::n_shear) {
                 lens_shear<NP, true>(ltab + q0, ltab + nq + q0, lu[0], lv[0], r);
             } else {
 #pragma unroll
@@ -73,8 +91,8 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
 #pragma unroll
             for (int i = 0; i < S::n_sie; ++i) {
                 const int m = L_SIE + i;
-                lens_sie<NP, MODE>(sder + (prog.lens_off[m] >> 2), ltab + (size_t)(2 * m) * nq + q0,
-                                   ltab + (size_t)(2 * m + 1) * nq + q0, lu[m], lv[m], r);
+                lens_sie<NP, MODE, S::direct>(sder + (prog.lens_off[m] >> 2), ltab + (size_t)(2 * m) * nq + q0,
+                                              ltab + (size_t)(2 * m + 1) * nq + q0, lu[m], lv[m], r);
             }
             // SIS / point mass: identity frame = slot 0
 #pragma unroll
@@ -94,7 +112,8 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
             // foreground lights first: they do not wait for the deflection
 #define LENSED_LIGHT(m, SRC, GAUSS, INIT)                                                                     \
     light_profile<NP, SRC, GAUSS, INIT>(sder + (prog.light_off[m] >> 2), gtab + (size_t)(2 * (m)) * nq + q0, \
-                                        gtab + (size_t)(2 * (m) + 1) * nq + q0, gu[m], gv[m], r)
+                                        gtab + (size_t)(2 * (m) + 1) * nq + q0, gu[m], gv[m], r,              \
+                                        (SRC) && S::direct ? tb.smat + (m) : nullptr)
             constexpr bool fg_first = S::n_fs + S::n_fg > 0;
 #pragma unroll
             for (int i = 0; i < S::n_fs; ++i) {
@@ -134,6 +153,28 @@ __global__ void __launch_bounds__(kTraceThreads, MINB) trace_static_kernel(Progr
     extern __shared__ float4 smem4[];
     const TraceBlock tb = trace_prologue(prog, a, smem4);
     if (!tb.valid) return;
+    if constexpr (S::direct) {
+        // source tables lose M Gamma (rule offset); B per source (TraceSig "direct frames")
+        const int nq = a.nq_pad;
+        float *stab = const_cast<float *>(tb.stab);
+        float *gtab = stab + (size_t)(2 * (1 + S::n_lens)) * nq;
+        if (S::n_shear) {
+            for (int i = threadIdx.x; i < S::n_src * nq; i += kTraceThreads) {
+                const int m = i / nq, k = i - m * nq;
+                const float4 M = tb.sder[(prog.light_off[m] >> 2) + 1];
+                const float su = stab[2 * nq + k], sv = stab[3 * nq + k];     // shear = lens 0
+                gtab[(size_t)(2 * m) * nq + k] -= fmaf(M.x, su, M.y * sv);
+                gtab[(size_t)(2 * m + 1) * nq + k] -= fmaf(M.z, su, M.w * sv);
+            }
+        }
+        if (threadIdx.x < S::n_src) {
+            const float4 M = tb.sder[(prog.light_off[threadIdx.x] >> 2) + 1];
+            const float4 c2 = tb.sder[(prog.lens_off[S::n_shear] >> 2) + 2];  // (cs A, sn A, cs A l, -sn A l)
+            tb.smat[threadIdx.x] = make_float4(fmaf(M.x, c2.x, M.y * c2.y), fmaf(M.x, c2.w, M.y * c2.z),
+                                               fmaf(M.z, c2.x, M.w * c2.y), fmaf(M.z, c2.w, M.w * c2.z));
+        }
+        __syncthreads();
+    }
     float *Lb = a.L + (size_t)blockIdx.y * a.l_stride;
     if constexpr (S::n_sie == 0) {
         trace_pixels<NP, S, 0>(prog, a, tb, Lb);
