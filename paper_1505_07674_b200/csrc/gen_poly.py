@@ -52,6 +52,8 @@ def horner32(m, x):
 
 
 TABLES = (  # name, function, T, degree, centred, scale
+    ("kAtan019", f_atan, 0.16 / 0.84, 4, False, 1.0),
+    ("kAtan056", f_atan, 0.36 / 0.64, 6, False, 1.0),
     ("kAtan1", f_atan, 1.0, 8, False, 1.0),
     ("kAtan2", f_atan, 2.0, 10, True, 1.0),
     ("kAtan3", f_atan, 3.0, 12, True, 1.0),

@@ -54,11 +54,13 @@ __device__ __forceinline__ void load_pairs(const float *row, f2 (&out)[NP])
 // atan(z)/z and (2/ln 2) atanh(z)/z in t = z^2 on [0, T]; highest degree first.  The tables
 // marked "in s" are monomials in s = (2/T) t - 1: FP32 Horner in t itself loses up to 1e-5
 // to cancellation for T >~ 1.  Relative error, fit / FP32 Horner:
-//   kAtan1    T = 1     deg  8 in t   1.5e-8 / 0.9e-7      kAtanh016  T = 0.16  deg  4 in t   2.8e-8 / 1.2e-7
-//   kAtan2    T = 2     deg 10 in s   5.5e-8 / 1.4e-7      kAtanh036  T = 0.36  deg  6 in t   2.6e-8 / 1.2e-7
-//   kAtan3    T = 3     deg 12 in s   6.1e-8 / 1.4e-7      kAtanh050  T = 0.50  deg  8 in t   1.3e-8 / 0.9e-7
-//                                                          kAtanh067  T = 2/3   deg 10 in s   4.0e-8 / 1.5e-7
-//                                                          kAtanh075  T = 0.75  deg 12 in s   4.1e-8 / 1.5e-7
+//   kAtan019  T = 4/21  deg  4 in t   2.9e-8 / 1.0e-7      kAtanh016  T = 0.16  deg  4 in t   2.8e-8 / 1.2e-7
+//   kAtan056  T = 9/16  deg  6 in t   3.0e-8 / 1.1e-7      kAtanh036  T = 0.36  deg  6 in t   2.6e-8 / 1.2e-7
+//   kAtan1    T = 1     deg  8 in t   1.5e-8 / 0.9e-7      kAtanh050  T = 0.50  deg  8 in t   1.3e-8 / 0.9e-7
+//   kAtan2    T = 2     deg 10 in s   5.5e-8 / 1.4e-7      kAtanh067  T = 2/3   deg 10 in s   4.0e-8 / 1.5e-7
+//   kAtan3    T = 3     deg 12 in s   6.1e-8 / 1.4e-7      kAtanh075  T = 0.75  deg 12 in s   4.1e-8 / 1.5e-7
+__device__ constexpr float kAtan019[5] = {7.7191768884e-02f, -1.3767447193e-01f, 1.9966269114e-01f, -3.3332551885e-01f, 9.9999997081e-01f};
+__device__ constexpr float kAtan056[7] = {1.8452358884e-02f, -5.8612542189e-02f, 1.0069710760e-01f, -1.4100846142e-01f, 1.9983821868e-01f, -3.3332792361e-01f, 9.9999997016e-01f};
 __device__ constexpr float kAtan1[9] = {2.8498055468e-03f, -1.6068293304e-02f, 4.2690975050e-02f, -7.5042486123e-02f, 1.0640912567e-01f, -1.4203639026e-01f, 1.9992618715e-01f, -3.3333073313e-01f, 9.9999998476e-01f};
 __device__ constexpr float kAtan2[11] = {9.1487060309e-05f, -1.8564391925e-04f, 1.5699309251e-04f, -3.9463378275e-04f, 1.1686782180e-03f, -2.7031232426e-03f, 6.4149697350e-03f, -1.6261596296e-02f, 4.4525141523e-02f, -1.4269952760e-01f, 7.8539815093e-01f};
 __device__ constexpr float kAtan3[13] = {3.0422385513e-04f, -4.8443279783e-04f, -1.2014446101e-04f, 2.3235041340e-05f, 1.2300481067e-03f, -2.0805755083e-03f, 3.1809357122e-03f, -6.3178359761e-03f, 1.2922699920e-02f, -2.7101507477e-02f, 6.1303160862e-02f, -1.6173893999e-01f, 7.2347895789e-01f};
@@ -88,8 +90,8 @@ __device__ __forceinline__ f2 odd_poly2(f2 z, const float (&c)[N], float two_ove
 // prep.cu stores the mode of a vector (the most general one any of its SIEs needs) in the
 // header of its derived block; it is block-uniform in the tracer.
 //   mode   q^2 >=   atan               atanh
-//   0      0.84     kAtan1             kAtanh016
-//   1      0.64     kAtan1             kAtanh036
+//   0      0.84     kAtan019           kAtanh016
+//   1      0.64     kAtan056           kAtanh036
 //   2      0.50     kAtan1             kAtanh050
 //   3      1/3      kAtan2             kAtanh067  (or log, kAtanhLogFrom)
 //   4      0.25     kAtan3             kAtanh075  (or log)
@@ -105,7 +107,9 @@ constexpr int kAtanhLogFrom = 5;           // modes >= this take the log form of
 template <int MODE>
 __device__ __forceinline__ f2 sie_atan2x(f2 z)
 {
-    if constexpr (MODE <= 2) return odd_poly2<9, false>(z, kAtan1, 0.0f);
+    if constexpr (MODE == 0) return odd_poly2<5, false>(z, kAtan019, 0.0f);
+    else if constexpr (MODE == 1) return odd_poly2<7, false>(z, kAtan056, 0.0f);
+    else if constexpr (MODE == 2) return odd_poly2<9, false>(z, kAtan1, 0.0f);
     else if constexpr (MODE == 3) return odd_poly2<11, true>(z, kAtan2, 1.0f);
     else if constexpr (MODE == 4) return odd_poly2<13, true>(z, kAtan3, 2.0f / 3.0f);
     else {
