@@ -319,3 +319,31 @@ def test_quadrature_error_map_of_the_gauss_kronrod_rule(L):
         assert ref.max() > 10 * bound.max()              # the map is well above the bound somewhere
         assert np.all(np.abs(err[b] - ref) <= bound), "error map off by %.3g of the bound" % (
             np.abs(err[b] - ref) / bound).max()
+
+
+def test_constant_tap_pool_is_shared_by_live_handles_and_released_on_destroy(L):
+    """The PSF taps of the live handles share 60 KB of constant memory (include/lensed.h):
+    two 63x63 PSFs (32.5 KB each) do not fit together; destroying one makes room; the
+    surviving handle still computes the right thing."""
+    rng = np.random.default_rng(7)
+    psf = rng.uniform(0.1, 1.0, size=(63, 63))
+    small = synth.shrunk(synth.get_config(1), 20, 24, 2)
+    cfg = synth.Config(1, "pool", small.H, small.W, small.scale, small.models, small.quad, psf, None,
+                       small.truth, 2, small._draw, 0.005, 2000.0)
+    prob = Problem(cfg)
+    h1 = prob.create()
+    try:
+        with pytest.raises(L.LensedError) as e:
+            prob.create()
+        assert e.value.status == L.ENOMEM
+        logl1, _ = _gpu_eval(L, h1, cfg.batch(), cfg.H, cfg.W, render=False)
+    finally:
+        L.lensed_destroy(h1)
+    h2 = prob.create()                                    # room again
+    try:
+        logl2, _ = _gpu_eval(L, h2, cfg.batch(), cfg.H, cfg.W, render=False)
+    finally:
+        L.lensed_destroy(h2)
+    assert np.array_equal(logl1, logl2)
+    logl_o = prob.oracle_loglike(cfg.batch())[0]
+    assert logl_errors(logl1, logl_o).max() <= LOGL_RTOL
