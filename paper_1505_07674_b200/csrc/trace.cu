@@ -61,8 +61,11 @@ __device__ __forceinline__ void sie_by_mode(int mode, const float4 *d, const flo
 //   | sum_k w_k I(x_k) - sum_k w'_k I(x_k) |,   w' = embedded lower-order rule,
 // accumulated as sum_k (w_k - w'_k) I(x_k), into a.err[vector][H][W] (NaN for vectors outside
 // the model domain).  A diagnostic output, not on the likelihood path: interpreter only.
+#ifndef LENSED_MINB_GENERIC
+#define LENSED_MINB_GENERIC 3      // Euclid list 49.5 -> 44.0 ms per 4096 vectors against 2 (multi-lens list 46.2 -> 47.1)
+#endif
 template <int NP, bool ERR>
-__global__ void __launch_bounds__(kTraceThreads, 2) trace_kernel(Program prog, TraceArgs a)
+__global__ void __launch_bounds__(kTraceThreads, LENSED_MINB_GENERIC) trace_kernel(Program prog, TraceArgs a)
 {
     constexpr int R = 2 * NP;
     extern __shared__ float4 smem4[];
