@@ -183,30 +183,38 @@ int trace_pick_R(int n_quad)
     return best;
 }
 
+namespace {
+
+// every static signature; a NULL err only asks whether the signature matches
+typedef bool (*StaticTracer)(const int (&)[K_COUNT], const Program &, const TraceArgs &, int, int, cudaStream_t,
+                             cudaError_t *);
+const StaticTracer kStaticTracers[] = {trace_static_a, trace_static_b, trace_static_c, trace_static_d, trace_static_e};
+
+void count_kinds(const Program &prog, int (&counts)[K_COUNT])
+{
+    for (int k = 0; k < K_COUNT; ++k) counts[k] = 0;
+    for (int m = 0; m < prog.n_models; ++m) counts[prog.kind[m]] += 1;
+}
+
+}  // namespace
+
 bool trace_has_static(const Program &prog)
 {
-    int counts[K_COUNT] = {0};
-    for (int m = 0; m < prog.n_models; ++m) counts[prog.kind[m]] += 1;
-    // the same list as in launch_trace
-    const int sigs[][8] = {{0, 0, 1, 0, 0, 1, 0, 0}, {1, 1, 0, 0, 1, 0, 1, 0}, {1, 1, 0, 0, 2, 0, 1, 0}, {1, 2, 0, 1, 2, 1, 1, 0}, {0, 1, 0, 0, 1, 0, 1, 0}};
-    for (const auto &s : sigs)
-        if (counts[K_SHEAR] == s[0] && counts[K_SIE] == s[1] && counts[K_SIS] == s[2] && counts[K_POINT] == s[3] &&
-            counts[K_SRC_SERSIC] == s[4] && counts[K_SRC_GAUSS] == s[5] && counts[K_FG_SERSIC] == s[6] &&
-            counts[K_FG_GAUSS] == s[7])
-            return true;
+    int counts[K_COUNT];
+    count_kinds(prog, counts);
+    for (StaticTracer f : kStaticTracers)
+        if (f(counts, prog, TraceArgs{}, 0, 0, nullptr, nullptr)) return true;
     return false;
 }
 
 cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nvec, bool allow_static, cudaStream_t st)
 {
     if (allow_static && a.err == nullptr) {
-        int counts[K_COUNT] = {0};
-        for (int m = 0; m < prog.n_models; ++m) counts[prog.kind[m]] += 1;
+        int counts[K_COUNT];
+        count_kinds(prog, counts);
         cudaError_t err = cudaSuccess;
-        if (trace_static_a(counts, prog, a, R, nvec, st, &err) || trace_static_b(counts, prog, a, R, nvec, st, &err) ||
-            trace_static_c(counts, prog, a, R, nvec, st, &err) || trace_static_d(counts, prog, a, R, nvec, st, &err) ||
-            trace_static_e(counts, prog, a, R, nvec, st, &err))
-            return err;
+        for (StaticTracer f : kStaticTracers)
+            if (f(counts, prog, a, R, nvec, st, &err)) return err;
     }
     const bool err = a.err != nullptr;
     switch (R) {

@@ -205,15 +205,15 @@ cudaError_t launch_trace_static(const Program &prog, const TraceArgs &a, int R, 
 }
 
 // Defines  bool NAME(counts, prog, args, R, nvec, stream, &err): false if the signature does
-// not match the list's per-kind counts, else launches and sets err.  One per .cu file, so
-// that the signatures compile in parallel (build.py).
+// not match the list's per-kind counts, else launches and sets err (a NULL err only asks).
+// One per .cu file, so that the signatures compile in parallel (build.py).
 #define LENSED_DEFINE_STATIC_TRACER(NAME, MINB, ...)                                                         \
     bool NAME(const int (&counts)[K_COUNT], const Program &prog, const TraceArgs &a, int R, int nvec,   \
               cudaStream_t st, cudaError_t *err)                                                        \
     {                                                                                                   \
         using S = TraceSig<__VA_ARGS__>;                                                                \
         if (!S::matches(counts)) return false;                                                          \
-        *err = launch_trace_static<S, MINB>(prog, a, R, nvec, st);                                           \
+        if (err) *err = launch_trace_static<S, MINB>(prog, a, R, nvec, st);                             \
         return true;                                                                                    \
     }
 

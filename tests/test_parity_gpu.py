@@ -347,3 +347,44 @@ def test_constant_tap_pool_is_shared_by_live_handles_and_released_on_destroy(L):
     assert np.array_equal(logl1, logl2)
     logl_o = prob.oracle_loglike(cfg.batch())[0]
     assert logl_errors(logl1, logl_o).max() <= LOGL_RTOL
+
+
+def test_largest_rule_and_longest_model_list(L):
+    """LENSED_MAX_QUAD-class rule (15 x 15 = 225 points, the size of the paper's g7k15) and a list
+    of LENSED_MAX_MODELS = 32 objects (interpreting tracer, every kind present)."""
+    rng = np.random.default_rng(11)
+    models, truth = [], []
+    for i in range(6):
+        models.append("sis"); truth += [rng.uniform(-0.3, 0.3), rng.uniform(-0.3, 0.3), rng.uniform(0.02, 0.08)]
+    for i in range(3):
+        models.append("sie"); truth += [rng.uniform(-0.2, 0.2), rng.uniform(-0.2, 0.2), rng.uniform(0.05, 0.15),
+                                        rng.uniform(0.3, 1.0), rng.uniform(0, 180)]
+    for i in range(3):
+        models.append("point"); truth += [rng.uniform(-0.3, 0.3), rng.uniform(-0.3, 0.3), rng.uniform(0.01, 0.04)]
+    models += ["shear", "shear"]; truth += [0.03, -0.02, -0.01, 0.04]
+    for i in range(6):
+        models.append("src_gauss"); truth += [rng.uniform(-0.2, 0.2), rng.uniform(-0.2, 0.2), rng.uniform(0.03, 0.1),
+                                              synth.mag_of_flux(rng.uniform(5, 20)), rng.uniform(0.4, 1.0), rng.uniform(0, 180)]
+    for i in range(5):
+        models.append("src_sersic"); truth += [rng.uniform(-0.2, 0.2), rng.uniform(-0.2, 0.2), rng.uniform(0.05, 0.15),
+                                               synth.mag_of_flux(rng.uniform(5, 20)), rng.uniform(0.5, 4.0),
+                                               rng.uniform(0.4, 1.0), rng.uniform(0, 180)]
+    for i in range(3):
+        models.append("fg_sersic"); truth += [rng.uniform(-0.2, 0.2), rng.uniform(-0.2, 0.2), rng.uniform(0.2, 0.6),
+                                              synth.mag_of_flux(rng.uniform(50, 200)), rng.uniform(1.0, 4.0),
+                                              rng.uniform(0.5, 1.0), rng.uniform(0, 180)]
+    models += ["fg_gauss", "fg_gauss"]
+    for i in range(2):
+        truth += [rng.uniform(-0.2, 0.2), rng.uniform(-0.2, 0.2), rng.uniform(0.1, 0.3),
+                  synth.mag_of_flux(rng.uniform(20, 50)), rng.uniform(0.5, 1.0), rng.uniform(0, 180)]
+    models += ["sky", "sky"]; truth += [0.01, 0.005]
+    assert len(models) == 32
+    cfg = _mini(tuple(models), truth, H=20, W=22, psf=synth.gaussian_psf(5, 1.6), quad=synth.gauss_legendre_rule(15))
+    assert len(cfg.quad) == 225
+    prob = Problem(cfg)
+    h = prob.create()
+    try:
+        assert L.lensed_get_static_tracer(h) == 0
+    finally:
+        L.lensed_destroy(h)
+    _check(L, prob, np.vstack([cfg.truth.astype(np.float32)[None]] * 2))
