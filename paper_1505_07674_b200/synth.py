@@ -57,22 +57,49 @@ _GK = {  # Gauss-Kronrod (Patterson 1968) nodes / Kronrod weights / embedded Gau
 }
 
 
+def kronrod_extension(n_gauss):
+    """(nodes, Kronrod weights, embedded Gauss weights) of the (2 n + 1)-point Kronrod extension
+    of the n-point Gauss-Legendre rule on [-1, 1], nodes ascending; computed, not tabulated:
+    the n + 1 added nodes are the roots of the Stieltjes polynomial E (degree n + 1, orthogonal
+    to every polynomial of degree <= n with weight P_n), the weights are the interpolatory ones.
+    g3k7 / g5k11 / g7k15 of PAPER.md:341-343 are n_gauss = 3 / 5 / 7."""
+    leg = np.polynomial.legendre
+    n = n_gauss
+    xg, wg = leg.leggauss(n)
+    xq, wq = leg.leggauss(2 * n + 4)                              # exact for the integrals below
+    Pn = leg.legval(xq, [0] * n + [1])
+    basis = np.stack([leg.legval(xq, [0] * j + [1]) for j in range(n + 2)])     # P_0 .. P_{n+1}
+    # sum_j c_j int P_n P_j P_k = 0 for k = 0..n, c_{n+1} = 1
+    A = np.array([[np.sum(wq * Pn * basis[j] * basis[k]) for j in range(n + 1)] for k in range(n + 1)])
+    rhs = -np.array([np.sum(wq * Pn * basis[n + 1] * basis[k]) for k in range(n + 1)])
+    c = np.append(np.linalg.solve(A, rhs), 1.0)
+    xe = np.real(leg.legroots(c))
+    x = np.sort(np.concatenate([xg, xe]))
+    x = 0.5 * (x - x[::-1])                                        # symmetrise
+    V = np.stack([leg.legval(x, [0] * j + [1]) for j in range(2 * n + 1)])
+    w = np.linalg.solve(V, np.array([2.0] + [0.0] * (2 * n)))
+    w = 0.5 * (w + w[::-1])
+    g = np.zeros_like(w)
+    for xi, wi in zip(xg, wg):
+        g[np.argmin(np.abs(x - xi))] = wi
+    return x, w, g
+
+
 def gauss_kronrod_rule(n=7):
-    """Cartesian square of the n-point Kronrod rule (the paper's default g3k7 for n = 7)."""
-    xs, ws, _ = _GK[n]
-    x = np.array([-v for v in xs[:0:-1]] + xs)
-    w = np.array(ws[:0:-1] + ws)
+    """Cartesian square of the n-point Kronrod rule (n = 7 / 11 / 15: the paper's g3k7 default,
+    g5k11, g7k15) on the pixel [-1/2, 1/2]^2, weights summing to 1."""
+    x, w, _ = kronrod_extension((n - 1) // 2)
     x, w = 0.5 * x, 0.5 * w
     q = [(x[a], x[b], w[a] * w[b]) for b in range(n) for a in range(n)]
     return np.array(q, dtype=np.float64)
 
 
 def gauss_kronrod_embedded_weights(n=7):
-    """Weights of the embedded Gauss rule (3-point for n = 7) at the abscissae of
-    gauss_kronrod_rule(n), same order, summing to 1: the rule whose difference from the Kronrod
-    sum is the per-pixel error estimate of PAPER.md:166."""
-    _, _, gs = _GK[n]
-    g = 0.5 * np.array(gs[:0:-1] + gs)
+    """Weights of the embedded Gauss rule at the abscissae of gauss_kronrod_rule(n), same order,
+    summing to 1: the rule whose difference from the Kronrod sum is the per-pixel error
+    estimate of PAPER.md:166."""
+    _, _, g = kronrod_extension((n - 1) // 2)
+    g = 0.5 * g
     return np.array([g[a] * g[b] for b in range(n) for a in range(n)], dtype=np.float64)
 
 

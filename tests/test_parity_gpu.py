@@ -283,15 +283,18 @@ def test_create_rejects_bad_arguments_on_the_gpu_box_too(L):
 
 
 # --------------------------------------------------- quadrature error estimate
-def test_quadrature_error_map_of_the_gauss_kronrod_rule(L):
-    """lensed_render_error against the oracle's |K - G| on the paper-mock list with the default
-    g3k7 rule; the estimate is a small difference of two FP32 sums, so the bound is absolute:
-    1e-5 of the pixel's own luminosity (floored at 1e-3 of the image peak)."""
+@pytest.mark.parametrize("n_kronrod", [7, 11, 15])
+def test_quadrature_error_map_of_the_gauss_kronrod_rule(L, n_kronrod):
+    """lensed_render_error against the oracle's |K - G| with the paper's g3k7 (default), g5k11
+    and g7k15 rules; the estimate is a small difference of two FP32 sums, so the bound is
+    absolute: 3e-5 of the pixel's own luminosity (floored at 1e-3 of the image peak), the FP32
+    noise of a pixel that holds the centre of a cuspy source.  With g3k7
+    the map stands well above that floor; with the higher rules most of it lies below."""
     import torch
     from oracle import lensed_oracle as orc
     models = ("sie", "shear", "src_sersic", "fg_sersic", "sky")
     base = synth.shrunk(synth.get_config(1), 40, 44, 5)
-    quad, emb = synth.gauss_kronrod_rule(7), synth.gauss_kronrod_embedded_weights(7)
+    quad, emb = synth.gauss_kronrod_rule(n_kronrod), synth.gauss_kronrod_embedded_weights(n_kronrod)
     cfg = synth.Config(1, "gk", base.H, base.W, base.scale, models, quad, base.psf, None, base.truth, 5,
                        base._draw, 0.005, 2000.0)
     params = cfg.batch()
@@ -315,8 +318,9 @@ def test_quadrature_error_map_of_the_gauss_kronrod_rule(L):
     for b in range(4):
         ref = orc.error_map(cfg.H, cfg.W, cfg.scale, quad, emb, kinds, params[b], zp=cfg.zp)
         raw = orc.render_raw(cfg.H, cfg.W, cfg.scale, quad, kinds, params[b], zp=cfg.zp)
-        bound = 1e-5 * np.maximum(raw, 1e-3 * raw.max())
-        assert ref.max() > 10 * bound.max()              # the map is well above the bound somewhere
+        bound = 3e-5 * np.maximum(raw, 1e-3 * raw.max())
+        if n_kronrod == 7:
+            assert ref.max() > 10 * bound.max()          # the map is well above the bound somewhere
         assert np.all(np.abs(err[b] - ref) <= bound), "error map off by %.3g of the bound" % (
             np.abs(err[b] - ref) / bound).max()
 

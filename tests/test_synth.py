@@ -48,3 +48,23 @@ def test_rules():
     x = gk[:7, 0]
     w = gk[:7, 2] / gk[:7, 2].sum()
     assert abs(np.sum(w * x ** 10) - (0.5 ** 10) / 11) < 1e-15
+
+
+def test_kronrod_extensions_match_the_tabulated_rule_and_their_exactness_degrees():
+    """g3k7 / g5k11 / g7k15 are computed, not tabulated: the 7-point one must
+    reproduce Patterson's table (the literal in synth._GK), and a (2n+1)-point Kronrod rule is
+    exact for polynomials up to degree 3n+1, its embedded n-point Gauss rule up to 2n-1."""
+    xs, ws, gs = synth._GK[7]
+    x, w, g = synth.kronrod_extension(3)
+    assert np.allclose(x[3:], xs, atol=1e-14) and np.allclose(w[3:], ws, atol=1e-14) and np.allclose(g[3:], gs, atol=1e-14)
+    for n in (3, 5, 7):
+        x, w, g = synth.kronrod_extension(n)
+        assert len(x) == 2 * n + 1 and np.all(np.diff(x) > 0) and np.all(w > 0)
+        moment = lambda k: 2.0 / (k + 1) if k % 2 == 0 else 0.0
+        assert all(abs(np.sum(w * x ** k) - moment(k)) < 1e-13 for k in range(3 * n + 2))
+        assert abs(np.sum(w * x ** (3 * n + 3)) - moment(3 * n + 3)) > 1e-9          # and no further
+        assert all(abs(np.sum(g * x ** k) - moment(k)) < 1e-13 for k in range(2 * n))
+        assert np.count_nonzero(g) == n
+        q, e = synth.gauss_kronrod_rule(2 * n + 1), synth.gauss_kronrod_embedded_weights(2 * n + 1)
+        assert q.shape == ((2 * n + 1) ** 2, 3) and abs(q[:, 2].sum() - 1) < 1e-14 and abs(e.sum() - 1) < 1e-14
+        assert np.abs(q[:, :2]).max() < 0.5
