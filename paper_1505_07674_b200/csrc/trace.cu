@@ -40,6 +40,9 @@ LENSED_DECLARE_STATIC_TRACER(trace_static_b)
 LENSED_DECLARE_STATIC_TRACER(trace_static_c)
 LENSED_DECLARE_STATIC_TRACER(trace_static_d)
 LENSED_DECLARE_STATIC_TRACER(trace_static_e)
+LENSED_DECLARE_STATIC_TRACER(trace_static_f)
+LENSED_DECLARE_STATIC_TRACER(trace_static_g)
+LENSED_DECLARE_STATIC_TRACER(trace_static_h)
 
 namespace {
 
@@ -188,7 +191,8 @@ namespace {
 // every static signature; a NULL err only asks whether the signature matches
 typedef bool (*StaticTracer)(const int (&)[K_COUNT], const Program &, const TraceArgs &, int, int, cudaStream_t,
                              cudaError_t *);
-const StaticTracer kStaticTracers[] = {trace_static_a, trace_static_b, trace_static_c, trace_static_d, trace_static_e};
+const StaticTracer kStaticTracers[] = {trace_static_a, trace_static_b, trace_static_c, trace_static_d,
+                                       trace_static_e, trace_static_f, trace_static_g, trace_static_h};
 
 void count_kinds(const Program &prog, int (&counts)[K_COUNT])
 {

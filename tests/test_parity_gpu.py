@@ -413,3 +413,31 @@ def test_error_envelope_over_192_draws_of_the_prior(L, index, H, W):
     el, ep = logl_errors(logl_g, logl_o), pixel_errors(model_g, model_o)
     assert np.median(el) <= 0.1 * LOGL_RTOL and np.percentile(el, 99) <= LOGL_RTOL and el.max() <= 5 * LOGL_RTOL
     assert np.percentile(ep, 99) <= PIXEL_RTOL and ep.max() <= 5 * PIXEL_RTOL
+
+
+@pytest.mark.parametrize("static", [True, False])
+@pytest.mark.parametrize("models", [("sie", "src_sersic"), ("sie", "shear", "src_sersic", "sky"),
+                                    ("sis", "src_sersic", "sky", "sky")])
+def test_static_signatures_outside_the_configs(L, models, static):
+    """trace_sig_[f-h].cu: common lists that are not BASELINE.json configs; sky components do not
+    enter the signature.  Both tracers against the oracle, SIE axis ratios across the modes."""
+    rng = np.random.default_rng(5)
+    rows = []
+    for q in (0.97, 0.85, 0.72, 0.6, 0.52, 0.3):
+        p = []
+        for m in models:
+            if m == "sie":
+                p += [0.02, -0.03, 0.45, q, rng.uniform(0, 180)]
+            elif m == "sis":
+                p += [0.02, -0.03, 0.45]
+            elif m == "shear":
+                p += [0.04, -0.03]
+            elif m == "src_sersic":
+                p += [rng.uniform(-0.1, 0.1), rng.uniform(-0.1, 0.1), 0.1, synth.mag_of_flux(20.0), rng.uniform(0.7, 3.0),
+                      0.7, rng.uniform(0, 180)]
+            else:
+                p += [0.01]
+        rows.append(p)
+    params = np.array(rows, dtype=np.float32)
+    cfg = _mini(models, rows[2], H=40, W=36, psf=synth.gaussian_psf(5, 1.7), quad=synth.subsample_rule(4))
+    _check(L, Problem(cfg), params, static=static)
