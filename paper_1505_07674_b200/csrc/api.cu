@@ -39,6 +39,7 @@ struct lensed_handle {
     int KH = 1, KW = 1, NC = 1;
     int tile_w = 0, tile_h = 0;
     int Hp = 0, Wp = 0;             // padded frame of the unconvolved images (conv.cu "Input")
+    int ox_ll = 0, oy_ll = 0;       // origin of the loglike tile grid (render tiles start at 0, 0)
     int n_sm = 1;
     int tap_off = -1, tap_pairs = 0; // this handle's range of the constant tap pool
 
@@ -160,16 +161,23 @@ void pixel_list(const std::vector<uint8_t> &sel, int H, int W, std::vector<uint3
             if (sel[(size_t)i * W + j]) out.push_back(((uint32_t)i << 16) | (uint32_t)j);
 }
 
-void tile_list(const std::vector<uint8_t> &cnt, int H, int W, int tw, int th, std::vector<uint32_t> &out)
+// Tiles of tw x th pixels with origin (ox, oy) that hold a selected pixel, packed
+// (tile row << 16) | tile column; *ny, *nx = extent of the grid in tiles.
+void tile_list(const std::vector<uint8_t> &cnt, int H, int W, int tw, int th, int ox, int oy,
+               std::vector<uint32_t> &out, int *ny, int *nx)
 {
     out.clear();
-    for (int ti = 0; ti * th < H; ++ti)
-        for (int tj = 0; tj * tw < W; ++tj) {
+    *ny = *nx = 0;
+    for (int ti = 0; oy + ti * th < H; ++ti)
+        for (int tj = 0; ox + tj * tw < W; ++tj) {
             bool any = false;
-            for (int i = ti * th; i < std::min(H, (ti + 1) * th) && !any; ++i)
-                for (int j = tj * tw; j < std::min(W, (tj + 1) * tw); ++j)
+            for (int i = oy + ti * th; i < std::min(H, oy + (ti + 1) * th) && !any; ++i)
+                for (int j = ox + tj * tw; j < std::min(W, ox + (tj + 1) * tw); ++j)
                     if (cnt[(size_t)i * W + j]) { any = true; break; }
-            if (any) out.push_back(((uint32_t)ti << 16) | (uint32_t)tj);
+            if (any) {
+                out.push_back(((uint32_t)ti << 16) | (uint32_t)tj);
+                *ny = std::max(*ny, ti + 1); *nx = std::max(*nx, tj + 1);
+            }
         }
 }
 
@@ -276,6 +284,7 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
             ca.D = prog.D;
             ca.H = h->H; ca.W = h->W; ca.Wp = h->Wp; ca.KH = h->KH; ca.KW = h->KW; ca.NC = h->NC;
             ca.n_tiles = n_tiles; ca.nb = nb; ca.tap_off = h->tap_off;
+            ca.ox = render ? 0 : h->ox_ll; ca.oy = render ? 0 : h->oy_ll;
             if ((s = timed_begin(h, PH_CONV, st)) != LENSED_OK) return s;
             CU(h, launch_conv(ca, render, h->n_sm, st));
             if ((s = timed_end(h, st)) != LENSED_OK) return s;
@@ -437,14 +446,28 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
 
     // pixel lists and tile lists
     conv_tile_shape(&h->tile_w, &h->tile_h);
-    conv_padded_shape(H, W, h->KH, h->NC, &h->Hp, &h->Wp);
     std::vector<uint32_t> pix_ll, pix_all, tiles_ll, tiles_all;
     // traced set: the PSF windows of the counted pixels, one more row each way because a
     // counted row's pair partner multiplies its first / last window row by a zero tap
     pixel_list(dilate(counted, H, W, (h->KH - 1) / 2 + 1, (h->KW - 1) / 2), H, W, pix_ll);
     pixel_list(all, H, W, pix_all);
-    tile_list(counted, H, W, h->tile_w, h->tile_h, tiles_ll);
-    tile_list(all, H, W, h->tile_w, h->tile_h, tiles_all);
+    // loglike tiles start at the corner of the counted pixels' bounding box (x rounded down to
+    // a 16-byte boundary for cp.async): a mask that is not tile-aligned costs fewer tiles
+    {
+        int x0 = W, y0 = H;
+        for (int i = 0; i < H; ++i)
+            for (int j = 0; j < W; ++j)
+                if (counted[(size_t)i * W + j]) { x0 = std::min(x0, j); y0 = std::min(y0, i); }
+        h->ox_ll = x0 < W ? x0 / 4 * 4 : 0;
+        h->oy_ll = y0 < H ? y0 : 0;
+        int ny_ll, nx_ll, ny_all, nx_all;
+        tile_list(counted, H, W, h->tile_w, h->tile_h, h->ox_ll, h->oy_ll, tiles_ll, &ny_ll, &nx_ll);
+        tile_list(all, H, W, h->tile_w, h->tile_h, 0, 0, tiles_all, &ny_all, &nx_all);
+        // padded frame: the image, and every tile of either grid with its PSF halo
+        const int rows = std::max(std::max(ny_all * h->tile_h, h->oy_ll + ny_ll * h->tile_h), H);
+        const int cols = std::max(std::max(nx_all * h->tile_w, h->ox_ll + nx_ll * h->tile_w), W);
+        conv_padded_shape(rows, cols, h->KH, h->NC, &h->Hp, &h->Wp);
+    }
     h->npix_ll = (int)pix_ll.size(); h->npix_all = (int)pix_all.size();
     h->ntiles_ll = (int)tiles_ll.size(); h->ntiles_all = (int)tiles_all.size();
 

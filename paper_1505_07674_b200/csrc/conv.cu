@@ -10,8 +10,10 @@
 // Input.  The tracer writes the unconvolved images into a PADDED buffer: pixel (i, j) sits at
 // (i + p, j + q) of a [Hp][Wp] frame and border pixels are replicated into the pad (L164), so
 // a tile with its PSF halo is a plain rectangle of that frame -- no clamping here.
-// Hp = 64 tiles_y + KH - 1, Wp = 128 tiles_x + 4 NC (NC = ceil(KW / 4)): tiles that overhang
-// the image read zeros / stale finite values whose outputs are dropped.
+// The frame spans the image and every tile in use (+ KH - 1 rows, + 4 NC columns, NC =
+// ceil(KW / 4)): tiles that overhang the image read zeros / stale finite values whose outputs
+// are dropped.  The loglike tile grid starts at the corner of the counted pixels' bounding
+// box (a.ox, a.oy), the render grid at (0, 0).
 //
 // Work.  One persistent block of 256 threads per SM.  A work item is (output tile of 64 x 128
 // pixels, parameter vector); items are ordered tile-major and split evenly over the blocks,
@@ -178,7 +180,7 @@ __global__ void __launch_bounds__(kThreads, 1) conv_kernel(ConvArgs a)
     auto issue = [&](int item, int s) {
         const int t = item / a.nb, b = item - t * a.nb;
         const uint32_t tile = a.tiles[t];
-        const int Y0 = (int)(tile >> 16) * kTH, X0 = (int)(tile & 0xffffu) * kTW;
+        const int Y0 = a.oy + (int)(tile >> 16) * kTH, X0 = a.ox + (int)(tile & 0xffffu) * kTW;
         const float *src = a.Lp + (size_t)b * a.lp_stride + (size_t)Y0 * a.Wp + X0;
         float *dst = s_stage + (size_t)s * IH * IW;
         for (int i = threadIdx.x; i < (IH - kSlackRows) * IW4; i += kThreads) {
@@ -200,7 +202,7 @@ __global__ void __launch_bounds__(kThreads, 1) conv_kernel(ConvArgs a)
         const int s = a.n_stages == 2 ? ((item - lo) & 1) : 0;
         const int t = item / a.nb, b = item - t * a.nb;
         const uint32_t tile = a.tiles[t];
-        const int Y0 = (int)(tile >> 16) * kTH, X0 = (int)(tile & 0xffffu) * kTW;
+        const int Y0 = a.oy + (int)(tile >> 16) * kTH, X0 = a.ox + (int)(tile & 0xffffu) * kTW;
         const bool more = item + 1 < hi;
         if (a.n_stages == 2 && more) issue(item + 1, s ^ 1);
 
@@ -332,10 +334,11 @@ __global__ void final_kernel(FinalArgs a)
 
 void conv_tile_shape(int *tile_w, int *tile_h) { *tile_w = kTW; *tile_h = kTH; }
 
-void conv_padded_shape(int H, int W, int KH, int NC, int *Hp, int *Wp)
+// rows x cols = the image rounded up to cover every tile of the grids in use (api.cu)
+void conv_padded_shape(int rows, int cols, int KH, int NC, int *Hp, int *Wp)
 {
-    *Hp = (H + kTH - 1) / kTH * kTH + KH - 1;
-    *Wp = (W + kTW - 1) / kTW * kTW + 4 * NC;
+    *Hp = rows + KH - 1;
+    *Wp = (cols + 3) / 4 * 4 + 4 * NC;
 }
 
 namespace {

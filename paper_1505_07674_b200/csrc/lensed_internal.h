@@ -107,6 +107,7 @@ struct ConvArgs {
     long long lp_stride;   // Hp*Wp
     int D;
     int H, W, Wp, KH, KW, NC, n_tiles;
+    int ox, oy;            // image coordinates of tile (0, 0); ox is a multiple of 4
     int nb;                // vectors in this launch
     int tap_off;           // first tap pair of this handle in c_taps: Q[j][c][k] at tap_off + (j NC + c) 4 + k,
                            // Q[j][c][k] = (G[j][4c+k], G[j-1][4c+k]), j = 0..KH, G = flipped normalised PSF
@@ -127,7 +128,7 @@ cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nve
 bool trace_has_static(const Program &prog);
 cudaError_t launch_conv(ConvArgs a, bool render, int n_blocks, cudaStream_t st);
 cudaError_t conv_upload_taps(const float *pairs, int n_pairs, int pool_offset);
-void conv_padded_shape(int H, int W, int KH, int NC, int *Hp, int *Wp);
+void conv_padded_shape(int rows, int cols, int KH, int NC, int *Hp, int *Wp);
 cudaError_t launch_final(const FinalArgs &a, cudaStream_t st);
 cudaError_t conv_setup();                 // one-time function attributes
 int trace_pick_R(int n_quad);             // rays per register block for an n_quad-point rule
