@@ -159,8 +159,12 @@ lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes);
 long long lensed_frame_bytes(const lensed_handle *h);
 
 /* Tracer selection.  The ray tracer exists as one kernel that interprets any model list
- * and as kernels specialised at compile time for the model lists of BASELINE.json's
- * configs (same arithmetic, straight-line code).  lensed_create picks the specialised
+ * and as kernels specialised at compile time for eight model lists (same arithmetic,
+ * straight-line code; a list matches by its per-kind counts, sky components aside:
+ * SIS + Gaussian source; SIE + shear + 1 or 2 Sersic sources + Sersic lens light; 2 SIE +
+ * point mass + shear + 2 Sersic + 1 Gaussian source + Sersic lens light; SIE + Sersic
+ * source with / without Sersic lens light; SIE + shear + Sersic source; SIS + Sersic
+ * source).  lensed_create picks the specialised
  * kernel when the list has one.  lensed_set_static_tracer(h, 0) forces the interpreting
  * kernel (tests compare the two); (h, 1) re-enables the specialised one and returns
  * LENSED_EUNSUPPORTED if the list has none.  lensed_get_static_tracer: 1 / 0 = which one
