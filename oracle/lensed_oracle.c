@@ -23,8 +23,14 @@
  * brute-force integration, total Sersic / Gaussian flux, Gaussian == Sersic
  * n=1/2, quadrature exactness and brute-force supersampling, one-hot PSF shift,
  * delta PSF identity, PSF auto-normalisation, logL closed forms, rotation /
- * mirror symmetry of the whole pipeline.  Parity unpinned: absolute pixel
- * values of any figure of the paper (it prints none).
+ * mirror symmetry of the whole pipeline; oracle_render_raw with a one-point
+ * rule against oracle_brightness and its summed flux against F for Sersic
+ * indices 0.5 .. 8 (both are built from the same two static functions
+ * light_constants / light_profile); oracle_source_position against the lens
+ * equation solved by inspection (SIS image positions), the additivity of
+ * deflections and grad(psi); oracle_estimate_weights against hand values and
+ * the unit mean of w (d - mu)^2 on seeded Poisson counts.  Parity unpinned:
+ * absolute pixel values of any figure of the paper (it prints none).
  *
  * Build: gcc -O2 -std=c99 -fopenmp -fPIC -shared lensed_oracle.c -o liblensed_oracle.so -lm
  */
@@ -223,36 +229,110 @@ double oracle_potential(int kind, const double *p, double x, double y)
 /* ------------------------------------------------------------------------ */
 /* Surface brightness of one source / foreground object at (x, y) arcsec, in
  * flux per pixel area (R6): integrating over the plane in pixel units gives
- * the total flux F = 10^(-0.4 (mag - zp)).                                   */
-double oracle_brightness(int kind, const double *p, double x, double y,
-                         double scale, double zp)
+ * the total flux F = 10^(-0.4 (mag - zp)).
+ *
+ * The arithmetic is split in two static functions that BOTH oracle_brightness
+ * (what the half-light, total-flux, profile-shape and ellipse-convention pins
+ * test) and oracle_render_raw (what every GPU parity test compares against)
+ * call, so that a pin on one is a pin on the other:
+ *   light_constants: what depends on the parameter vector only (b_n, I_0);
+ *   light_profile:   the profile at a point, given those constants.          */
+static void light_constants(int kind, const double *p, double scale, double zp,
+                            double *bn, double *I0)
 {
+    *bn = 0.0; *I0 = 0.0;
     switch (kind) {
     case ORACLE_SRC_SERSIC: case ORACLE_FG_SERSIC: { /* PAPER.md:244-252 eqs 22-23 */
-        double rs = p[2], mag = p[3], n = p[4], q = p[5], pa = p[6] * (ORACLE_PI / 180.0);
+        double rs = p[2], mag = p[3], n = p[4];
+        double F = pow(10.0, -0.4 * (mag - zp));     /* total magnitude, L252 */
+        *bn = oracle_sersic_bn(n);                    /* R5: half-light radius */
+        *I0 = F * exp(2.0 * n * log(*bn) - lgamma(2.0 * n))
+              / (2.0 * ORACLE_PI * n * rs * rs) * scale * scale;      /* R6   */
+        break;
+    }
+    case ORACLE_SRC_GAUSS: case ORACLE_FG_GAUSS: {                    /* R7     */
+        double sg = p[2], mag = p[3];
+        double F = pow(10.0, -0.4 * (mag - zp));
+        *I0 = F / (2.0 * ORACLE_PI * sg * sg) * scale * scale;
+        break;
+    }
+    default: break;
+    }
+}
+
+static double light_profile(int kind, const double *p, double bn, double I0,
+                            double x, double y)
+{
+    switch (kind) {
+    case ORACLE_SRC_SERSIC: case ORACLE_FG_SERSIC: { /* PAPER.md:244-250 eqs 22-23 */
+        double rs = p[2], n = p[4], q = p[5], pa = p[6] * (ORACLE_PI / 180.0);
         double c = cos(pa), s = sin(pa);
         double dx = x - p[0], dy = y - p[1];
         double u = c * dx + s * dy, v = -s * dx + c * dy;
         double R = sqrt(u * u * q + v * v / q);                      /* eq. 23 */
-        double bn = oracle_sersic_bn(n);                              /* R5     */
-        double F = pow(10.0, -0.4 * (mag - zp));
-        double I0 = F * exp(2.0 * n * log(bn) - lgamma(2.0 * n))
-                    / (2.0 * ORACLE_PI * n * rs * rs) * scale * scale; /* R6   */
         return I0 * exp(-bn * pow(R / rs, 1.0 / n));                  /* eq. 22 */
     }
     case ORACLE_SRC_GAUSS: case ORACLE_FG_GAUSS: {                    /* R7     */
-        double sg = p[2], mag = p[3], q = p[4], pa = p[5] * (ORACLE_PI / 180.0);
+        double sg = p[2], q = p[4], pa = p[5] * (ORACLE_PI / 180.0);
         double c = cos(pa), s = sin(pa);
         double dx = x - p[0], dy = y - p[1];
         double u = c * dx + s * dy, v = -s * dx + c * dy;
-        double R2 = u * u * q + v * v / q;
-        double F = pow(10.0, -0.4 * (mag - zp));
-        double I0 = F / (2.0 * ORACLE_PI * sg * sg) * scale * scale;
+        double R2 = u * u * q + v * v / q;                            /* eq. 23 squared */
         return I0 * exp(-R2 / (2.0 * sg * sg));
     }
     case ORACLE_FG_SKY: return p[0];
     default: return 0.0;
     }
+}
+
+double oracle_brightness(int kind, const double *p, double x, double y,
+                         double scale, double zp)
+{
+    double bn, I0;
+    light_constants(kind, p, scale, zp, &bn, &I0);
+    return light_profile(kind, p, bn, I0, x, y);
+}
+
+/* Source-plane position of the image-plane point (x, y), arcsec:
+ *   y(x) = x - sum over the lenses of the list of alpha(x)    PAPER.md:53-57 eq. 1;
+ * deflections of several lens objects add.  Non-lens entries
+ * of the model list are skipped.  This is also the map of the image-plane
+ * priors ("sampling a position on the image plane,
+ * mapping it to the source plane, and assigning it to the source").
+ * offs[m] = offset of model m's parameters in params.                        */
+static void source_position(const int *kinds, int n_models, const int *offs,
+                            const double *params, double x, double y,
+                            double *sx, double *sy)
+{
+    double ax = 0.0, ay = 0.0;
+    for (int m = 0; m < n_models; ++m) if (is_lens(kinds[m])) {
+        double dax, day;
+        oracle_deflection(kinds[m], params + offs[m], x, y, &dax, &day);
+        ax += dax; ay += day;
+    }
+    *sx = x - ax; *sy = y - ay;
+}
+
+/* The same for K points of ONE parameter vector: xy[K][2] -> out[K][2].
+ * Returns 0 (out = NaN) if a LENS of the vector is outside the domain; the
+ * lights of the list do not enter.                                           */
+int oracle_source_position(const int *kinds, int n_models, const double *params,
+                           const double *xy, int K, double *out)
+{
+    int *offs = (int *)calloc((size_t)n_models, sizeof(int));
+    int off = 0, valid = 1;
+    for (int m = 0; m < n_models; ++m) {
+        offs[m] = off;
+        if (is_lens(kinds[m]) && !params_valid(kinds[m], params + off)) valid = 0;
+        off += oracle_kind_num_params(kinds[m]);
+    }
+    for (int k = 0; k < K; ++k) {
+        if (valid) source_position(kinds, n_models, offs, params, xy[2 * k], xy[2 * k + 1],
+                                   out + 2 * k, out + 2 * k + 1);
+        else out[2 * k] = out[2 * k + 1] = NAN;
+    }
+    free(offs);
+    return valid;
 }
 
 /* ------------------------------------------------------------------------ */
@@ -267,9 +347,8 @@ int oracle_render_raw(int H, int W, double scale, const double *quad, int n_quad
                       const double *params, double *L)
 {
     int valid = 1, off = 0;
-    /* Sersic b_n and I_0 depend on the vector only: oracle_brightness recomputes
-     * them per call, which is too slow for whole images, so the per-object
-     * constants are evaluated once here by the same expressions.             */
+    /* b_n and I_0 depend on the vector only: light_constants once per object,
+     * light_profile per ray -- the two functions oracle_brightness is made of. */
     double *bn = (double *)calloc((size_t)n_models, sizeof(double));
     double *I0 = (double *)calloc((size_t)n_models, sizeof(double));
     int *offs = (int *)calloc((size_t)n_models, sizeof(int));
@@ -278,14 +357,7 @@ int oracle_render_raw(int H, int W, double scale, const double *quad, int n_quad
         offs[m] = off;
         off += oracle_kind_num_params(kinds[m]);
         if (!params_valid(kinds[m], p)) { valid = 0; continue; }
-        if (kinds[m] == ORACLE_SRC_SERSIC || kinds[m] == ORACLE_FG_SERSIC) {
-            double n = p[4], rs = p[2];
-            bn[m] = oracle_sersic_bn(n);
-            I0[m] = pow(10.0, -0.4 * (p[3] - zp)) * exp(2.0 * n * log(bn[m]) - lgamma(2.0 * n))
-                    / (2.0 * ORACLE_PI * n * rs * rs) * scale * scale;
-        } else if (kinds[m] == ORACLE_SRC_GAUSS || kinds[m] == ORACLE_FG_GAUSS) {
-            I0[m] = pow(10.0, -0.4 * (p[3] - zp)) / (2.0 * ORACLE_PI * p[2] * p[2]) * scale * scale;
-        }
+        if (!is_lens(kinds[m])) light_constants(kinds[m], p, scale, zp, &bn[m], &I0[m]);
     }
     if (!valid) {
         for (long i = 0; i < (long)H * W; ++i) L[i] = NAN;
@@ -302,31 +374,14 @@ int oracle_render_raw(int H, int W, double scale, const double *quad, int n_quad
             double Li = 0.0;
             for (int k = 0; k < n_quad; ++k) {
                 double x = xc + quad[3 * k] * scale, y = yc + quad[3 * k + 1] * scale;
-                double ax = 0.0, ay = 0.0;                   /* eq. 1, lens sum */
-                for (int m = 0; m < n_models; ++m) if (is_lens(kinds[m])) {
-                    double dax, day;
-                    oracle_deflection(kinds[m], params + offs[m], x, y, &dax, &day);
-                    ax += dax; ay += day;
-                }
-                double sx = x - ax, sy = y - ay;             /* y(x) = x - alpha */
+                double sx, sy;                               /* eq. 1: y(x) = x - sum alpha */
+                source_position(kinds, n_models, offs, params, x, y, &sx, &sy);
                 double I = 0.0;                              /* eq. 2           */
                 for (int m = 0; m < n_models; ++m) {
                     int kd = kinds[m];
                     if (is_lens(kd)) continue;
-                    const double *p = params + offs[m];
-                    double px = is_source(kd) ? sx : x, py = is_source(kd) ? sy : y;
-                    if (kd == ORACLE_FG_SKY) { I += p[0]; continue; }
-                    int sersic = (kd == ORACLE_SRC_SERSIC || kd == ORACLE_FG_SERSIC);
-                    double q = sersic ? p[5] : p[4];
-                    double pa = (sersic ? p[6] : p[5]) * (ORACLE_PI / 180.0);
-                    double c = cos(pa), s = sin(pa);
-                    double dx = px - p[0], dy = py - p[1];
-                    double u = c * dx + s * dy, v = -s * dx + c * dy;
-                    double R2 = u * u * q + v * v / q;        /* eq. 23 squared  */
-                    if (sersic)
-                        I += I0[m] * exp(-bn[m] * pow(sqrt(R2) / p[2], 1.0 / p[4]));
-                    else
-                        I += I0[m] * exp(-R2 / (2.0 * p[2] * p[2]));
+                    if (is_source(kd)) I += light_profile(kd, params + offs[m], bn[m], I0[m], sx, sy);
+                    else               I += light_profile(kd, params + offs[m], bn[m], I0[m], x, y);
                 }
                 Li += (quad[3 * k + 2] / wsum) * I;          /* eq. 14          */
             }
@@ -434,6 +489,37 @@ int oracle_loglike(int H, int W, double scale, const double *image, const double
     }
     free(raw); free(cv);
     return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* Variance estimation from the data, section 3.3:
+ *   k_i = g_i (d_i + b_i)                      photon counts          eq. 18
+ *   Var(k_i) = k_i                             Poisson                eq. 20
+ *   s_i^2 = g_i^-2 Var(k_i) = (d_i + b_i)/g_i                         eq. 21
+ *   w_i = x_i / s_i^2                          weights of eq. 17 times the
+ *                                              "multiplicative extra weight factor" (L212)
+ * gain / offset / extra: maps [n], or NULL for the scalar gain0 / offset0 / 1.
+ * R15: a pixel whose counts k_i are not positive has no Poisson variance and
+ * gets w_i = 0 (masked).  variance (optional) receives s_i^2 (NaN where R15).
+ * Returns the number of pixels R15 masked, or -1 for an input outside the
+ * domain (g_i <= 0, x_i < 0, non-finite).                                    */
+long oracle_estimate_weights(long n, const double *image, const double *gain, double gain0,
+                             const double *offset, double offset0, const double *extra,
+                             double *weight, double *variance)
+{
+    long masked = 0;
+    for (long i = 0; i < n; ++i) {
+        double g = gain ? gain[i] : gain0, b = offset ? offset[i] : offset0;
+        double x = extra ? extra[i] : 1.0;
+        if (!isfinite(image[i]) || !isfinite(g) || !isfinite(b) || !isfinite(x)) return -1;
+        if (!(g > 0.0) || x < 0.0) return -1;
+        double k = g * (image[i] + b);                        /* eq. 18 */
+        double var_k = k;                                     /* eq. 20 */
+        double s2 = var_k / (g * g);                          /* eq. 21 */
+        if (k > 0.0) { weight[i] = x / s2; if (variance) variance[i] = s2; }
+        else { weight[i] = 0.0; if (variance) variance[i] = NAN; ++masked; }
+    }
+    return masked;
 }
 
 int oracle_threads(void)

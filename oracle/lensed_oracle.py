@@ -21,11 +21,20 @@ LENS_SIS, LENS_SIE, LENS_POINT, LENS_SHEAR = 0, 1, 2, 3
 SRC_SERSIC, SRC_GAUSS, FG_SERSIC, FG_GAUSS, FG_SKY = 4, 5, 6, 7, 8
 
 
+_SAN = os.environ.get("LENSED_ORACLE_SANITIZE") == "1"
+if _SAN:
+    _LIB = os.path.join(_HERE, "liblensed_oracle_san.so")
+
+
 def build(force=False):
-    """gcc -O2 (no fast-math) build of the oracle, the command its header states."""
+    """gcc -O2 (no fast-math) build of the oracle, the command its header states.  With
+    LENSED_ORACLE_SANITIZE=1 in the environment: an -fsanitize=address,undefined build beside it
+    (tests/test_oracle_sanitized.py runs the pins on it; the process must preload libasan)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+                 "-fno-omit-frame-pointer"] if _SAN else ["-O2"]
         subprocess.check_call(
-            ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", _SRC, "-o", _LIB, "-lm"])
+            ["gcc"] + flags + ["-std=c99", "-fopenmp", "-fPIC", "-shared", _SRC, "-o", _LIB, "-lm"])
     return _LIB
 
 
@@ -61,6 +70,10 @@ def lib():
         L.oracle_render.argtypes = [i, i, d, p, i, i, p, i, p, i, d, p, i, p, i]
         L.oracle_loglike.restype = i
         L.oracle_loglike.argtypes = [i, i, d, p, p, p, p, i, i, p, i, p, i, d, p, i, p, p, i]
+        L.oracle_source_position.restype = i
+        L.oracle_source_position.argtypes = [p, i, p, p, i, p]
+        L.oracle_estimate_weights.restype = ctypes.c_long
+        L.oracle_estimate_weights.argtypes = [ctypes.c_long, p, p, d, p, d, p, p, p]
         L.oracle_threads.restype = i
         L.oracle_threads.argtypes = []
         _lib = L
@@ -108,6 +121,31 @@ def potential(kind, p, x, y):
 def brightness(kind, p, x, y, scale=1.0, zp=0.0):
     p = _f64(p)
     return lib().oracle_brightness(int(kind), _ptr(p), float(x), float(y), float(scale), float(zp))
+
+
+def source_position(kinds, params, xy):
+    """y(x) = x - sum_lenses alpha(x) (eq. 1) for the K image-plane points xy[K][2] of ONE
+    parameter vector; NaN if a lens of the vector is outside the domain."""
+    k, params = _kinds(kinds), _f64(params)
+    xy = _f64(xy).reshape(-1, 2)
+    out = np.empty_like(xy)
+    lib().oracle_source_position(_ptr(k), len(k), _ptr(params), _ptr(xy), len(xy), _ptr(out))
+    return out
+
+
+def estimate_weights(image, gain, offset=0.0, extra=None, want_variance=False):
+    """w_i = x_i g_i / (d_i + b_i) (eqs. 18-21); gain / offset: scalars or maps."""
+    img = _f64(image)
+    g = None if np.isscalar(gain) else _f64(gain)
+    b = None if np.isscalar(offset) else _f64(offset)
+    x = None if extra is None else _f64(extra)
+    w = np.empty_like(img)
+    var = np.empty_like(img) if want_variance else None
+    rc = lib().oracle_estimate_weights(img.size, _ptr(img), _ptr(g), float(gain) if g is None else 0.0,
+                                       _ptr(b), float(offset) if b is None else 0.0, _ptr(x), _ptr(w), _ptr(var))
+    if rc < 0:
+        raise ValueError("oracle_estimate_weights: input outside the domain")
+    return (w, var) if want_variance else w
 
 
 def render_raw(H, W, scale, quad, kinds, params, zp=0.0):

@@ -1,4 +1,4 @@
-"""Writes the minimax polynomial tables of trace_math.cuh (run by hand; output pasted there).
+"""Writes the minimax polynomial tables of trace_math.cuh (output pasted there; tests/test_gen_poly.py regenerates and compares).
 
 atan(z)/z and atanh(z)/z as polynomials in t = z^2 on [0, T], fitted in relative error by
 Lawson's iteratively reweighted least squares on Chebyshev nodes (float64).  'centred'
@@ -64,14 +64,22 @@ TABLES = (  # name, function, T, degree, centred, scale
     ("kAtanh075", f_atanh, 0.75, 12, True, 2 / np.log(2)),
 )
 
-if __name__ == "__main__":
+def generate():
+    """[(name, T, degree, centred, coefficients highest degree first, fit error, FP32 Horner error)]"""
+    out = []
     for name, f, T, deg, centred, scale in TABLES:
         ms, e = lawson(f, T, deg)
         m = ms if centred else to_t(ms, T)
         t = np.linspace(0, T, 200001)
         x = 2 * t / T - 1 if centred else t
         e32 = np.max(np.abs(horner32(m, x).astype(np.float64) - f(t)) / f(t))
+        out.append((name, T, deg, centred, (m * scale)[::-1], e, e32))
+    return out
+
+
+if __name__ == "__main__":
+    for name, T, deg, centred, coef, e, e32 in generate():
         print("// %s: t in [0, %.4g], degree %d, %s; fit %.2e, FP32 Horner %.2e"
               % (name, T, deg, "in s = %.9g t - 1" % (2 / T) if centred else "in t", e, e32))
         print("__device__ constexpr float %s[%d] = {%s};"
-              % (name, deg + 1, ", ".join("%.10ef" % (v * scale) for v in m[::-1])))
+              % (name, deg + 1, ", ".join("%.10ef" % v for v in coef)))

@@ -612,3 +612,155 @@ def test_error_map_tracks_the_true_error_of_the_embedded_rule():
     true_err = np.abs(exact - g)
     assert true_err.max() > 1e-5 * exact.max()
     assert np.allclose(e, true_err, rtol=0.02, atol=1e-3 * true_err.max())
+
+
+# ------------------------------ render_raw's Sersic against oracle_brightness and the total flux
+@pytest.mark.parametrize("n", [0.5, 1.5, 2.5, 4.0, 8.0])
+def test_render_raw_sersic_is_the_pinned_brightness_pixel_by_pixel(n):
+    """PAPER.md:244-252 eqs. 22-23.  Every GPU parity test compares against oracle_render_raw;
+    the half-light / total-flux / profile-shape pins above go through oracle_brightness.  With a
+    one-point rule at the pixel centre the two must agree to rounding, as a source behind
+    zero-strength lenses (evaluated at y = x) and as a foreground, for q < 1 and PA != 0."""
+    H, W, s, zp = 14, 17, 0.05, 1.5
+    p = [0.031, -0.047, 0.12, -0.7, n, 0.55, 37.0]
+    fg = orc.render_raw(H, W, s, [[0, 0, 1]], [orc.FG_SERSIC], p, zp=zp)
+    src = orc.render_raw(H, W, s, [[0, 0, 1]], [orc.LENS_SIS, orc.LENS_SHEAR, orc.SRC_SERSIC],
+                         [0.1, 0.1, 0.0, 0.0, 0.0] + p, zp=zp)
+    for i in range(H):
+        for j in range(W):
+            x, y = (j - (W - 1) / 2) * s, (i - (H - 1) / 2) * s
+            ref = orc.brightness(orc.SRC_SERSIC, p, x, y, scale=s, zp=zp)
+            assert fg[i, j] == pytest.approx(ref, rel=1e-13)
+            assert src[i, j] == pytest.approx(ref, rel=1e-13)
+    # and the profile itself, retyped with the library's b_n: I/I_0 = exp(-b (R/r)^(1/n)), eq. 22
+    bn = special.gammaincinv(2 * n, 0.5)
+    I0 = 10 ** (-0.4 * (p[3] - zp)) * bn ** (2 * n) / (2 * math.pi * n * p[2] ** 2 * math.gamma(2 * n)) * s * s
+    t = math.radians(p[6])
+    i, j = 3, 12
+    dx, dy = (j - (W - 1) / 2) * s - p[0], (i - (H - 1) / 2) * s - p[1]
+    u, v = math.cos(t) * dx + math.sin(t) * dy, -math.sin(t) * dx + math.cos(t) * dy
+    R = math.sqrt(u * u * p[5] + v * v / p[5])
+    assert fg[i, j] == pytest.approx(I0 * math.exp(-bn * (R / p[2]) ** (1 / n)), rel=1e-11)
+
+
+def test_render_raw_sersic_sums_to_the_total_flux():
+    """I_0 is chosen so that the source has total magnitude mag_S.  Through
+    render_raw: sum_i L_i -> F for n = 1/2 (Gaussian tails, smooth: tight) and n = 4 (de
+    Vaucouleurs): there the flux outside radius R is F Q(8, b_4 (R/r)^(1/4)), so the sum over
+    the square image lies between the fluxes of its inscribed and circumscribed circles (the
+    central cusp is integrated with the 15 x 15 rule; it holds < 1e-3 of the flux error)."""
+    H = W = 96
+    s, mag = 0.05, -2.0
+    F = 10 ** (-0.4 * mag)
+    L = orc.render_raw(H, W, s, synth.gauss_legendre_rule(5), [orc.FG_SERSIC], [0.01, -0.02, 0.3, mag, 0.5, 0.6, 25.0])
+    assert L.sum() == pytest.approx(F, rel=1e-7)
+    rs = 0.1
+    L = orc.render_raw(H, W, s, synth.gauss_legendre_rule(15), [orc.FG_SERSIC], [0.0, 0.0, rs, mag, 4.0, 1.0, 0.0])
+    b4 = special.gammaincinv(8.0, 0.5)
+    half = 0.5 * H * s
+    inside = lambda R: F * special.gammainc(8.0, b4 * (R / rs) ** 0.25)
+    assert inside(half) * (1 - 1e-3) < L.sum() < inside(half * math.sqrt(2.0))
+    assert inside(half * math.sqrt(2.0)) - inside(half) < 4e-3 * F          # the bracket is tight
+    # a source behind a zero-strength lens: the same sum
+    Ls = orc.render_raw(H, W, s, synth.gauss_legendre_rule(15), [orc.LENS_SIE, orc.SRC_SERSIC],
+                        [0.2, 0.1, 0.0, 0.7, 30.0, 0.0, 0.0, rs, mag, 4.0, 1.0, 0.0])
+    assert Ls.sum() == pytest.approx(L.sum(), rel=1e-13)
+
+
+# -------------------------------------- source-plane positions (eq. 1; image-plane priors, L363)
+def test_source_position_solves_the_sis_lens_equation_by_inspection():
+    # a source at beta < theta_E on the x axis has images at beta + theta_E and beta - theta_E
+    b, beta = 0.9, 0.25
+    xy = [[beta + b, 0.0], [beta - b, 0.0]]
+    out = orc.source_position([orc.LENS_SIS], [0.0, 0.0, b], xy)
+    assert np.allclose(out, [[beta, 0.0], [beta, 0.0]], rtol=0, atol=1e-15)
+    # off-axis lens centre and a rotated axis: same thing along the direction t
+    c, t = np.array([0.3, -0.2]), np.array([math.cos(0.7), math.sin(0.7)])
+    out = orc.source_position([orc.LENS_SIS], [c[0], c[1], b], [c + (beta + b) * t, c + (beta - b) * t])
+    assert np.allclose(out, [c + beta * t, c + beta * t], rtol=0, atol=1e-15)
+
+
+def test_source_position_sums_the_lenses_of_the_list_and_skips_the_lights():
+    kinds = [orc.LENS_SIE, orc.SRC_SERSIC, orc.LENS_SHEAR, orc.FG_SKY, orc.LENS_POINT, orc.LENS_SIS]
+    sie, shear, pm, sis = [0.02, -0.03, 1.2, 0.7, 35.0], [0.03, -0.05], [0.8, 0.6, 0.1], [-0.4, 0.3, 0.3]
+    src = [0.1, 0.2, 0.15, 0.0, 2.0, 0.5, 10.0]
+    params = sie + src + shear + [0.01] + pm + sis
+    pts = RNG.uniform(-2.0, 2.0, size=(20, 2))
+    out = orc.source_position(kinds, params, pts)
+    lenses = ((orc.LENS_SIE, sie), (orc.LENS_SHEAR, shear), (orc.LENS_POINT, pm), (orc.LENS_SIS, sis))
+    for (x, y), (sx, sy) in zip(pts, out):
+        # y = x - grad(sum of the potentials), by finite differences of the pinned potentials
+        gx, gy = _grad(lambda a, b: sum(orc.potential(k, p, a, b) for k, p in lenses), x, y, h=1e-3)
+        assert sx == pytest.approx(x - gx, abs=2e-9) and sy == pytest.approx(y - gy, abs=2e-9)
+        ax = sum(orc.deflection(k, p, x, y)[0] for k, p in lenses)
+        ay = sum(orc.deflection(k, p, x, y)[1] for k, p in lenses)
+        assert sx == pytest.approx(x - ax, abs=1e-15) and sy == pytest.approx(y - ay, abs=1e-15)
+    # changing a light changes nothing; a lens outside its domain gives NaN
+    params2 = list(params); params2[7] = 99.0
+    assert np.array_equal(out, orc.source_position(kinds, params2, pts))
+    params3 = list(params); params3[3] = 1.5
+    assert np.all(np.isnan(orc.source_position(kinds, params3, pts)))
+    # no lens at all: y = x
+    assert np.array_equal(orc.source_position([orc.SRC_GAUSS], [0, 0, 0.1, 0, 1, 0], pts), pts)
+
+
+def test_render_raw_evaluates_sources_at_the_source_position():
+    # eq. 2 with the map above: one-point rule, I_S(y(x)) pixel by pixel
+    H, W, s = 9, 11, 0.05
+    kinds = [orc.LENS_SIE, orc.LENS_SHEAR, orc.SRC_GAUSS]
+    params = [0.02, -0.03, 0.2, 0.7, 35.0, 0.05, -0.02, 0.03, 0.01, 0.08, 0.0, 0.6, 20.0]
+    L = orc.render_raw(H, W, s, [[0.1, -0.2, 1]], kinds, params)
+    pts = [[(j - (W - 1) / 2 + 0.1) * s, (i - (H - 1) / 2 - 0.2) * s] for i in range(H) for j in range(W)]
+    src = orc.source_position(kinds, params, pts)
+    ref = [orc.brightness(orc.SRC_GAUSS, params[7:], sx, sy, scale=s) for sx, sy in src]
+    assert np.allclose(L.ravel(), ref, rtol=1e-13, atol=0)
+
+
+# --------------------------------------------- variance estimation (PAPER.md:190-212 eqs. 18-21)
+def test_estimate_weights_hand_values_maps_and_the_extra_factor():
+    d = np.array([3.0, 0.5, 10.0, -0.25])
+    w, var = orc.estimate_weights(d, 2.0, 0.25, want_variance=True)
+    # s^2 = (d + b)/g by hand: 3.25/2, 0.75/2, 10.25/2; d + b = 0: no Poisson variance (R15)
+    assert np.allclose(var[:3], [1.625, 0.375, 5.125], rtol=1e-15) and np.isnan(var[3])
+    assert np.allclose(w, [1 / 1.625, 1 / 0.375, 1 / 5.125, 0.0], rtol=1e-15)
+    g, b = np.array([2.0, 4.0, 1.0, 3.0]), np.array([0.25, 0.0, -2.0, 1.0])
+    w2 = orc.estimate_weights(d, g, b)
+    assert np.allclose(w2, [2 / 3.25, 4 / 0.5, 1 / 8.0, 3 / 0.75], rtol=1e-15)
+    x = np.array([1.0, 0.5, 0.0, 2.0])
+    assert np.allclose(orc.estimate_weights(d, g, b, x), w2 * x, rtol=1e-15)
+    assert np.array_equal(orc.estimate_weights(d, 2.0, 0.25), orc.estimate_weights(d, np.full(4, 2.0), np.full(4, 0.25)))
+    for bad in (dict(gain=0.0), dict(gain=-1.0), dict(gain=float("nan")), dict(offset=float("inf")),
+                dict(extra=np.array([1.0, -0.1, 1.0, 1.0]))):
+        args = dict(image=d, gain=1.0, offset=0.0, extra=None)
+        args.update(bad)
+        with pytest.raises(ValueError):
+            orc.estimate_weights(**args)
+
+
+def test_estimated_variance_is_the_variance_of_poisson_data():
+    """d = k/g - b with k ~ Poisson(mu): Var(d) = mu/g^2 (eq. 21 at k = mu), the sample variance
+    of d matches the mean estimated s^2, and w (d - E d)^2 averages to E[(k - mu)^2/k] ~ 1 + 1/mu."""
+    rng = np.random.default_rng(150507674)
+    mu, g, b = 400.0, 3.0, 20.0
+    k = rng.poisson(mu, size=200000)
+    d = k / g - b
+    w, var = orc.estimate_weights(d, g, b, want_variance=True)
+    assert var.mean() == pytest.approx(mu / g ** 2, rel=2e-3)
+    assert d.var() == pytest.approx(var.mean(), rel=1e-2)
+    assert np.mean(w * (d - (mu / g - b)) ** 2) == pytest.approx(1.0 + 1.0 / mu, abs=0.01)
+
+
+def test_library_weight_estimate_matches_the_oracle():
+    """lensed_estimate_weights is host code of the product library (no device needed): the same
+    seeded inputs through it and through the oracle."""
+    from paper_1505_07674_b200 import lensed
+    rng = np.random.default_rng(7)
+    d = rng.uniform(-1.0, 50.0, size=(31, 17)).astype(np.float32)
+    g = rng.uniform(0.5, 4.0, size=d.shape).astype(np.float32)
+    b = rng.uniform(0.0, 2.0, size=d.shape).astype(np.float32)
+    x = rng.uniform(0.0, 2.0, size=d.shape).astype(np.float32)
+    for args in ((d, 2.5, 0.75, None), (d, g, b, None), (d, g, 0.5, x)):
+        w_lib = lensed.lensed_estimate_weights(*args)
+        w_orc = orc.estimate_weights(*args)
+        assert np.array_equal(w_lib == 0, w_orc == 0)
+        assert np.allclose(w_lib, w_orc, rtol=1e-6, atol=0)
