@@ -110,6 +110,9 @@ int lensed_num_params(const lensed_handle *h);
  * -1 for NULL.                                                                           */
 int lensed_num_traced(const lensed_handle *h);
 
+/* H * W, the pixels of one model image (the stride of lensed_render's output); -1 for NULL. */
+int lensed_num_pixels(const lensed_handle *h);
+
 /*
  * lensed_render -- model images L* (PAPER.md:136 step iv; eqs. 14, 15), mask ignored.
  *   params_dev  [B][P] device f32
@@ -142,12 +145,29 @@ lensed_status lensed_loglike_host(lensed_handle *h, const float *params_host, in
  * lensed_set_profiling(h, 1) brackets every kernel the library launches with CUDA
  * events on the launching stream.  lensed_get_profile synchronises those events and
  * returns, since the last lensed_reset_profile: milliseconds and launch counts of the
- * parameter-prep, ray-trace, convolution(+chi-square) and final-reduction kernels as
- * ms[4] / launches[4] (host arrays, either may be NULL).  Launch counts are kept even
- * with profiling off (ms are then 0).                                                   */
+ * parameter-prep, ray-trace, FP64-refinement, convolution(+chi-square) and final-reduction
+ * kernels as ms[5] / launches[5] (host arrays, either may be NULL).  Launch counts are kept
+ * even with profiling off (ms are then 0).  lensed_reset_profile synchronises the device.  */
 lensed_status lensed_set_profiling(lensed_handle *h, int on);
 lensed_status lensed_get_profile(lensed_handle *h, double *ms, long long *launches);
 lensed_status lensed_reset_profile(lensed_handle *h);
+
+/*
+ * FP64 refinement of cusp pixels.  FP32 ray positions carry ~1e-6 pixel of rounding noise
+ * (y = x - alpha with |alpha| of tens of pixels, eq. 1); near the centre of a
+ * compact Sersic source of high index (the paper's prior reaches n = 8) the
+ * profile's logarithmic slope per pixel is large enough to turn that into more than 1e-5 in the
+ * pixel -- and, those being the brightest pixels, in logL.  The ray tracer therefore flags the
+ * pixels that have a ray where a source Sersic's slope  d ln I / dx  exceeds
+ *   G = gain * 200 / max(deflection scale in pixels, 25)      per pixel
+ * (deflection scale = sum of the lenses' Einstein radii + shear * image half-diagonal), and a
+ * second kernel re-traces those pixels -- all rule points, all components -- in double
+ * precision before the convolution.  Typically 1-20 pixels per vector.
+ * lensed_set_refine: gain = 1 is the default; larger = fewer pixels refined; gain <= 0 turns
+ * the refinement off (plain FP32 everywhere).  EINVAL for NaN.
+ * lensed_get_refined: pixels refined since the last lensed_reset_profile (synchronises).    */
+lensed_status lensed_set_refine(lensed_handle *h, double gain);
+lensed_status lensed_get_refined(lensed_handle *h, long long *pixels);
 
 /* Tuning knob: bytes of device scratch the unconvolved images L[b] of one batch chunk
  * may take (default 1 GiB: the buffer costs ~3.5 bytes of traffic per 3500 flops, so

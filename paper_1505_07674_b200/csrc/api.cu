@@ -22,7 +22,7 @@ namespace {
 
 thread_local std::string g_last_error;
 
-enum { PH_PREP = 0, PH_TRACE = 1, PH_CONV = 2, PH_FINAL = 3, PH_COUNT = 4 };
+enum { PH_PREP = 0, PH_TRACE = 1, PH_REFINE = 2, PH_CONV = 3, PH_FINAL = 4, PH_COUNT = 5 };
 
 struct EventPair { cudaEvent_t a, b; int phase; };
 
@@ -51,6 +51,12 @@ struct lensed_handle {
 
     // device scratch, grown on demand
     float *d_derived = nullptr; size_t cap_derived = 0;
+    double *d_derived64 = nullptr; size_t cap_derived64 = 0;
+    uint32_t *d_fixmask = nullptr; size_t cap_fixmask = 0;
+    uint2 *d_queue = nullptr; size_t cap_queue = 0;      // refine.cu: flagged pixels of one chunk
+    unsigned *d_queue_count = nullptr;
+    unsigned long long *d_refined = nullptr;   // pixels refined in FP64 since the last profile reset
+    double refine_gain = 1.0;                  // lensed_set_refine
     float *d_L = nullptr; size_t cap_L = 0;
     double *d_partial = nullptr; size_t cap_partial = 0;
     float *d_stage_in = nullptr; size_t cap_stage_in = 0;
@@ -62,8 +68,8 @@ struct lensed_handle {
     bool profiling = false;
     std::vector<EventPair> used;
     std::vector<EventPair> pool;
-    double ms[PH_COUNT] = {0, 0, 0, 0};
-    long long launches[PH_COUNT] = {0, 0, 0, 0};
+    double ms[PH_COUNT] = {0, 0, 0, 0, 0};
+    long long launches[PH_COUNT] = {0, 0, 0, 0, 0};
 
     std::string err;
 };
@@ -125,12 +131,15 @@ lensed_status upload(lensed_handle *h, T **dst, const T *src, size_t n)
     return LENSED_OK;
 }
 
+// Scratch grows to the high-water mark of the calls made so far, with stream-ordered
+// allocation on the caller's stream: no device-wide synchronisation inside an asynchronous
+// call (cudaFree / cudaMalloc would be one), and none at all once a batch size has been seen.
 template <class T>
-lensed_status grow(lensed_handle *h, T **buf, size_t *cap, size_t need)
+lensed_status grow(lensed_handle *h, T **buf, size_t *cap, size_t need, cudaStream_t st)
 {
     if (need <= *cap) return LENSED_OK;
-    if (*buf) { CU(h, cudaFree(*buf)); *buf = nullptr; *cap = 0; }   // cudaFree synchronises
-    CU(h, cudaMalloc((void **)buf, need * sizeof(T)));
+    if (*buf) { CU(h, cudaFreeAsync(*buf, st)); *buf = nullptr; *cap = 0; }
+    CU(h, cudaMallocAsync((void **)buf, need * sizeof(T), st));
     *cap = need;
     return LENSED_OK;
 }
@@ -214,6 +223,19 @@ lensed_status collect_profile(lensed_handle *h)
     return LENSED_OK;
 }
 
+// Pixels of the traced list one tracer block walks: it amortises its prologue (constants +
+// frame tables) over them.  Measured per config (ms per step at 512 / 1024 / 2048 / 4096 / 8192
+// pixels): HST 0.296 / 0.273 / 0.264 / 0.269 / 0.288, SLACS 4.55 / 4.34 / 4.23 / 4.15 / 4.13,
+// Euclid - / 34.6 / 34.0 / 33.6 / 33.5 per 4096 vectors.  At most 8192 (TraceArgs::fixmask).
+int pix_per_block(int npix)
+{
+#ifdef LENSED_PIX_PER_BLOCK             // tuning builds (build.py defines=...)
+    return LENSED_PIX_PER_BLOCK;
+#else
+    return npix >= (1 << 16) ? 8192 : npix >= (1 << 14) ? 4096 : npix >= (1 << 11) ? 2048 : 256;
+#endif
+}
+
 // The whole path for B vectors already on the device.
 lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_dev, bool render,
                   cudaStream_t st)
@@ -232,16 +254,24 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
     const int Bc = (int)std::min<long long>(std::min<long long>(per_chunk, 65535), B);
 
     lensed_status s;
-    if ((s = grow(h, &h->d_derived, &h->cap_derived, (size_t)B * prog.D)) != LENSED_OK) return s;
+    if ((s = grow(h, &h->d_derived, &h->cap_derived, (size_t)B * prog.D, st)) != LENSED_OK) return s;
+    if ((s = grow(h, &h->d_derived64, &h->cap_derived64, (size_t)B * prog.n_models * kD64PerModel, st)) != LENSED_OK) return s;
     if ((size_t)Bc * HWp > h->cap_L) {
         // pad cells no pixel clamps to (tile overhang) are read, never written: keep them zero
-        if ((s = grow(h, &h->d_L, &h->cap_L, (size_t)Bc * HWp)) != LENSED_OK) return s;
+        if ((s = grow(h, &h->d_L, &h->cap_L, (size_t)Bc * HWp, st)) != LENSED_OK) return s;
         CU(h, cudaMemsetAsync(h->d_L, 0, (size_t)Bc * HWp * sizeof(float), st));
     }
-    if (!render && (s = grow(h, &h->d_partial, &h->cap_partial, (size_t)B * std::max(n_tiles, 1))) != LENSED_OK)
+    if (!render && (s = grow(h, &h->d_partial, &h->cap_partial, (size_t)B * std::max(n_tiles, 1), st)) != LENSED_OK)
         return s;
+    const int ppb = pix_per_block(npix);
+    const int n_tblocks = npix > 0 ? (npix + ppb - 1) / ppb : 0;
+    const bool refine = h->refine_gain > 0.0 && n_tblocks > 0;
+    if (refine && (s = grow(h, &h->d_fixmask, &h->cap_fixmask, (size_t)Bc * n_tblocks * 256, st)) != LENSED_OK) return s;
+    const size_t queue_cap = (size_t)Bc * 64 + 4096;
+    if (refine && (s = grow(h, &h->d_queue, &h->cap_queue, queue_cap, st)) != LENSED_OK) return s;
 
-    PrepArgs pa{params_dev, h->d_derived, B, h->scale, h->zp, 0.5 * (h->W - 1), 0.5 * (h->H - 1)};
+    PrepArgs pa{params_dev, h->d_derived, h->d_derived64, B,
+                h->refine_gain > 0.0 ? h->refine_gain : (double)INFINITY, h->scale, h->zp, 0.5 * (h->W - 1), 0.5 * (h->H - 1)};
     if ((s = timed_begin(h, PH_PREP, st)) != LENSED_OK) return s;
     CU(h, launch_prep(prog, pa, st));
     if ((s = timed_end(h, st)) != LENSED_OK) return s;
@@ -253,23 +283,25 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
             ta.derived = h->d_derived + (size_t)b0 * prog.D;
             ta.pix = render ? h->d_pix_all : h->d_pix_ll;
             ta.quad = h->d_quad;
+            ta.fixmask = refine ? h->d_fixmask : nullptr;
             ta.L = h->d_L;
             ta.l_stride = (long long)HWp;
             ta.npix = npix; ta.nq_pad = h->nq_pad;
             ta.H = h->H; ta.W = h->W; ta.Wp = h->Wp; ta.px = (h->KW - 1) / 2; ta.py = (h->KH - 1) / 2;
-            // a block amortises its prologue (constants + frame tables) over this many pixels
-#ifdef LENSED_PIX_PER_BLOCK             // tuning builds (build.py defines=...)
-            ta.pix_per_block = LENSED_PIX_PER_BLOCK;
-#else
-            // measured per config (ms per step at 512 / 1024 / 2048 / 4096 / 8192 pixels): HST 0.296 /
-            // 0.273 / 0.264 / 0.269 / 0.288, SLACS 4.55 / 4.34 / 4.23 / 4.15 / 4.13, Euclid - / 34.6 /
-            // 34.0 / 33.6 / 33.5 per 4096 vectors
-            ta.pix_per_block = npix >= (1 << 16) ? 8192 : npix >= (1 << 14) ? 4096 : npix >= (1 << 11) ? 2048 : 256;
-#endif
+            ta.pix_per_block = ppb;
             ta.cxh = 0.5f * (h->W - 1); ta.cyh = 0.5f * (h->H - 1);
             if ((s = timed_begin(h, PH_TRACE, st)) != LENSED_OK) return s;
             CU(h, launch_trace(prog, ta, h->R, nb, h->static_tracer, st));
             if ((s = timed_end(h, st)) != LENSED_OK) return s;
+            if (refine) {
+                // FP64 re-trace of the pixels the tracer flagged (refine.cu), before the convolution
+                RefineArgs ra{ta, h->d_derived64 + (size_t)b0 * prog.n_models * kD64PerModel, ta.derived, h->d_refined,
+                              h->d_queue, h->d_queue_count, (int)queue_cap, nb, n_tblocks, h->n_quad};
+                if ((s = timed_begin(h, PH_REFINE, st)) != LENSED_OK) return s;
+                CU(h, launch_refine(prog, ra, h->n_sm, st));
+                h->launches[PH_REFINE] += 1;                       // two kernels: scan, queue
+                if ((s = timed_end(h, st)) != LENSED_OK) return s;
+            }
         }
         if (n_tiles > 0) {
             ConvArgs ca{};
@@ -309,8 +341,8 @@ lensed_status run_host(lensed_handle *h, const float *params_host, int B, float 
     const size_t n_in = (size_t)B * h->prog.P;
     const size_t n_out = render ? (size_t)B * h->H * h->W : (size_t)B;
     lensed_status s;
-    if ((s = grow(h, &h->d_stage_in, &h->cap_stage_in, n_in)) != LENSED_OK) return s;
-    if ((s = grow(h, &h->d_stage_out, &h->cap_stage_out, n_out)) != LENSED_OK) return s;
+    if ((s = grow(h, &h->d_stage_in, &h->cap_stage_in, n_in, st)) != LENSED_OK) return s;
+    if ((s = grow(h, &h->d_stage_out, &h->cap_stage_out, n_out, st)) != LENSED_OK) return s;
     CU(h, cudaMemcpyAsync(h->d_stage_in, params_host, n_in * sizeof(float), cudaMemcpyHostToDevice, st));
     if ((s = run(h, h->d_stage_in, B, h->d_stage_out, render, st)) != LENSED_OK) return s;
     CU(h, cudaMemcpyAsync(out_host, h->d_stage_out, n_out * sizeof(float), cudaMemcpyDeviceToHost, st));
@@ -509,6 +541,12 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
         if (e2 != cudaSuccess) { lensed_destroy(h); return fail(nullptr, LENSED_ECUDA, "tap upload: %s", cudaGetErrorString(e2)); }
     }
     CREATE_FAIL(upload(h, &h->d_quad, hq.data(), hq.size()));
+    {
+        const unsigned long long zero = 0;
+        CREATE_FAIL(upload(h, &h->d_refined, &zero, 1));
+        const unsigned zero32 = 0;
+        CREATE_FAIL(upload(h, &h->d_queue_count, &zero32, 1));
+    }
     h->h_quad = hq;
     CREATE_FAIL(upload(h, &h->d_pix_ll, pix_ll.data(), pix_ll.size()));
     CREATE_FAIL(upload(h, &h->d_pix_all, pix_all.data(), pix_all.size()));
@@ -521,6 +559,7 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
 
 int lensed_num_params(const lensed_handle *h) { return h ? h->prog.P : -1; }
 int lensed_num_traced(const lensed_handle *h) { return h ? h->npix_ll : -1; }
+int lensed_num_pixels(const lensed_handle *h) { return h ? h->H * h->W : -1; }
 
 lensed_status lensed_estimate_weights(long long n, const float *image, const float *gain, double gain0,
                                       const float *offset, double offset0, const float *extra, float *weight)
@@ -569,8 +608,10 @@ lensed_status lensed_render_error(lensed_handle *h, const float *params_dev, int
     CU(h, cudaSetDevice(h->device));
     const Program &prog = h->prog;
     lensed_status s;
-    if ((s = grow(h, &h->d_derived, &h->cap_derived, (size_t)B * prog.D)) != LENSED_OK) return s;
-    PrepArgs pa{params_dev, h->d_derived, B, h->scale, h->zp, 0.5 * (h->W - 1), 0.5 * (h->H - 1)};
+    if ((s = grow(h, &h->d_derived, &h->cap_derived, (size_t)B * prog.D, st)) != LENSED_OK) return s;
+    if ((s = grow(h, &h->d_derived64, &h->cap_derived64, (size_t)B * prog.n_models * kD64PerModel, st)) != LENSED_OK) return s;
+    PrepArgs pa{params_dev, h->d_derived, h->d_derived64, B, (double)INFINITY, h->scale, h->zp, 0.5 * (h->W - 1),
+                0.5 * (h->H - 1)};
     if ((s = timed_begin(h, PH_PREP, st)) != LENSED_OK) return s;
     CU(h, launch_prep(prog, pa, st));
     if ((s = timed_end(h, st)) != LENSED_OK) return s;
@@ -638,6 +679,29 @@ lensed_status lensed_reset_profile(lensed_handle *h)
     lensed_status s = collect_profile(h);
     if (s != LENSED_OK) return s;
     for (int i = 0; i < PH_COUNT; ++i) { h->ms[i] = 0.0; h->launches[i] = 0; }
+    CU(h, cudaSetDevice(h->device));
+    CU(h, cudaDeviceSynchronize());
+    CU(h, cudaMemset(h->d_refined, 0, sizeof(unsigned long long)));
+    return LENSED_OK;
+}
+
+lensed_status lensed_set_refine(lensed_handle *h, double gain)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (gain != gain) return fail(h, LENSED_EINVAL, "gain is NaN");
+    h->refine_gain = gain > 0.0 ? gain : 0.0;
+    return LENSED_OK;
+}
+
+lensed_status lensed_get_refined(lensed_handle *h, long long *pixels)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (!pixels) return fail(h, LENSED_EINVAL, "pixels is NULL");
+    CU(h, cudaSetDevice(h->device));
+    CU(h, cudaDeviceSynchronize());
+    unsigned long long n = 0;
+    CU(h, cudaMemcpy(&n, h->d_refined, sizeof n, cudaMemcpyDeviceToHost));
+    *pixels = (long long)n;
     return LENSED_OK;
 }
 
@@ -694,6 +758,8 @@ void lensed_destroy(lensed_handle *h)
     if (h->tap_off >= 0) g_tap_pool.give(h->device, h->tap_off);
     cudaFree(h->d_pix_ll); cudaFree(h->d_pix_all); cudaFree(h->d_tiles_ll); cudaFree(h->d_tiles_all);
     cudaFree(h->d_derived); cudaFree(h->d_L); cudaFree(h->d_partial);
+    cudaFree(h->d_derived64); cudaFree(h->d_fixmask); cudaFree(h->d_refined);
+    cudaFree(h->d_queue); cudaFree(h->d_queue_count);
     cudaFree(h->d_stage_in); cudaFree(h->d_stage_out);
     delete h;
 }

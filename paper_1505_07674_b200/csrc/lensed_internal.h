@@ -22,11 +22,19 @@ namespace lensed {
 //         A = b sqrt(q)/q' with q' floored at 1e-4, l = ln(2)/2 (trace.cu lens_sie)
 //  POINT  [c0][thetaE^2, 0, 0, 0]                                       8
 //  SHEAR  [g1, g2, 0, 0]                                                4
-//  SERSIC [c0][a1, a2, a3, a4][log2 I0, b_n*log2(e), 1/(2n), 0]         12
+//  SERSIC [c0][a1, a2, a3, a4][log2 I0, b_n*log2(e), 1/(2n), T2]        12
+//         T2 = squared scaled radius inside which a source's pixels are refined in FP64
+//         (prep.cu "refinement threshold"; 0 for foregrounds and n <= 1)
 //         (u', v') = (a1 dx + a2 dy, a3 dx + a4 dy) = rotated, q-stretched offset / r_S,
 //         so that u'^2 + v'^2 = (R / r_S)^2 with R of PAPER.md:250 eq. 23
 //  GAUSS  [c0][a1, a2, a3, a4][log2 I0, log2(e)/2, 0, 0]                12   (offset / sigma)
 //  SKY    [level, 0, 0, 0]                                              4
+//
+// derived64 [B][n_models][kD64PerModel] doubles, LIST order, lengths in pixels, centres in
+// pixel-index coordinates (column, row) -- the unrounded constants refine.cu re-traces with:
+//  SIS cx, cy, b | SIE cx, cy, cos, sin, q, b | POINT cx, cy, thetaE^2 | SHEAR g1, g2
+//  SERSIC cx, cy, cos, sin, q, r_S, 1/n, b_n, ln I0 | GAUSS cx, cy, cos, sin, q, sigma, ln I0 | SKY level
+//
 // Block 0 of every vector is the header [valid, SIE mode, 0, 0]; the mode (trace_math.cuh
 // "SIE") is the most general one any SIE of the vector needs, 0 without an SIE.
 enum Kind : int {
@@ -46,6 +54,7 @@ constexpr int kMaxModels = 32;
 constexpr int kMaxQuad = 256;
 constexpr int kMaxPsf = 63;
 constexpr int kHeaderFloats = 4;
+constexpr int kD64PerModel = 12;
 constexpr int kTapPoolPairs = 7680;   // conv.cu c_taps: 60 KB of constant bank shared by the live handles
 
 __host__ __device__ constexpr int kind_num_params(int k) {
@@ -76,7 +85,9 @@ struct Program {
 struct PrepArgs {
     const float *params;   // [B][P]
     float *derived;        // [B][D]
+    double *derived64;     // [B][n_models][kD64PerModel]
     int B;
+    double refine_gain;    // scales the refinement threshold G (1 = default; prep.cu)
     double scale, zp;      // arcsec per pixel, magnitude zero point
     double cxh, cyh;       // (W-1)/2, (H-1)/2
 };
@@ -87,13 +98,27 @@ struct TraceArgs {
     const float4 *quad;    // [nq_pad] (xi, eta, w, w - w'), zero-weight padding up to a multiple of R (even);
                            // w' = embedded rule of lensed_set_error_rule (0 before it is set)
     float *err;            // [.][H*W] quadrature error estimates instead of L (trace.cu ERR), or NULL
+    uint32_t *fixmask;     // [nvec][blocks per vector][256] or NULL: per tracer thread, bit i = its i-th
+                           // pixel (list index block base + 256 i + thread) wants the FP64 refinement (refine.cu)
     float *L;              // [.][Hp*Wp], chunk-local PADDED frames: pixel (i, j) at (i + py, j + px),
                            // border pixels replicated into the pad (conv.cu "Input")
     long long l_stride;    // Hp*Wp
     int npix, nq_pad;
     int H, W, Wp, px, py;
-    int pix_per_block;     // pixels of the list one block walks (a multiple of 256)
+    int pix_per_block;     // pixels of the list one block walks (a multiple of 256, at most 8192)
     float cxh, cyh;
+};
+
+struct RefineArgs {
+    TraceArgs t;               // the launch whose flags are refined (pix, quad, L, fixmask, geometry)
+    const double *derived64;   // [nvec][n_models][kD64PerModel], offset to the chunk's first vector
+    const float *derived;      // [nvec][D] (validity is not needed: invalid vectors have no flags)
+    unsigned long long *count; // refined pixels, accumulated (statistic) or NULL
+    uint2 *queue;              // [queue_cap] (vector, pixel-list index) between the two passes
+    unsigned *queue_count;     // entries requested (may exceed queue_cap)
+    int queue_cap;
+    int nvec, n_blocks;        // grid of that launch: vectors, blocks per vector
+    int n_quad;                // unpadded rule length
 };
 
 struct ConvArgs {
@@ -125,6 +150,8 @@ struct FinalArgs {
 cudaError_t launch_prep(const Program &prog, const PrepArgs &a, cudaStream_t st);
 // allow_static: use the compile-time-specialised kernel when the list has one (trace.cu)
 cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nvec, bool allow_static, cudaStream_t st);
+inline int trace_blocks_per_vector(const TraceArgs &a) { return (a.npix + a.pix_per_block - 1) / a.pix_per_block; }
+cudaError_t launch_refine(const Program &prog, const RefineArgs &a, int n_sm, cudaStream_t st);
 bool trace_has_static(const Program &prog);
 cudaError_t launch_conv(ConvArgs a, bool render, int n_blocks, cudaStream_t st);
 cudaError_t conv_upload_taps(const float *pairs, int n_pairs, int pool_offset);

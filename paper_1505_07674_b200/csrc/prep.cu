@@ -1,14 +1,16 @@
 // prep.cu -- step a0: parameter vectors xi -> kernel-ready constants, in FP64 on the device.
 //
-// One thread per parameter vector.  Everything the ray tracer would otherwise recompute per
-// ray is evaluated once here, in double, and rounded to FP32 once:
+// One thread per (parameter vector, model).  Everything the ray tracer would otherwise recompute
+// per ray is evaluated once here, in double, and rounded to FP32 once:
 //   * component centres as (integer pixel, fraction)
 //   * SIE: cos/sin PA, q^2, q' = sqrt(1-q^2), A = b sqrt(q)/q' folded into the rotation
 //     back to the image frame                                  (R2)
 //   * Sersic: b_n from P(2n, b_n) = 1/2 (r_S is the half-light radius; R5),
 //     log2 I_0 from the total magnitude (R6), the rotated, q-stretched,
 //     r_S-scaled frame of eq. 23
-//   * the domain check: outside it the vector is flagged invalid.
+//   * the domain check: outside it the vector is flagged invalid;
+//   * an unrounded FP64 copy of the same constants and, per source Sersic, the squared radius
+//     inside which its pixels are re-traced in FP64 (refine.cu).
 #include "lensed_internal.h"
 #include <math.h>
 
@@ -79,47 +81,74 @@ __device__ inline void put_frame(float *d, double pa_deg, double q, double len_p
     d[3] = (float)(c / (sq * len_px));
 }
 
-__global__ void __launch_bounds__(128) prep_kernel(Program prog, PrepArgs a)
+// FP64 copy of a model's constants for the refinement pass (refine.cu), lengths in pixels
+__device__ inline void put64(double *e, double a0 = 0, double a1 = 0, double a2 = 0, double a3 = 0, double a4 = 0,
+                             double a5 = 0, double a6 = 0, double a7 = 0, double a8 = 0)
 {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= a.B) return;
-    const float *par = a.params + (size_t)b * prog.P;
-    float *der = a.derived + (size_t)b * prog.D;
-    bool valid = true;
-    int mode = 0;
-    for (int i = 0; i < prog.D; ++i) der[i] = 0.0f;
+    e[0] = a0; e[1] = a1; e[2] = a2; e[3] = a3; e[4] = a4; e[5] = a5; e[6] = a6; e[7] = a7; e[8] = a8;
+}
 
-    for (int m = 0; m < prog.n_models; ++m) {
-        const int kind = prog.kind[m];
-        const float *pf = par + prog.par_off[m];
-        float *d = der + prog.der_off[m];
-        double p[7];
-        const int np = kind_num_params(kind);
+constexpr int kPrepVec = 8;            // vectors per block; threadIdx.x = model slot (kMaxModels = 32)
+
+// One thread per (vector, model): the b_n solves of a vector's Sersic components run side by
+// side.  Per vector, shared memory collects validity, the SIE mode and the deflection scale.
+__global__ void __launch_bounds__(kMaxModels * kPrepVec) prep_kernel(Program prog, PrepArgs a)
+{
+    __shared__ int s_valid[kPrepVec], s_mode[kPrepVec];
+    __shared__ float s_defl[kPrepVec][kMaxModels];   // deflection scale of each lens, pixels
+    const int m = threadIdx.x, lv = threadIdx.y;
+    const int b = blockIdx.x * kPrepVec + lv;
+    const bool active = b < a.B && m < prog.n_models;
+    if (m == 0) { s_valid[lv] = 1; s_mode[lv] = 0; }
+    s_defl[lv][m] = 0.0f;
+    __syncthreads();
+
+    float *d = nullptr;
+    double *e = nullptr;
+    int kind = -1;
+    double p[7];
+    bool valid = true;
+    double sersic_c = 0.0, sersic_n = 0.0;          // source Sersic: threshold constants (below)
+    if (active) {
+        kind = prog.kind[m];
+        const float *pf = a.params + (size_t)b * prog.P + prog.par_off[m];
+        d = a.derived + (size_t)b * prog.D + prog.der_off[m];
+        e = a.derived64 + ((size_t)b * prog.n_models + m) * kD64PerModel;
+        const int np = kind_num_params(kind), nd = kind_num_derived(kind);
+        for (int i = 0; i < nd; ++i) d[i] = 0.0f;
+        put64(e);
         for (int i = 0; i < np; ++i) {
             p[i] = (double)pf[i];
             if (!isfinite(p[i])) valid = false;
         }
-        if (!valid) continue;
+    }
+    if (active && valid) {
         switch (kind) {
         case K_SIS:
-            valid = valid && p[2] >= 0.0;
+            valid = p[2] >= 0.0;
             put_centre(d, p[0], p[1], a);
             d[4] = (float)(p[2] / a.scale);
+            put64(e, p[0] / a.scale + a.cxh, p[1] / a.scale + a.cyh, p[2] / a.scale);
+            s_defl[lv][m] = (float)(p[2] / a.scale);
             break;
         case K_POINT:
-            valid = valid && p[2] >= 0.0;
+            valid = p[2] >= 0.0;
             put_centre(d, p[0], p[1], a);
             d[4] = (float)((p[2] / a.scale) * (p[2] / a.scale));
+            put64(e, p[0] / a.scale + a.cxh, p[1] / a.scale + a.cyh, (p[2] / a.scale) * (p[2] / a.scale));
+            s_defl[lv][m] = (float)(p[2] / a.scale);
             break;
         case K_SHEAR:
             d[0] = (float)p[0]; d[1] = (float)p[1];
+            put64(e, p[0], p[1]);
+            s_defl[lv][m] = (float)(sqrt(p[0] * p[0] + p[1] * p[1]) * sqrt(a.cxh * a.cxh + a.cyh * a.cyh));
             break;
         case K_SIE: {
             const double q = p[3];
-            valid = valid && p[2] >= 0.0 && q > 0.0 && q <= 1.0;
+            valid = p[2] >= 0.0 && q > 0.0 && q <= 1.0;
             if (!valid) break;
             put_centre(d, p[0], p[1], a);
-            mode = max(mode, sie_mode(q));
+            atomicMax(&s_mode[lv], sie_mode(q));
             double s, c;
             sincos(p[4] * (kPi / 180.0), &s, &c);
             d[4] = (float)c; d[5] = (float)s;
@@ -131,11 +160,13 @@ __global__ void __launch_bounds__(128) prep_kernel(Program prog, PrepArgs a)
             d[7] = (float)qp;
             d[8] = (float)(c * A); d[9] = (float)(s * A);
             d[10] = (float)(c * A * (0.5 * kLn2)); d[11] = (float)(-s * A * (0.5 * kLn2));
+            put64(e, p[0] / a.scale + a.cxh, p[1] / a.scale + a.cyh, c, s, q, p[2] / a.scale);
+            s_defl[lv][m] = (float)(p[2] / a.scale);
             break;
         }
         case K_SRC_SERSIC: case K_FG_SERSIC: {
             const double rs = p[2] / a.scale, mag = p[3], n = p[4], q = p[5];
-            valid = valid && p[2] > 0.0 && n >= 0.02 && n <= 20.0 && q > 0.0 && q <= 1.0;
+            valid = p[2] > 0.0 && n >= 0.02 && n <= 20.0 && q > 0.0 && q <= 1.0;
             if (!valid) break;
             put_centre(d, p[0], p[1], a);
             put_frame(d + 4, p[6], q, rs);
@@ -146,36 +177,63 @@ __global__ void __launch_bounds__(128) prep_kernel(Program prog, PrepArgs a)
             d[8] = (float)(ln_i0 / kLn2);
             d[9] = (float)(bn / kLn2);
             d[10] = (float)(0.5 / n);
+            double s, c;
+            sincos(p[6] * (kPi / 180.0), &s, &c);
+            put64(e, p[0] / a.scale + a.cxh, p[1] / a.scale + a.cyh, c, s, q, rs, 1.0 / n, bn, ln_i0);
+            if (kind == K_SRC_SERSIC && n > 1.0) { sersic_c = n * sqrt(q) * rs / bn; sersic_n = n; }
             break;
         }
         case K_SRC_GAUSS: case K_FG_GAUSS: {
             const double sg = p[2] / a.scale, mag = p[3], q = p[4];
-            valid = valid && p[2] > 0.0 && q > 0.0 && q <= 1.0;
+            valid = p[2] > 0.0 && q > 0.0 && q <= 1.0;
             if (!valid) break;
             put_centre(d, p[0], p[1], a);
             put_frame(d + 4, p[5], q, sg);
             const double ln_i0 = -0.4 * (mag - a.zp) * kLn10 - log(2.0 * kPi * sg * sg);
             d[8] = (float)(ln_i0 / kLn2);
             d[9] = (float)(0.5 / kLn2);
+            double s, c;
+            sincos(p[5] * (kPi / 180.0), &s, &c);
+            put64(e, p[0] / a.scale + a.cxh, p[1] / a.scale + a.cyh, c, s, q, sg, ln_i0);
             break;
         }
         case K_SKY:
             d[0] = (float)p[0];
+            put64(e, p[0]);
             break;
         default:
             valid = false;
         }
     }
-    der[0] = valid ? 1.0f : 0.0f;
-    der[1] = (float)mode;
+    if (active && !valid) atomicAnd(&s_valid[lv], 0);
+    __syncthreads();
+    if (!active) return;
+    // Refinement threshold of a source Sersic with n > 1 (refine.cu; DESIGN.md "FP32 and the
+    // cusp"): a ray position carries ~eps |alpha| of FP32 rounding noise, and the profile turns a
+    // displacement dx (pixels) into  d ln I = (b_n/n) R'^(1/n-1) / (sqrt(q) r_S) dx  at most,
+    // R' = R/r_S.  Pixels with a ray where that slope exceeds G = 200 / max(deflection scale, 25 px)
+    // per pixel are re-traced in FP64:  R'^2 < T2 = (G n sqrt(q) r_S / b_n)^(-2n/(n-1)).
+    if (sersic_c > 0.0 && s_valid[lv]) {
+        float defl = 0.0f;
+        for (int i = 0; i < prog.n_models; ++i) defl += s_defl[lv][i];     // list order: deterministic
+        const double G = a.refine_gain * 200.0 / fmax((double)defl, 25.0);
+        const double cc = G * sersic_c;
+        d[11] = (float)fmin(pow(cc, -2.0 * sersic_n / (sersic_n - 1.0)), 1e30);
+    }
+    if (m == 0) {
+        float *der = a.derived + (size_t)b * prog.D;
+        der[0] = s_valid[lv] ? 1.0f : 0.0f;
+        der[1] = (float)s_mode[lv];
+        der[2] = 0.0f; der[3] = 0.0f;
+    }
 }
 
 }  // namespace
 
 cudaError_t launch_prep(const Program &prog, const PrepArgs &a, cudaStream_t st)
 {
-    const int threads = 128;
-    prep_kernel<<<(a.B + threads - 1) / threads, threads, 0, st>>>(prog, a);
+    const dim3 block(kMaxModels, kPrepVec);
+    prep_kernel<<<(a.B + kPrepVec - 1) / kPrepVec, block, 0, st>>>(prog, a);
     return cudaGetLastError();
 }
 

@@ -74,6 +74,7 @@ __global__ void __launch_bounds__(kTraceThreads, LENSED_MINB_GENERIC) trace_kern
     extern __shared__ float4 smem4[];
     const TraceBlock tb = trace_prologue(prog, a, smem4);
     if (!tb.valid) {
+        if (!ERR && a.fixmask) a.fixmask[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = 0;
         if (ERR) {
             const int base = blockIdx.x * a.pix_per_block, end = min(base + a.pix_per_block, a.npix);
             for (int ip = base + threadIdx.x; ip < end; ip += kTraceThreads) {
@@ -91,12 +92,14 @@ __global__ void __launch_bounds__(kTraceThreads, LENSED_MINB_GENERIC) trace_kern
 
     const int base = blockIdx.x * a.pix_per_block;
     const int end = min(base + a.pix_per_block, a.npix);
+    uint32_t flags = 0;                // bit i: this thread's i-th pixel is flagged for refine.cu
 #pragma unroll 1
     for (int ip = base + threadIdx.x; ip < end; ip += kTraceThreads) {
         const uint32_t rc = a.pix[ip];
         const int row = (int)(rc >> 16), col = (int)(rc & 0xffffu);
         const float jf = (float)col, rf = (float)row;
         f2 acc = bc(0.0f);
+        bool flag = false;
 #pragma unroll 1
         for (int q0 = 0; q0 < nq; q0 += R) {
             Rays<NP> r;
@@ -142,11 +145,15 @@ __global__ void __launch_bounds__(kTraceThreads, LENSED_MINB_GENERIC) trace_kern
                 const float4 *d = sder + (prog.light_off[m] >> 2);
                 const float *tu = stab + (size_t)(2 * (1 + prog.n_lens + m)) * nq + q0, *tv = tu + nq;
                 light_origin(d, jf, rf, u0, v0);
+                float rmin = 3e38f;
                 switch (kind) {
-                case K_SRC_SERSIC: light_profile<NP, true, false, false>(d, tu, tv, u0, v0, r); break;
-                case K_FG_SERSIC:  light_profile<NP, false, false, false>(d, tu, tv, u0, v0, r); break;
-                case K_SRC_GAUSS:  light_profile<NP, true, true, false>(d, tu, tv, u0, v0, r); break;
-                default:           light_profile<NP, false, true, false>(d, tu, tv, u0, v0, r); break;
+                case K_SRC_SERSIC:
+                    light_profile<NP, true, false, false>(d, tu, tv, u0, v0, r, nullptr, rmin);
+                    flag = flag || rmin < d[2].w;
+                    break;
+                case K_FG_SERSIC:  light_profile<NP, false, false, false>(d, tu, tv, u0, v0, r, nullptr, rmin); break;
+                case K_SRC_GAUSS:  light_profile<NP, true, true, false>(d, tu, tv, u0, v0, r, nullptr, rmin); break;
+                default:           light_profile<NP, false, true, false>(d, tu, tv, u0, v0, r, nullptr, rmin); break;
                 }
             }
             f2 w[NP];
@@ -156,7 +163,9 @@ __global__ void __launch_bounds__(kTraceThreads, LENSED_MINB_GENERIC) trace_kern
         }
         if (ERR) a.err[(size_t)blockIdx.y * a.H * a.W + (size_t)row * a.W + col] = fabsf(lo2(acc) + hi2(acc));
         else store_pixel(a, Lb, row, col, (lo2(acc) + hi2(acc)) + tb.sky);
+        if (flag) flags |= 1u << ((ip - base) >> 8);
     }
+    if (!ERR && a.fixmask) a.fixmask[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = flags;
 }
 
 }  // namespace

@@ -20,6 +20,7 @@ __device__ __forceinline__ float mufu_rsq(float x) { float y; asm("rsqrt.approx.
 __device__ __forceinline__ float mufu_rcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float mufu_lg2(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float mufu_ex2(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float min3(float a, float b, float c) { float y; asm("min.f32 %0, %1, %2, %3;" : "=f"(y) : "f"(a), "f"(b), "f"(c)); return y; }   // FMNMX3
 
 constexpr float kTiny = 1e-30f;            // floor of squared radii: rsqrt / rcp stay finite, 0 * finite = 0
 constexpr float kHalfPi = 1.5707963267948966f;
@@ -125,11 +126,16 @@ __device__ __forceinline__ f2 sie_atan2x(f2 z)
     }
 }
 
-// (2/ln 2) atanh(q' v / psi) for a pair, from v and s = q'/psi
+// (2/ln 2) atanh(q' v / psi) for a pair, from v and s = q'/psi; qp = q' of THIS lens.
+// The mode is per vector (the most general one any of its SIEs needs), so in mode 5 a second,
+// rounder SIE of the same vector arrives here too: its A = b sqrt(q)/q' is large and the log
+// form's absolute error would be multiplied by it.  The branch on its own q' (block-uniform)
+// keeps the invariant "log form only where q' >= 0.6, A <= 1.7 b".
 template <int MODE>
-__device__ __forceinline__ f2 sie_atanh2x(f2 v, f2 s)
+__device__ __forceinline__ f2 sie_atanh2x(f2 v, f2 s, float qp)
 {
     if constexpr (MODE >= kAtanhLogFrom) {
+        if (qp < 0.6f) return odd_poly2<7, false>(mul2(v, s), kAtanh036, 0.0f);    // z^2 <= q'^2 < 0.36
         const f2 num = fma2(v, s, bc(1.0f));
         f2 den = fma2(v, mul2(s, bc(-1.0f)), bc(1.0f));
         if (MODE >= 5) den = map2(den, [](float x) { return fmaxf(x, 1e-7f); });   // q' -> 1 on the v axis
@@ -180,7 +186,7 @@ __device__ __forceinline__ void lens_sie(const float4 *d, const float *tu, const
         const f2 ipsi = map2(psi2, [](float x) { return mufu_rsq(fmaxf(x, kTiny)); });
         const f2 s = mul2(ipsi, bc(c1.w));
         const f2 at = sie_atan2x<MODE>(mul2(u, s));
-        const f2 lv = sie_atanh2x<MODE>(v, s);
+        const f2 lv = sie_atanh2x<MODE>(v, s, c1.w);
         if (RAW) {
             r.ax[k] = at;
             r.ay[k] = lv;
@@ -261,9 +267,11 @@ __device__ __forceinline__ void light_origin(const float4 *d, float jf, float rf
 
 // cm: the 2 x 2 matrix applied to (r.ax, r.ay) of a source -- the frame M itself (d[1]) when
 // they hold the deflection, B when they hold the SIE's raw functions.
+// rmin (source Sersic only): running minimum of (R/r_S)^2 over the rays of the pixel; the caller
+// compares it with the block's T2 (lensed_internal.h) to flag the pixel for the FP64 refinement.
 template <int NP, bool SRC, bool GAUSS, bool INIT>
 __device__ __forceinline__ void light_profile(const float4 *d, const float *tu, const float *tv, float u0, float v0,
-                                              Rays<NP> &r, const float4 *cm = nullptr)
+                                              Rays<NP> &r, const float4 *cm, float &rmin)
 {
     const float4 c1 = cm ? cm[0] : d[1], c2 = d[2];
     const float nk = -c2.y;
@@ -282,6 +290,9 @@ __device__ __forceinline__ void light_profile(const float4 *d, const float *tu, 
         if (GAUSS) {
             x = fma2(r2, bc(nk), bc(c2.x));
         } else {
+#ifndef LENSED_NO_FLAG                  // tuning builds: what the flagging costs
+            if (SRC) rmin = min3(rmin, lo2(r2), hi2(r2));
+#endif
             const f2 lg = map2(r2, [](float a) { return mufu_lg2(a); });
             const f2 e = map2(mul2(lg, bc(c2.z)), [](float a) { return mufu_ex2(a); });
             x = fma2(e, bc(nk), bc(c2.x));

@@ -50,11 +50,18 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
 
     const int base = blockIdx.x * a.pix_per_block;
     const int end = min(base + a.pix_per_block, a.npix);
+    // this thread's flags: bit i = its i-th pixel has a ray inside a source Sersic's cusp zone,
+    // (R/r_S)^2 < T2 of lensed_internal.h (refine.cu)
+    uint32_t flags = 0, bit = 1;
 #pragma unroll 1
-    for (int ip = base + threadIdx.x; ip < end; ip += kTraceThreads) {
+    for (int ip = base + threadIdx.x; ip < end; ip += kTraceThreads, bit += bit) {
         const uint32_t rc = a.pix[ip];
         const int row = (int)(rc >> 16), col = (int)(rc & 0xffffu);
         const float jf = (float)col, rf = (float)row;
+        float rmin[S::n_ss > 0 ? S::n_ss : 1];
+#pragma unroll
+        for (int i = 0; i < S::n_ss; ++i) rmin[i] = 3e38f;
+        float rdummy = 0.0f;
 
         // frame origins of this pixel
         float lu[NL > 0 ? NL : 1], lv[NL > 0 ? NL : 1], gu[NPOS > 0 ? NPOS : 1], gv[NPOS > 0 ? NPOS : 1];
@@ -113,7 +120,8 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
 #define LENSED_LIGHT(m, SRC, GAUSS, INIT)                                                                     \
     light_profile<NP, SRC, GAUSS, INIT>(sder + (prog.light_off[m] >> 2), gtab + (size_t)(2 * (m)) * nq + q0, \
                                         gtab + (size_t)(2 * (m) + 1) * nq + q0, gu[m], gv[m], r,              \
-                                        (SRC) && S::direct ? tb.smat + (m) : nullptr)
+                                        (SRC) && S::direct ? tb.smat + (m) : nullptr,                         \
+                                        (SRC) && !(GAUSS) ? rmin[(m) < S::n_ss ? (m) : 0] : rdummy)
             constexpr bool fg_first = S::n_fs + S::n_fg > 0;
 #pragma unroll
             for (int i = 0; i < S::n_fs; ++i) {
@@ -142,7 +150,11 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
             for (int k = 0; k < NP; ++k) acc = fma2(w[k], r.I[k], acc);
         }
         store_pixel(a, Lb, row, col, (lo2(acc) + hi2(acc)) + tb.sky);
+#pragma unroll
+        for (int i = 0; i < S::n_ss; ++i)
+            if (rmin[i] < sder[(prog.light_off[i] >> 2) + 2].w) flags |= bit;
     }
+    if (a.fixmask) a.fixmask[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = flags;
 }
 
 // MINB = resident blocks per SM the register budget is cut for (3 -> 80 registers, 2 -> 128):
@@ -152,7 +164,10 @@ __global__ void __launch_bounds__(kTraceThreads, MINB) trace_static_kernel(Progr
 {
     extern __shared__ float4 smem4[];
     const TraceBlock tb = trace_prologue(prog, a, smem4);
-    if (!tb.valid) return;
+    if (!tb.valid) {
+        if (a.fixmask) a.fixmask[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = 0;
+        return;
+    }
     if constexpr (S::direct) {
         // source tables lose M Gamma (rule offset); B per source (TraceSig "direct frames")
         const int nq = a.nq_pad;

@@ -19,7 +19,7 @@ STATUS_NAMES = {0: "LENSED_OK", 1: "LENSED_EINVAL", 2: "LENSED_ENOMEM", 3: "LENS
 # lensed_kind (include/lensed.h)
 LENS_SIS, LENS_SIE, LENS_POINT, LENS_SHEAR = 0, 1, 2, 3
 SRC_SERSIC, SRC_GAUSS, FG_SERSIC, FG_GAUSS, FG_SKY = 4, 5, 6, 7, 8
-PHASES = ("prep", "trace", "conv", "final")
+PHASES = ("prep", "trace", "refine", "conv", "final")
 
 # every symbol include/lensed.h declares: (restype, argtypes)
 _c, _i, _d, _p, _ll = ctypes.c_char_p, ctypes.c_int, ctypes.c_double, ctypes.c_void_p, ctypes.c_longlong
@@ -27,6 +27,7 @@ SYMBOLS = {
     "lensed_create": (_i, [_i, _i, _d, _p, _p, _p, _p, _i, _i, _p, _i, _p, _i, _d, _i, _p]),
     "lensed_num_params": (_i, [_p]),
     "lensed_num_traced": (_i, [_p]),
+    "lensed_num_pixels": (_i, [_p]),
     "lensed_render": (_i, [_p, _p, _i, _p, _p]),
     "lensed_loglike": (_i, [_p, _p, _i, _p, _p]),
     "lensed_render_host": (_i, [_p, _p, _i, _p, _p]),
@@ -37,6 +38,8 @@ SYMBOLS = {
     "lensed_set_profiling": (_i, [_p, _i]),
     "lensed_get_profile": (_i, [_p, _p, _p]),
     "lensed_reset_profile": (_i, [_p]),
+    "lensed_set_refine": (_i, [_p, _d]),
+    "lensed_get_refined": (_i, [_p, _p]),
     "lensed_set_chunk_bytes": (_i, [_p, _ll]),
     "lensed_frame_bytes": (_ll, [_p]),
     "lensed_set_static_tracer": (_i, [_p, _i]),
@@ -121,10 +124,15 @@ def lensed_num_traced(h):
     return lib().lensed_num_traced(h)
 
 
+def lensed_num_pixels(h):
+    """H * W of the handle's image."""
+    return lib().lensed_num_pixels(h)
+
+
 def lensed_render(h, params_dev, model_dev, stream=None):
     """params_dev [B][P], model_dev [B][H][W]: contiguous float32 CUDA tensors."""
     B = _check_dev(h, params_dev)
-    _check_out(model_dev, B)
+    _check_out(model_dev, B, B * lensed_num_pixels(h))
     _check(lib().lensed_render(h, params_dev.data_ptr(), B, model_dev.data_ptr(), _stream(stream)), h)
     return model_dev
 
@@ -150,7 +158,7 @@ def lensed_set_error_rule(h, w_embedded):
 def lensed_render_error(h, params_dev, err_dev, stream=None):
     """params_dev [B][P], err_dev [B][H][W]: contiguous float32 CUDA tensors."""
     B = _check_dev(h, params_dev)
-    _check_out(err_dev, B)
+    _check_out(err_dev, B, B * lensed_num_pixels(h))
     _check(lib().lensed_render_error(h, params_dev.data_ptr(), B, err_dev.data_ptr(), _stream(stream)), h)
     return err_dev
 
@@ -158,7 +166,7 @@ def lensed_render_error(h, params_dev, err_dev, stream=None):
 def lensed_loglike(h, params_dev, logl_dev, stream=None):
     """params_dev [B][P], logl_dev [B]: contiguous float32 CUDA tensors."""
     B = _check_dev(h, params_dev)
-    _check_out(logl_dev, B)
+    _check_out(logl_dev, B, B)
     _check(lib().lensed_loglike(h, params_dev.data_ptr(), B, logl_dev.data_ptr(), _stream(stream)), h)
     return logl_dev
 
@@ -184,14 +192,25 @@ def lensed_set_profiling(h, on):
 
 def lensed_get_profile(h):
     """-> ({phase: ms}, {phase: launches}) since the last reset."""
-    ms = (ctypes.c_double * 4)()
-    n = (ctypes.c_longlong * 4)()
+    ms = (ctypes.c_double * len(PHASES))()
+    n = (ctypes.c_longlong * len(PHASES))()
     _check(lib().lensed_get_profile(h, ms, n), h)
     return dict(zip(PHASES, ms)), dict(zip(PHASES, n))
 
 
 def lensed_reset_profile(h):
     _check(lib().lensed_reset_profile(h), h)
+
+
+def lensed_set_refine(h, gain):
+    _check(lib().lensed_set_refine(h, float(gain)), h)
+
+
+def lensed_get_refined(h):
+    """-> pixels re-traced in FP64 since the last lensed_reset_profile."""
+    n = ctypes.c_longlong()
+    _check(lib().lensed_get_refined(h, ctypes.byref(n)), h)
+    return n.value
 
 
 def lensed_set_chunk_bytes(h, nbytes):
@@ -236,9 +255,11 @@ def _check_dev(h, params_dev):
     return int(params_dev.shape[0])
 
 
-def _check_out(t, B):
-    if not (t.is_cuda and t.is_contiguous() and str(t.dtype) == "torch.float32" and t.shape[0] == B):
-        raise LensedError(EINVAL, "output must be a contiguous float32 CUDA tensor with leading dim B")
+def _check_out(t, B, numel):
+    if not (t.is_cuda and t.is_contiguous() and str(t.dtype) == "torch.float32" and t.dim() >= 1
+            and t.shape[0] == B and t.numel() == numel):
+        raise LensedError(EINVAL, "output must be a contiguous float32 CUDA tensor of %d elements with leading dim %d"
+                          % (numel, B))
 
 
 def _host_ptr(a, P):

@@ -125,8 +125,11 @@ def test_paper_mock_scenario_gauss_kronrod_rule(L):
 
 
 # ------------------------------------------------- full sizes, bench launch configuration
-@pytest.mark.parametrize("index,B,n_sample", [(1, 1024, 6), (2, 4096, 3), (3, 4096, 2), (4, 16384, 3), (5, 4096, 3)])
+@pytest.mark.parametrize("index,B,n_sample", [(1, 1024, 128), (2, 4096, 96), (3, 4096, 64), (4, 16384, 64), (5, 4096, 128)])
 def test_full_size_configs_on_sampled_vectors(L, index, B, n_sample):
+    """BASELINE.json's full sizes in the launch configuration bench.py times; 64-128 vectors per
+    config spread over the batch, each against the oracle on every pixel, so that the test sees
+    the tail of the prior (about one draw in a hundred has a source cusp on a pixel)."""
     import torch
     cfg = synth.get_config(index)
     prob = Problem(cfg)
@@ -265,7 +268,7 @@ def test_host_buffer_calls_match_device_calls_and_chunking_does_not_change_resul
     assert np.array_equal(logl_dev, logl_host) and np.array_equal(logl_dev, out_pinned.numpy())
     assert np.array_equal(model_dev, model_host)
     assert np.array_equal(logl_dev, logl_chunked) and np.array_equal(model_dev, model_chunked)
-    assert n == {"prep": 1, "trace": 14, "conv": 14, "final": 1}
+    assert n == {"prep": 1, "trace": 14, "refine": 28, "conv": 14, "final": 1}
     assert all(v > 0 for v in ms.values())
 
 
@@ -394,25 +397,77 @@ def test_largest_rule_and_longest_model_list(L):
     _check(L, prob, np.vstack([cfg.truth.astype(np.float32)[None]] * 2))
 
 
-@pytest.mark.parametrize("index,H,W", [(1, 48, 40), (2, 64, 56), (3, 56, 48), (4, 60, 52)])
-def test_error_envelope_over_192_draws_of_the_prior(L, index, H, W):
-    """The small-batch tests above meet north_star's bounds on every vector they draw.  Over a
-    larger sample of the same priors FP32 ray positions (~3e-6 px of noise on a 20-px
-    deflection) meet the cusp of compact high-n Sersic sources, and about one draw in a hundred
-    lands above 1e-5 on logL.  This pins the envelope: median and 99th
-    percentile inside the bounds, the worst draw within 5x of them."""
+@pytest.mark.parametrize("static", [True, False])
+@pytest.mark.parametrize("index,H,W", [(1, 48, 40), (2, 64, 56), (3, 56, 48), (4, 60, 52), (5, 60, 64)])
+def test_every_one_of_192_draws_of_the_prior_meets_the_tolerances(L, index, H, W, static):
+    """192 draws per prior -- BASELINE.json's four and the paper's own mock prior (n <= 8,
+    q_S >= 0.1) -- on shrunk images, both tracers: EVERY vector inside north_star's
+    bounds.  In plain FP32 about one draw in a hundred misses 1e-5 on logL (a source cusp on a
+    pixel: DESIGN.md section 6); the FP64 refinement of the flagged pixels (refine.cu) closes
+    that tail, and switching it off brings it back (test_refinement_switch below)."""
     cfg = synth.shrunk(synth.get_config(index), H, W, 4)
     params = cfg.batch(192)
     prob = Problem(cfg)
     h = prob.create()
     try:
+        if not static:
+            L.lensed_set_static_tracer(h, 0)
         logl_g, model_g = _gpu_eval(L, h, params, cfg.H, cfg.W)
     finally:
         L.lensed_destroy(h)
     logl_o, model_o = prob.oracle_loglike(params, want_model=True)
     el, ep = logl_errors(logl_g, logl_o), pixel_errors(model_g, model_o)
-    assert np.median(el) <= 0.1 * LOGL_RTOL and np.percentile(el, 99) <= LOGL_RTOL and el.max() <= 5 * LOGL_RTOL
-    assert np.percentile(ep, 99) <= PIXEL_RTOL and ep.max() <= 5 * PIXEL_RTOL
+    assert np.median(el) <= 0.1 * LOGL_RTOL and el.max() <= LOGL_RTOL, "logL rel err %.3g at %d" % (el.max(), el.argmax())
+    assert ep.max() <= PIXEL_RTOL, "pixel rel err %.3g at %d" % (ep.max(), ep.argmax())
+
+
+def test_refinement_switch(L):
+    """lensed_set_refine: with the default gain a few pixels per vector are re-traced in FP64 and
+    the paper's mock prior meets the tolerances; with gain 0 nothing is refined and the known FP32
+    tail is back (if this second half ever passes the tolerances, the refinement is dead weight);
+    a larger gain refines fewer pixels; results are bitwise reproducible either way."""
+    import torch
+    cfg = synth.shrunk(synth.get_config(5), 60, 64, 4)
+    params = cfg.batch(192)
+    prob = Problem(cfg)
+    logl_o = prob.oracle_loglike(params, want_model=False)
+    p = torch.from_numpy(params).cuda()
+    out = {}
+    h = prob.create()
+    try:
+        for gain in (1.0, 4.0, 0.0):
+            L.lensed_set_refine(h, gain)
+            L.lensed_reset_profile(h)
+            a = torch.empty(len(params), dtype=torch.float32, device="cuda")
+            b = torch.empty_like(a)
+            L.lensed_loglike(h, p, a)
+            n = L.lensed_get_refined(h)
+            L.lensed_loglike(h, p, b)
+            assert torch.equal(a, b)
+            assert L.lensed_get_refined(h) == 2 * n
+            out[gain] = (logl_errors(a.cpu().numpy(), logl_o), n)
+    finally:
+        L.lensed_destroy(h)
+    assert out[1.0][0].max() <= LOGL_RTOL and 192 <= out[1.0][1] <= 192 * 40
+    assert 0 < out[4.0][1] < out[1.0][1]
+    assert out[0.0][1] == 0 and out[0.0][0].max() > 3 * LOGL_RTOL
+
+
+@pytest.mark.parametrize("static", [True, False])
+def test_two_sies_in_different_modes_one_flat_one_round(L, static):
+    """The SIE mode is per vector (the most general one any of its SIEs needs).  A flat SIE
+    (q = 0.3: log-form atanh) beside a round one (q = 1, 0.9999, 0.97: A = b sqrt(q)/q' is huge)
+    must not push the round one through the log form (its absolute error times A); realistic
+    Einstein radii, the multi-lens list of config 3 in both tracers."""
+    cfg = synth.shrunk(synth.get_config(3), 64, 72, 4)
+    assert cfg.models[:2] == ("sie", "sie")
+    rows = []
+    for q1, q2 in ((0.3, 1.0), (0.3, 0.9999), (0.45, 0.97), (1.0, 0.3), (0.99999, 0.2), (0.3, 0.35)):
+        p = cfg.truth.astype(np.float32).copy()
+        p[3], p[8] = q1, q2
+        p[7] = 0.9                                     # second Einstein radius 0.9": 18 pixels
+        rows.append(p)
+    _check(L, Problem(cfg), np.array(rows), static=static)
 
 
 @pytest.mark.parametrize("static", [True, False])
