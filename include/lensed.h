@@ -132,6 +132,33 @@ lensed_status lensed_render(lensed_handle *h, const float *params_dev, int B,
 lensed_status lensed_loglike(lensed_handle *h, const float *params_dev, int B,
                              float *logl_dev, void *cuda_stream);
 
+/*
+ * Image-plane priors (section 5): "Instead of defining the prior
+ * distribution on the source plane, one can define a prior on the image plane for the position
+ * at which one of the images of the source is required to appear.  Drawing from such a
+ * distribution is done ... by first sampling a position on the image plane, mapping it to the
+ * source plane, and assigning it to the source."
+ *
+ * lensed_deflect -- the map itself, y = x - sum_lenses alpha(x) (eq. 1), for K
+ * image-plane points per parameter vector through that vector's own lens list.
+ *   params_dev  [B][P] device f32 (light components of the list are ignored)
+ *   xy_dev      [B][K][2] device f32: image-plane (x, y), arcsec (R1)
+ *   out_dev     [B][K][2] device f32: source-plane (x, y), arcsec; NaN where a lens parameter of
+ *               the vector is outside its domain or the point is not finite
+ * Double-precision arithmetic on the device.  Asynchronous.  EINVAL for null pointers, B < 1, K < 1.
+ *
+ * lensed_image_plane_prior -- the assignment, in place: for every vector and every listed
+ * source component, its (x, y) parameters hold an image-plane position on entry (what the
+ * sampler drew from the image-plane prior) and the source-plane position y(x) on return.
+ *   params_dev     [B][P] device f32, read and written (only those (x, y) entries change)
+ *   source_models  [n_sources] HOST: indices into the model list given to lensed_create; each
+ *                  must be a LENSED_SRC_* component, none twice
+ * Asynchronous.  EINVAL for null pointers, B < 1, a bad or repeated index, a non-source.        */
+lensed_status lensed_deflect(lensed_handle *h, const float *params_dev, int B, const float *xy_dev, int K,
+                             float *out_dev, void *cuda_stream);
+lensed_status lensed_image_plane_prior(lensed_handle *h, float *params_dev, int B, const int *source_models,
+                                       int n_sources, void *cuda_stream);
+
 /* The same two calls with HOST buffers: the parameters are copied to the device, the
  * result is copied back and the stream is synchronised before returning.  Pinned host
  * memory makes the copies asynchronous until that final synchronisation.                */

@@ -634,6 +634,41 @@ lensed_status lensed_render_error(lensed_handle *h, const float *params_dev, int
     return LENSED_OK;
 }
 
+lensed_status lensed_deflect(lensed_handle *h, const float *params_dev, int B, const float *xy_dev, int K,
+                             float *out_dev, void *stream)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (!params_dev || !xy_dev || !out_dev) return fail(h, LENSED_EINVAL, "null device pointer");
+    if (B < 1 || K < 1) return fail(h, LENSED_EINVAL, "B = %d, K = %d: both must be >= 1", B, K);
+    CU(h, cudaSetDevice(h->device));
+    CU(h, launch_deflect(h->prog, params_dev, B, xy_dev, K, out_dev, (cudaStream_t)stream));
+    return LENSED_OK;
+}
+
+lensed_status lensed_image_plane_prior(lensed_handle *h, float *params_dev, int B, const int *source_models,
+                                       int n_sources, void *stream)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (!params_dev || !source_models) return fail(h, LENSED_EINVAL, "null pointer");
+    if (B < 1) return fail(h, LENSED_EINVAL, "B = %d < 1", B);
+    if (n_sources < 1 || n_sources > kMaxModels) return fail(h, LENSED_EINVAL, "n_sources = %d", n_sources);
+    int offs[kMaxModels];
+    for (int i = 0; i < n_sources; ++i) {
+        const int m = source_models[i];
+        if (m < 0 || m >= h->prog.n_models)
+            return fail(h, LENSED_EINVAL, "source_models[%d] = %d is not an index of the model list", i, m);
+        const int k = h->prog.kind[m];
+        if (k != K_SRC_SERSIC && k != K_SRC_GAUSS)
+            return fail(h, LENSED_EINVAL, "model %d is not a source (LENSED_SRC_*): only sources live in the source plane", m);
+        for (int j = 0; j < i; ++j)
+            if (source_models[j] == m) return fail(h, LENSED_EINVAL, "model %d listed twice", m);
+        offs[i] = h->prog.par_off[m];
+    }
+    CU(h, cudaSetDevice(h->device));
+    CU(h, launch_image_plane_prior(h->prog, offs, n_sources, params_dev, B, (cudaStream_t)stream));
+    return LENSED_OK;
+}
+
 lensed_status lensed_render(lensed_handle *h, const float *params_dev, int B, float *model_dev, void *stream)
 {
     return run(h, params_dev, B, model_dev, true, (cudaStream_t)stream);

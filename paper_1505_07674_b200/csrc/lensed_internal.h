@@ -157,6 +157,11 @@ cudaError_t launch_conv(ConvArgs a, bool render, int n_blocks, cudaStream_t st);
 cudaError_t conv_upload_taps(const float *pairs, int n_pairs, int pool_offset);
 void conv_padded_shape(int rows, int cols, int KH, int NC, int *Hp, int *Wp);
 cudaError_t launch_final(const FinalArgs &a, cudaStream_t st);
+// deflect.cu: y = x - sum alpha for K points per vector / in place for the listed sources' (x, y)
+cudaError_t launch_deflect(const Program &prog, const float *params, int B, const float *xy, int K, float *out,
+                           cudaStream_t st);
+cudaError_t launch_image_plane_prior(const Program &prog, const int *par_offs, int n_src, float *params, int B,
+                                     cudaStream_t st);
 cudaError_t conv_setup();                 // one-time function attributes
 int trace_pick_R(int n_quad);             // rays per register block for an n_quad-point rule
 size_t trace_smem_bytes(const Program &prog, int nq_pad);

@@ -31,6 +31,8 @@ SYMBOLS = {
     "lensed_render": (_i, [_p, _p, _i, _p, _p]),
     "lensed_loglike": (_i, [_p, _p, _i, _p, _p]),
     "lensed_render_host": (_i, [_p, _p, _i, _p, _p]),
+    "lensed_deflect": (_i, [_p, _p, _i, _p, _i, _p, _p]),
+    "lensed_image_plane_prior": (_i, [_p, _p, _i, _p, _i, _p]),
     "lensed_estimate_weights": (_i, [_ll, _p, _p, _d, _p, _d, _p, _p]),
     "lensed_set_error_rule": (_i, [_p, _p]),
     "lensed_render_error": (_i, [_p, _p, _i, _p, _p]),
@@ -169,6 +171,26 @@ def lensed_loglike(h, params_dev, logl_dev, stream=None):
     _check_out(logl_dev, B, B)
     _check(lib().lensed_loglike(h, params_dev.data_ptr(), B, logl_dev.data_ptr(), _stream(stream)), h)
     return logl_dev
+
+
+def lensed_deflect(h, params_dev, xy_dev, out_dev, stream=None):
+    """params_dev [B][P], xy_dev / out_dev [B][K][2]: contiguous float32 CUDA tensors (arcsec)."""
+    B = _check_dev(h, params_dev)
+    if xy_dev.dim() != 3 or xy_dev.shape[0] != B or xy_dev.shape[2] != 2 or xy_dev.shape[1] < 1:
+        raise LensedError(EINVAL, "xy must be [B][K][2]")
+    for t in (xy_dev, out_dev):
+        _check_out(t, B, xy_dev.numel())
+    _check(lib().lensed_deflect(h, params_dev.data_ptr(), B, xy_dev.data_ptr(), int(xy_dev.shape[1]),
+                                out_dev.data_ptr(), _stream(stream)), h)
+    return out_dev
+
+
+def lensed_image_plane_prior(h, params_dev, source_models, stream=None):
+    """In place: the (x, y) of the listed source components, image plane -> source plane."""
+    B = _check_dev(h, params_dev)
+    idx = _np(source_models, np.int32).reshape(-1)
+    _check(lib().lensed_image_plane_prior(h, params_dev.data_ptr(), B, _hp(idx), len(idx), _stream(stream)), h)
+    return params_dev
 
 
 def lensed_render_host(h, params_host, model_host, stream=None):
