@@ -254,6 +254,50 @@ lensed_status lensed_set_error_rule(lensed_handle *h, const float *w_embedded);
 lensed_status lensed_render_error(lensed_handle *h, const float *params_dev, int B, float *err_dev, void *stream);
 
 /*
+ * lensed_ns_run -- device-resident nested sampling with the batched likelihood.
+ * PAPER.md:134-139 steps (iii)-(vii): draw parameters from the prior, compute their likelihood,
+ * accumulate the posterior, repeat until the parameter space is sufficiently sampled;
+ * the sampler is Nested Sampling (Skilling 2004, 2006), which also gives
+ * the evidence (eq. 13).  The paper delegates this to the MultiNest library;
+ * this call is the base algorithm with MultiNest's ellipsoidal bound (a single ellipsoid), run
+ * with everything on the device: live points, proposal batches, evidence accumulators and dead
+ * points.  Each round proposes `batch` vectors inside the current likelihood contour, evaluates
+ * them with ONE lensed_loglike call and consumes them in order against the rising threshold.
+ *   prior_lo, prior_hi  [P] HOST: uniform priors; lo == hi fixes a parameter (PAPER.md:133 step ii)
+ *   image_plane_sources [n_image_plane] HOST or NULL: model-list indices of source components
+ *                       whose (x, y) prior box is an IMAGE-plane box: every drawn vector goes
+ *                       through lensed_image_plane_prior before its likelihood
+ *   opt                 n_live in [free parameters + 1, 4096]; batch >= 1; tol: stop when
+ *                       max live L * X < tol * Z; enlarge >= 1: linear enlargement of the ellipsoid
+ *                       that bounds the live points; seed of the counter-based generator
+ *   res                 HOST, receives ln Z, its error sqrt(H/n_live), the information H, counts
+ *   samples_dev [capacity][P], logl_dev [capacity], logw_dev [capacity]: device f32 or NULL with
+ *                       capacity 0: the dead points in order of death, then the live points; logw =
+ *                       ln(L w / Z), i.e. posterior weights summing to 1.  Points beyond capacity are
+ *                       dropped (res->n_samples = written, res->n_dead = all deaths before the live set).
+ * Synchronous: returns when the run has converged or max_rounds is reached.  At most 48 free
+ * parameters (LENSED_EUNSUPPORTED beyond).  EINVAL for null pointers, hi < lo, no free parameter,
+ * bad options.  The handle's one-call-at-a-time rule applies for the whole run.               */
+typedef struct {
+    int n_live, batch, max_rounds;
+    double tol, enlarge;
+    unsigned long long seed;
+} lensed_ns_options;
+typedef struct {
+    double ln_z, ln_z_err, information;
+    long long n_rounds, n_likelihood, n_dead, n_samples;
+    int converged;
+} lensed_ns_result;
+lensed_status lensed_ns_run(lensed_handle *h, const float *prior_lo, const float *prior_hi,
+                            const int *image_plane_sources, int n_image_plane,
+                            const lensed_ns_options *opt, lensed_ns_result *res,
+                            float *samples_dev, float *logl_dev, float *logw_dev, long long capacity,
+                            void *cuda_stream);
+/* The sampler's random number generator, Philox4x32-10 (Salmon et al. 2011), for tests:
+ * counter[4], key[2] -> out[4], host arrays.                                                  */
+void lensed_ns_philox(const unsigned *counter, const unsigned *key, unsigned *out);
+
+/*
  * lensed_fma_peak -- FP32 FFMA micro-benchmark used as the measured roofline
  * denominator: runs `iters` dependent-chain FFMAs per thread on a full grid and returns
  * the achieved TFLOP/s (2 flops per FFMA) in *tflops.  Synchronous.                     */

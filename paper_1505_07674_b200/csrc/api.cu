@@ -352,6 +352,19 @@ lensed_status run_host(lensed_handle *h, const float *params_host, int B, float 
 
 }  // namespace
 
+namespace lensed {
+int handle_fail(::lensed_handle *h, int status, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    return fail(h, (lensed_status)status, "%s", buf);
+}
+int handle_device(const ::lensed_handle *h) { return h->device; }
+}  // namespace lensed
+
 extern "C" {
 
 lensed_status lensed_create(int H, int W, double pixel_scale, const float *image, const float *weight,

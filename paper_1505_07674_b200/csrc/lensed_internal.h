@@ -9,6 +9,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+struct lensed_handle;
+
 namespace lensed {
 
 // ---- derived-constant blocks (floats per model, each a multiple of 4 for LDS.128) ------
@@ -168,5 +170,9 @@ size_t trace_smem_bytes(const Program &prog, int nq_pad);
 void conv_tile_shape(int *tile_w, int *tile_h);
 size_t conv_smem_bytes(int KH, int NC, bool render);
 cudaError_t run_fma_peak(int iters, double *tflops);
+
+// for the clients of the handle outside api.cu (nested.cu): error text on the handle, its device
+int handle_fail(::lensed_handle *h, int status, const char *fmt, ...);
+int handle_device(const ::lensed_handle *h);
 
 }  // namespace lensed

@@ -46,6 +46,8 @@ SYMBOLS = {
     "lensed_frame_bytes": (_ll, [_p]),
     "lensed_set_static_tracer": (_i, [_p, _i]),
     "lensed_get_static_tracer": (_i, [_p]),
+    "lensed_ns_run": (_i, [_p, _p, _p, _p, _i, _p, _p, _p, _p, _p, _ll, _p]),
+    "lensed_ns_philox": (None, [_p, _p, _p]),
     "lensed_fma_peak": (_i, [_i, _i, _p]),
     "lensed_last_error": (_c, [_p]),
     "lensed_destroy": (None, [_p]),
@@ -249,6 +251,48 @@ def lensed_set_static_tracer(h, on):
 
 def lensed_get_static_tracer(h):
     return lib().lensed_get_static_tracer(h)
+
+
+class NsOptions(ctypes.Structure):
+    _fields_ = [("n_live", _i), ("batch", _i), ("max_rounds", _i), ("tol", _d), ("enlarge", _d),
+                ("seed", ctypes.c_ulonglong)]
+
+
+class NsResult(ctypes.Structure):
+    _fields_ = [("ln_z", _d), ("ln_z_err", _d), ("information", _d), ("n_rounds", _ll), ("n_likelihood", _ll),
+                ("n_dead", _ll), ("n_samples", _ll), ("converged", _i)]
+
+
+def lensed_ns_run(h, prior_lo, prior_hi, n_live=400, batch=256, tol=1e-3, enlarge=1.2, seed=1, max_rounds=100000,
+                  image_plane_sources=None, samples_dev=None, logl_dev=None, logw_dev=None, stream=None):
+    """-> dict of the lensed_ns_result fields.  prior_lo / prior_hi: host arrays [P]; the three
+    output tensors (float32 CUDA, [cap][P], [cap], [cap]) are optional."""
+    lo, hi = _np(prior_lo, np.float32), _np(prior_hi, np.float32)
+    P = lensed_num_params(h)
+    if lo.shape != (P,) or hi.shape != (P,):
+        raise LensedError(EINVAL, "priors must be [%d]" % P)
+    ip = None if image_plane_sources is None else _np(image_plane_sources, np.int32).reshape(-1)
+    cap = 0
+    if samples_dev is not None:
+        cap = int(samples_dev.shape[0])
+        _check_out(samples_dev, cap, cap * P)
+        _check_out(logl_dev, cap, cap)
+        _check_out(logw_dev, cap, cap)
+    opt = NsOptions(int(n_live), int(batch), int(max_rounds), float(tol), float(enlarge), int(seed))
+    res = NsResult()
+    ptr = lambda t: None if t is None else ctypes.c_void_p(t.data_ptr())
+    _check(lib().lensed_ns_run(h, _hp(lo), _hp(hi), _hp(ip), 0 if ip is None else len(ip), ctypes.byref(opt),
+                               ctypes.byref(res), ptr(samples_dev), ptr(logl_dev), ptr(logw_dev), cap,
+                               _stream(stream)), h)
+    return {k: getattr(res, k) for k, _ in NsResult._fields_}
+
+
+def lensed_ns_philox(counter, key):
+    c = (ctypes.c_uint * 4)(*[int(x) for x in counter])
+    k = (ctypes.c_uint * 2)(*[int(x) for x in key])
+    out = (ctypes.c_uint * 4)()
+    lib().lensed_ns_philox(c, k, out)
+    return [int(x) for x in out]
 
 
 def lensed_fma_peak(device=0, iters=4096):

@@ -1,0 +1,177 @@
+"""The device-resident nested-sampling driver (lensed_ns_run, csrc/nested.cu) against the CPU
+oracle driver (oracle/nested_oracle.py) running the oracle likelihood: the same counter-based
+random numbers on both sides, so short runs agree point by point and full runs agree in ln Z and
+in the posterior within the sampler's own statistical error."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import lensed_oracle as orc
+from oracle import nested_oracle as ns
+from paper_1505_07674_b200 import synth
+from tests.cases import Problem
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def L():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1505_07674_b200 import lensed
+    lensed.lib()
+    return lensed
+
+
+def _tiny_priors(cfg):
+    """BASELINE.json `tiny`: +-20 % of the truth, zero-valued positions +-0.02", q and PA fixed"""
+    t = cfg.truth
+    lo, hi = t.copy(), t.copy()
+    for c, v in enumerate(t):
+        if c in (7, 8):
+            continue
+        if c in (0, 1, 3, 4):
+            lo[c], hi[c] = v - 0.02, v + 0.02
+        else:
+            lo[c], hi[c] = sorted((0.8 * v, 1.2 * v))
+    return lo.astype(np.float32), hi.astype(np.float32)
+
+
+def _gpu_run(L, prob, lo, hi, cap, **kw):
+    import torch
+    P = len(lo)
+    samples = torch.zeros((cap, P), dtype=torch.float32, device="cuda")
+    logl = torch.zeros(cap, dtype=torch.float32, device="cuda")
+    logw = torch.zeros(cap, dtype=torch.float32, device="cuda")
+    h = prob.create()
+    try:
+        res = L.lensed_ns_run(h, lo, hi, samples_dev=samples, logl_dev=logl, logw_dev=logw, **kw)
+    finally:
+        L.lensed_destroy(h)
+    n = res["n_samples"]
+    res.update(samples=samples[:n].cpu().numpy(), logl=logl[:n].cpu().numpy().astype(np.float64),
+               logw=logw[:n].cpu().numpy().astype(np.float64))
+    return res
+
+
+def _moments(res):
+    w = np.exp(res["logw"] - res["logw"].max())
+    w /= w.sum()
+    mean = (w[:, None] * res["samples"]).sum(axis=0)
+    return mean, np.sqrt((w[:, None] * (res["samples"] - mean) ** 2).sum(axis=0))
+
+
+def test_generator_known_answers_on_the_library_side(L):
+    for line in open(__file__.replace("test_nested_gpu.py", "golden/philox_kat.txt")):
+        if line.strip() and not line.startswith("#"):
+            v = [int(x, 16) for x in line.split()]
+            assert L.lensed_ns_philox(v[:4], v[4:6]) == v[6:]
+
+
+def test_three_rounds_agree_point_by_point_with_the_oracle_driver(L):
+    """Same seed, same options, three rounds: initial draw, bound, proposals, prior transform,
+    acceptance against the rising threshold, weights and the final live-point step must give the
+    same set of points with the same weights (float32 parameter vectors: exactly)."""
+    cfg = synth.get_config(0)
+    prob = Problem(cfg)
+    lo, hi = _tiny_priors(cfg)
+    kw = dict(n_live=64, batch=48, tol=1e-9, enlarge=1.25, seed=2024, max_rounds=3)
+    ref = ns.run(lambda t: prob.oracle_loglike(t.astype(np.float32), want_model=False), lo, hi, **kw)
+    # the driver checks convergence every 4 rounds: ask for 4 and compare with 4 oracle rounds
+    kw4 = dict(kw, max_rounds=4)
+    ref = ns.run(lambda t: prob.oracle_loglike(t.astype(np.float32), want_model=False), lo, hi, **kw4)
+    got = _gpu_run(L, prob, lo, hi, 4096, **kw4)
+    assert got["n_rounds"] == 4 and ref["n_rounds"] == 4 and not got["converged"]
+    assert got["n_dead"] == ref["n_dead"] and got["n_samples"] == len(ref["logl"])
+    nd = ref["n_dead"]
+    assert np.array_equal(got["samples"][:nd], ref["samples"][:nd].astype(np.float32))       # deaths, in order
+    key = lambda a: a[np.lexsort(a.T[::-1])]
+    assert np.array_equal(key(got["samples"][nd:]), key(ref["samples"][nd:].astype(np.float32)))   # live set
+    assert np.allclose(got["logl"][:nd], ref["logl"][:nd], rtol=1e-5)
+    assert got["ln_z"] == pytest.approx(ref["ln_z"], rel=1e-5)
+    assert got["information"] == pytest.approx(ref["information"], rel=1e-3, abs=1e-3)
+    assert np.exp(got["logw"]).sum() == pytest.approx(1.0, rel=1e-4)
+
+
+def test_tiny_config_evidence_and_posterior_match_the_oracle_driver_and_recover_the_truth(L):
+    cfg = synth.get_config(0)
+    prob = Problem(cfg)
+    lo, hi = _tiny_priors(cfg)
+    kw = dict(n_live=300, batch=256, tol=1e-3, enlarge=1.2, seed=7)
+    got = _gpu_run(L, prob, lo, hi, 60000, **kw)
+    ref = ns.run(lambda t: prob.oracle_loglike(t.astype(np.float32), want_model=False), lo, hi, **kw)
+    assert got["converged"] and ref["converged"]
+    err = math.hypot(got["ln_z_err"], ref["ln_z_err"])
+    assert abs(got["ln_z"] - ref["ln_z"]) < 3.0 * err, (got["ln_z"], ref["ln_z"], err)
+    assert got["information"] == pytest.approx(ref["information"], rel=0.1)
+    assert got["ln_z_err"] == pytest.approx(math.sqrt(got["information"] / 300), rel=1e-9)
+    mg, sg = _moments(got)
+    mr, sr = ns.posterior_moments(ref)
+    free = np.flatnonzero(hi > lo)
+    assert np.all(np.abs(mg[free] - mr[free]) < 0.5 * sr[free])            # same posterior ...
+    assert np.all(np.abs(sg[free] / sr[free] - 1.0) < 0.35)
+    assert np.all(np.abs(mg[free] - cfg.truth[free]) < 4.0 * sr[free])      # ... that holds the truth
+    assert np.all(sg[[7, 8]] < 1e-12)                                        # fixed parameters stay fixed
+    assert got["n_likelihood"] >= 300 + got["n_rounds"] * 256
+    assert np.all(np.diff(got["logl"][:got["n_dead"]]) >= 0)               # deaths in order of likelihood
+
+
+def test_shrunk_hst_case_with_an_image_plane_prior(L):
+    """SIE + shear + Sersic source + lens light + sky on a 40 x 36 image; six free parameters with
+    priors a few posterior widths around the truth, the source position drawn in the IMAGE plane
+    around one of its images and mapped through each vector's own lens."""
+    cfg = synth.shrunk(synth.get_config(1), 40, 36, 4)
+    prob = Problem(cfg)
+    t = cfg.truth.astype(np.float64)
+    # image-plane position of the source's brightest image under the true lens
+    _, model = prob.oracle_loglike(t.astype(np.float32)[None], want_model=True)
+    fg = orc.render(cfg.H, cfg.W, cfg.scale, cfg.psf, cfg.quad, synth.kind_ids(("fg_sersic", "sky")), t[14:].astype(np.float32))[0]
+    i, j = np.unravel_index(np.argmax(model[0] - fg), fg.shape)
+    img = np.array([(j - (cfg.W - 1) / 2) * cfg.scale, (i - (cfg.H - 1) / 2) * cfg.scale])
+    lo, hi = t.copy(), t.copy()
+    lo[2], hi[2] = t[2] - 0.03, t[2] + 0.03                 # Einstein radius
+    lo[3], hi[3] = t[3] - 0.05, t[3] + 0.05                 # axis ratio
+    lo[7:9], hi[7:9] = img - 0.06, img + 0.06               # source (x, y): an IMAGE-plane box
+    lo[9], hi[9] = 0.8 * t[9], 1.25 * t[9]                  # source radius
+    lo[10], hi[10] = t[10] - 0.3, t[10] + 0.3               # source magnitude
+    lo, hi = lo.astype(np.float32), hi.astype(np.float32)
+    src = [2]                                               # index of src_sersic in the model list
+    kw = dict(n_live=200, batch=256, tol=1e-2, enlarge=1.3, seed=11)
+
+    def transform(theta):
+        out = theta.copy()
+        for b in range(len(out)):
+            out[b, 7:9] = orc.source_position(prob.kinds, theta[b], theta[b, 7:9][None])[0]
+        return out.astype(np.float32).astype(np.float64)
+
+    got = _gpu_run(L, prob, lo, hi, 40000, image_plane_sources=src, **kw)
+    ref = ns.run(lambda th: prob.oracle_loglike(th.astype(np.float32), want_model=False), lo, hi, transform=transform, **kw)
+    assert got["converged"] and ref["converged"]
+    err = math.hypot(got["ln_z_err"], ref["ln_z_err"])
+    assert abs(got["ln_z"] - ref["ln_z"]) < 3.0 * err, (got["ln_z"], ref["ln_z"], err)
+    mg, sg = _moments(got)
+    mr, sr = ns.posterior_moments(ref)
+    for c in (2, 3, 7, 8, 9, 10):
+        assert abs(mg[c] - mr[c]) < 0.6 * sr[c], (c, mg[c], mr[c], sr[c])
+    # the samples hold SOURCE-plane positions (after the map): near the true source position
+    assert abs(mg[7] - t[7]) < 5 * sr[7] + 0.01 and abs(mg[8] - t[8]) < 5 * sr[8] + 0.01
+
+
+def test_bad_arguments_are_rejected(L):
+    cfg = synth.get_config(0)
+    lo, hi = _tiny_priors(cfg)
+    h = Problem(cfg).create()
+    try:
+        for kw, status in ((dict(n_live=4), L.EINVAL), (dict(n_live=5000), L.EINVAL), (dict(batch=0), L.EINVAL),
+                           (dict(tol=0.0), L.EINVAL), (dict(enlarge=0.5), L.EINVAL),
+                           (dict(image_plane_sources=[0]), L.EINVAL)):          # model 0 is the lens
+            with pytest.raises(L.LensedError) as e:
+                L.lensed_ns_run(h, lo, hi, **dict(dict(n_live=32, batch=8, max_rounds=2), **kw))
+            assert e.value.status == status, kw
+        with pytest.raises(L.LensedError):
+            L.lensed_ns_run(h, hi, lo)                                          # hi < lo
+        with pytest.raises(L.LensedError):
+            L.lensed_ns_run(h, lo, lo)                                          # nothing free
+    finally:
+        L.lensed_destroy(h)
