@@ -182,6 +182,8 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="vectors per GPU per step (0 = the config's)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the batch sweep of the Euclid config")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--conv-shape", default="auto", choices=("auto", "wide", "narrow"),
+                    help="convolution block shape (include/lensed.h); auto = what lensed_create picks")
     ap.add_argument("--interpreter", action="store_true",
                     help="run the interpreting tracer instead of the compile-time specialised one")
     args = ap.parse_args()
@@ -209,7 +211,10 @@ def main():
     h = lensed.lensed_create(image, weight, cfg.mask, cfg.psf, cfg.quad, kinds, cfg.scale, cfg.zp, local)
     if args.interpreter:
         lensed.lensed_set_static_tracer(h, 0)
+    if args.conv_shape != "auto":
+        lensed.lensed_set_conv_shape(h, args.conv_shape == "wide")
     tracer_kind = "static" if lensed.lensed_get_static_tracer(h) == 1 else "interpreter"
+    conv_shape = "wide" if lensed.lensed_get_conv_shape(h) else "narrow"
     n_traced = cfg.n_traced()                               # m_d, the required set
     assert n_traced <= lensed.lensed_num_traced(h)
     n_counted = int(cfg.H * cfg.W if cfg.mask is None else cfg.mask.sum())
@@ -330,7 +335,7 @@ def main():
             "config": {"workload": workload_name(cfg, B), "batch_per_gpu": B, "global_batch": B * world,
                        "traced_pixels": n_traced, "rays_per_step": B * world * n_traced * len(cfg.quad),
                        "parallelism": "batch-sharded x%d, no collective" % world,
-                       "tracer": tracer_kind,
+                       "tracer": tracer_kind, "conv_shape": conv_shape,
                        "timing": "CUDA events per step, L2 flushed (256 MB write) between steps, max over ranks"},
             "rays_per_sec": rays_per_s,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(params.nbytes),

@@ -88,10 +88,7 @@ typedef enum {
  *   out         receives the handle (NULL on failure)
  * Errors: EINVAL for null pointers, non-positive sizes, negative or non-finite weights,
  * non-finite image values at unmasked pixels, bad PSF / rule / kind; ECUDA if there is
- * no usable device; ENOMEM also when the on-chip tap pool is full: the PSFs of the live
- * handles of a device share 60 KB of constant memory, (psf_h + 1) * 4 ceil(psf_w / 4) * 8
- * bytes each (8 KB for 31 x 31, 32 KB for 63 x 63), released by lensed_destroy.
- * Synchronous.                                                                          */
+ * no usable device; ENOMEM for a failed allocation.  Synchronous.                       */
 lensed_status lensed_create(int H, int W, double pixel_scale,
                             const float *image, const float *weight,
                             const unsigned char *mask,
@@ -204,6 +201,25 @@ lensed_status lensed_get_refined(lensed_handle *h, long long *pixels);
  * lensed_frame_bytes: -1 for NULL.                                                      */
 lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes);
 long long lensed_frame_bytes(const lensed_handle *h);
+
+/* Convolution block shape.  The convolution exists in two shapes (same arithmetic): "wide",
+ * 256 threads on 64 x 128 output tiles, one block per SM, and "narrow", 128 threads on 64 x 64
+ * tiles, two blocks per SM (small or masked images, small PSFs).  lensed_create picks one;
+ * lensed_set_conv_shape(h, 1 / 0) forces wide / narrow (it rebuilds the tile lists and the frame
+ * layout and synchronises the device; LENSED_EUNSUPPORTED if the PSF is too large for the narrow
+ * shape's shared memory).  lensed_get_conv_shape: 1 / 0, -1 for NULL.  Results do not depend on
+ * the shape beyond the order of the per-tile chi-square partials.
+ *
+ * PSF taps.  The taps of a handle normally sit in a 60 KB pool of constant memory shared by
+ * the live handles of a device ((psf_h + 1) * 4 ceil(psf_w / 4) * 8 bytes each: 8 KB for 31 x 31,
+ * 32 KB for 63 x 63).  A handle created when the pool is full keeps its taps in global memory
+ * and runs a variant of the convolution that reads them from there (same results, somewhat
+ * slower); lensed_uses_global_taps tells (1 / 0, -1 for NULL).
+ * lensed_debug_force_global_taps(1) makes every later lensed_create take that path (tests).   */
+lensed_status lensed_set_conv_shape(lensed_handle *h, int wide);
+int lensed_get_conv_shape(const lensed_handle *h);
+int lensed_uses_global_taps(const lensed_handle *h);
+void lensed_debug_force_global_taps(int on);
 
 /* Tracer selection.  The ray tracer exists as one kernel that interprets any model list
  * and as kernels specialised at compile time for eight model lists (same arithmetic,

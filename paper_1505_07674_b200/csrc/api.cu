@@ -42,6 +42,9 @@ struct lensed_handle {
     int ox_ll = 0, oy_ll = 0;       // origin of the loglike tile grid (render tiles start at 0, 0)
     int n_sm = 1;
     int tap_off = -1, tap_pairs = 0; // this handle's range of the constant tap pool
+    unsigned long long *d_gtaps = nullptr;   // the taps in global memory instead, when the pool was full
+    bool wide = true;               // convolution block shape (conv.cu "Two block shapes")
+    std::vector<uint8_t> counted;   // host copy of the counted-pixel map (lensed_set_conv_shape rebuilds the tiles)
 
     // device, immutable after create
     float *d_image = nullptr, *d_wmask = nullptr;
@@ -58,6 +61,7 @@ struct lensed_handle {
     unsigned long long *d_refined = nullptr;   // pixels refined in FP64 since the last profile reset
     double refine_gain = 1.0;                  // lensed_set_refine
     float *d_L = nullptr; size_t cap_L = 0;
+    alignas(64) unsigned char tmap_L[128] = {};    // CUtensorMap of d_L for the convolution's tile loads (conv.cu)
     double *d_partial = nullptr; size_t cap_partial = 0;
     float *d_stage_in = nullptr; size_t cap_stage_in = 0;
     float *d_stage_out = nullptr; size_t cap_stage_out = 0;
@@ -223,6 +227,66 @@ lensed_status collect_profile(lensed_handle *h)
     return LENSED_OK;
 }
 
+bool g_force_global_taps = false;     // lensed_debug_force_global_taps (tests)
+
+// Tile lists and padded frame for one block shape of the convolution; frees the frame buffer
+// (its layout changes).  Loglike tiles start at the corner of the counted pixels' bounding box
+// (x rounded down to a 16-byte boundary for cp.async): a mask that is not tile-aligned costs
+// fewer tiles.  The render grid starts at (0, 0).
+lensed_status build_tiles(lensed_handle *h, bool wide)
+{
+    const int H = h->H, W = h->W;
+    h->wide = wide;
+    conv_tile_shape(wide, &h->tile_w, &h->tile_h);
+    std::vector<uint8_t> all((size_t)H * W, 1);
+    std::vector<uint32_t> tiles_ll, tiles_all;
+    int x0 = W, y0 = H;
+    for (int i = 0; i < H; ++i)
+        for (int j = 0; j < W; ++j)
+            if (h->counted[(size_t)i * W + j]) { x0 = std::min(x0, j); y0 = std::min(y0, i); }
+    h->ox_ll = x0 < W ? x0 / 4 * 4 : 0;
+    h->oy_ll = y0 < H ? y0 : 0;
+    int ny_ll, nx_ll, ny_all, nx_all;
+    tile_list(h->counted, H, W, h->tile_w, h->tile_h, h->ox_ll, h->oy_ll, tiles_ll, &ny_ll, &nx_ll);
+    tile_list(all, H, W, h->tile_w, h->tile_h, 0, 0, tiles_all, &ny_all, &nx_all);
+    // padded frame: the image, and every tile of either grid with its PSF halo
+    const int rows = std::max(std::max(ny_all * h->tile_h, h->oy_ll + ny_ll * h->tile_h), H);
+    const int cols = std::max(std::max(nx_all * h->tile_w, h->ox_ll + nx_ll * h->tile_w), W);
+    conv_padded_shape(rows, cols, h->KH, h->NC, &h->Hp, &h->Wp);
+    h->ntiles_ll = (int)tiles_ll.size(); h->ntiles_all = (int)tiles_all.size();
+    CU(h, cudaSetDevice(h->device));
+    CU(h, cudaDeviceSynchronize());
+    cudaFree(h->d_tiles_ll); cudaFree(h->d_tiles_all); cudaFree(h->d_L);
+    h->d_tiles_ll = h->d_tiles_all = nullptr; h->d_L = nullptr; h->cap_L = 0;
+    lensed_status s;
+    if ((s = upload(h, &h->d_tiles_ll, tiles_ll.data(), tiles_ll.size())) != LENSED_OK) return s;
+    return upload(h, &h->d_tiles_all, tiles_all.data(), tiles_all.size());
+}
+
+// Block shape lensed_create picks.  Measured on the configs (profiles/r2b.md): with full tiles
+// the wide shape is as fast (small PSFs) or faster (31 x 31: 32.9 against 35.7 ms per 4096
+// Euclid vectors); the narrow one wins where its 64-column tiles cover a masked image with
+// fewer pixels (SLACS annulus: 9 x 4096 against 6 x 8192 pixels per vector, 2.58 -> 2.21 ms).
+bool default_wide(const lensed_handle *h)
+{
+#ifdef LENSED_CONV_FORCE_WIDE
+    return LENSED_CONV_FORCE_WIDE != 0;
+#endif
+    if (!conv_narrow_fits(h->KH, h->NC)) return true;
+    long long px[2];
+    for (int wide = 0; wide < 2; ++wide) {
+        int tw, th, ny, nx, x0 = h->W, y0 = h->H;
+        conv_tile_shape(wide != 0, &tw, &th);
+        for (int i = 0; i < h->H; ++i)
+            for (int j = 0; j < h->W; ++j)
+                if (h->counted[(size_t)i * h->W + j]) { x0 = std::min(x0, j); y0 = std::min(y0, i); }
+        std::vector<uint32_t> tiles;
+        tile_list(h->counted, h->H, h->W, tw, th, x0 < h->W ? x0 / 4 * 4 : 0, y0 < h->H ? y0 : 0, tiles, &ny, &nx);
+        px[wide] = (long long)tiles.size() * tw * th;
+    }
+    return !(px[0] * 100 <= px[1] * 85);
+}
+
 // Pixels of the traced list one tracer block walks: it amortises its prologue (constants +
 // frame tables) over them.  Measured per config (ms per step at 512 / 1024 / 2048 / 4096 / 8192
 // pixels): HST 0.296 / 0.273 / 0.264 / 0.269 / 0.288, SLACS 4.55 / 4.34 / 4.23 / 4.15 / 4.13,
@@ -260,6 +324,7 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
         // pad cells no pixel clamps to (tile overhang) are read, never written: keep them zero
         if ((s = grow(h, &h->d_L, &h->cap_L, (size_t)Bc * HWp, st)) != LENSED_OK) return s;
         CU(h, cudaMemsetAsync(h->d_L, 0, (size_t)Bc * HWp * sizeof(float), st));
+        CU(h, conv_make_tensor_map(h->tmap_L, h->d_L, h->Wp, h->Hp, Bc, h->KH, h->NC, h->wide));
     }
     if (!render && (s = grow(h, &h->d_partial, &h->cap_partial, (size_t)B * std::max(n_tiles, 1), st)) != LENSED_OK)
         return s;
@@ -315,10 +380,11 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
             ca.lp_stride = (long long)HWp;
             ca.D = prog.D;
             ca.H = h->H; ca.W = h->W; ca.Wp = h->Wp; ca.KH = h->KH; ca.KW = h->KW; ca.NC = h->NC;
-            ca.n_tiles = n_tiles; ca.nb = nb; ca.tap_off = h->tap_off;
+            ca.n_tiles = n_tiles; ca.nb = nb;
+            ca.tap_off = h->d_gtaps ? 0 : h->tap_off; ca.gtaps = h->d_gtaps; ca.wide = h->wide ? 1 : 0;
             ca.ox = render ? 0 : h->ox_ll; ca.oy = render ? 0 : h->oy_ll;
             if ((s = timed_begin(h, PH_CONV, st)) != LENSED_OK) return s;
-            CU(h, launch_conv(ca, render, h->n_sm, st));
+            CU(h, launch_conv(ca, h->tmap_L, render, h->n_sm, st));
             if ((s = timed_end(h, st)) != LENSED_OK) return s;
         }
     }
@@ -489,32 +555,14 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
             if (j > 0) pair[1] = G[(size_t)(j - 1) * h->KW + kx];
         }
 
-    // pixel lists and tile lists
-    conv_tile_shape(&h->tile_w, &h->tile_h);
-    std::vector<uint32_t> pix_ll, pix_all, tiles_ll, tiles_all;
+    // pixel lists; the tile lists and the padded frame follow the convolution's block shape
+    std::vector<uint32_t> pix_ll, pix_all;
     // traced set: the PSF windows of the counted pixels, one more row each way because a
     // counted row's pair partner multiplies its first / last window row by a zero tap
     pixel_list(dilate(counted, H, W, (h->KH - 1) / 2 + 1, (h->KW - 1) / 2), H, W, pix_ll);
     pixel_list(all, H, W, pix_all);
-    // loglike tiles start at the corner of the counted pixels' bounding box (x rounded down to
-    // a 16-byte boundary for cp.async): a mask that is not tile-aligned costs fewer tiles
-    {
-        int x0 = W, y0 = H;
-        for (int i = 0; i < H; ++i)
-            for (int j = 0; j < W; ++j)
-                if (counted[(size_t)i * W + j]) { x0 = std::min(x0, j); y0 = std::min(y0, i); }
-        h->ox_ll = x0 < W ? x0 / 4 * 4 : 0;
-        h->oy_ll = y0 < H ? y0 : 0;
-        int ny_ll, nx_ll, ny_all, nx_all;
-        tile_list(counted, H, W, h->tile_w, h->tile_h, h->ox_ll, h->oy_ll, tiles_ll, &ny_ll, &nx_ll);
-        tile_list(all, H, W, h->tile_w, h->tile_h, 0, 0, tiles_all, &ny_all, &nx_all);
-        // padded frame: the image, and every tile of either grid with its PSF halo
-        const int rows = std::max(std::max(ny_all * h->tile_h, h->oy_ll + ny_ll * h->tile_h), H);
-        const int cols = std::max(std::max(nx_all * h->tile_w, h->ox_ll + nx_ll * h->tile_w), W);
-        conv_padded_shape(rows, cols, h->KH, h->NC, &h->Hp, &h->Wp);
-    }
+    h->counted = counted;
     h->npix_ll = (int)pix_ll.size(); h->npix_all = (int)pix_all.size();
-    h->ntiles_ll = (int)tiles_ll.size(); h->ntiles_all = (int)tiles_all.size();
 
     int ndev = 0;
     cudaError_t ce = cudaGetDeviceCount(&ndev);
@@ -544,14 +592,15 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     {
         // tap pairs into this handle's range of the constant pool (conv.cu "Taps")
         h->tap_pairs = (int)(taps.size() / 2);
-        h->tap_off = g_tap_pool.take(device, h->tap_pairs);
+        h->tap_off = g_force_global_taps ? -1 : g_tap_pool.take(device, h->tap_pairs);
         if (h->tap_off < 0) {
-            lensed_destroy(h);
-            return fail(nullptr, LENSED_ENOMEM, "constant tap pool full: %d pairs wanted, pool of %d shared by the live handles",
-                        (int)(taps.size() / 2), kTapPoolPairs);
+            // pool full: this handle's convolution reads its taps from global memory instead
+            // (conv.cu GT: same values, LDG through L1 instead of the uniform datapath)
+            CREATE_FAIL(upload(h, &h->d_gtaps, reinterpret_cast<const unsigned long long *>(taps.data()), (size_t)h->tap_pairs));
+        } else {
+            cudaError_t e2 = conv_upload_taps(taps.data(), h->tap_pairs, h->tap_off);
+            if (e2 != cudaSuccess) { lensed_destroy(h); return fail(nullptr, LENSED_ECUDA, "tap upload: %s", cudaGetErrorString(e2)); }
         }
-        cudaError_t e2 = conv_upload_taps(taps.data(), h->tap_pairs, h->tap_off);
-        if (e2 != cudaSuccess) { lensed_destroy(h); return fail(nullptr, LENSED_ECUDA, "tap upload: %s", cudaGetErrorString(e2)); }
     }
     CREATE_FAIL(upload(h, &h->d_quad, hq.data(), hq.size()));
     {
@@ -563,8 +612,7 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     h->h_quad = hq;
     CREATE_FAIL(upload(h, &h->d_pix_ll, pix_ll.data(), pix_ll.size()));
     CREATE_FAIL(upload(h, &h->d_pix_all, pix_all.data(), pix_all.size()));
-    CREATE_FAIL(upload(h, &h->d_tiles_ll, tiles_ll.data(), tiles_ll.size()));
-    CREATE_FAIL(upload(h, &h->d_tiles_all, tiles_all.data(), tiles_all.size()));
+    CREATE_FAIL(build_tiles(h, default_wide(h)));
 #undef CREATE_FAIL
     *out = h;
     return LENSED_OK;
@@ -768,6 +816,20 @@ lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes)
     return LENSED_OK;
 }
 
+lensed_status lensed_set_conv_shape(lensed_handle *h, int wide)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (!wide && !conv_narrow_fits(h->KH, h->NC))
+        return fail(h, LENSED_EUNSUPPORTED, "a %d x %d PSF does not fit the narrow block shape", h->KH, h->KW);
+    return build_tiles(h, wide != 0);
+}
+
+int lensed_get_conv_shape(const lensed_handle *h) { return h ? (h->wide ? 1 : 0) : -1; }
+
+void lensed_debug_force_global_taps(int on) { g_force_global_taps = on != 0; }
+
+int lensed_uses_global_taps(const lensed_handle *h) { return h ? (h->d_gtaps ? 1 : 0) : -1; }
+
 lensed_status lensed_set_static_tracer(lensed_handle *h, int on)
 {
     if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
@@ -807,7 +869,7 @@ void lensed_destroy(lensed_handle *h)
     cudaFree(h->d_pix_ll); cudaFree(h->d_pix_all); cudaFree(h->d_tiles_ll); cudaFree(h->d_tiles_all);
     cudaFree(h->d_derived); cudaFree(h->d_L); cudaFree(h->d_partial);
     cudaFree(h->d_derived64); cudaFree(h->d_fixmask); cudaFree(h->d_refined);
-    cudaFree(h->d_queue); cudaFree(h->d_queue_count);
+    cudaFree(h->d_queue); cudaFree(h->d_queue_count); cudaFree(h->d_gtaps);
     cudaFree(h->d_stage_in); cudaFree(h->d_stage_out);
     delete h;
 }

@@ -15,12 +15,17 @@
 // are dropped.  The loglike tile grid starts at the corner of the counted pixels' bounding
 // box (a.ox, a.oy), the render grid at (0, 0).
 //
-// Work.  One persistent block of 256 threads per SM.  A work item is (output tile of 64 x 128
-// pixels, parameter vector); items are ordered tile-major and split evenly over the blocks,
-// so a block stays on one tile position for many vectors: the tile's data d and weights w
-// are staged in shared memory once per position.  The input tile (64 + KH - 1 rows of
-// 128 + 4 NC floats) comes in with cp.async, double buffered: item i+1 loads while item i is
-// convolved (single buffer when two do not fit: PSFs beyond ~45 x 45).
+// Work.  Persistent blocks: one of 256 threads per SM ("wide", 64 x 128 output tiles) or two of
+// 128 threads ("narrow", 64 x 64 tiles; see Shape below).  A work item is (output tile,
+// parameter vector); items are ordered tile-major and split evenly over the blocks, so a block
+// stays on one tile position for many vectors: the tile's data d and weights w are staged in
+// shared memory once per position.  The input tile with its halo (64 + KH - 1 rows of
+// tile width + 4 NC floats) is a plain box of the padded frame: ONE thread moves it with one TMA
+// tensor copy (cp.async.bulk.tensor.3d over (x, y, vector), completion on an mbarrier), double
+// buffered: item i+1 loads while item i is convolved (single buffer when two do not fit: PSFs
+// beyond ~45 x 45).  Against 256 threads x cp.async 16 B with an integer divide per element
+// (LENSED_CONV_TMA=0) the tensor copy is worth 0.8 % at 31 x 31 and 5-9 % at 9 x 9 ... 21 x 21
+// (profiles/r2b.md).
 //
 // Thread tile: 4 rows x 8 columns of outputs (two 4-column groups 64 columns apart, so that
 // the 8 lanes of a quarter-warp read consecutive 16-byte words: conflict-free LDS.128).
@@ -55,6 +60,13 @@
 #include "lensed_internal.h"
 #include "f32x2.cuh"
 #include <math.h>
+#include <cuda.h>                 // CUtensorMap (types only; the encoder is fetched from the driver at run time)
+#include <cudaTypedefs.h>
+#include <algorithm>
+
+#ifndef LENSED_CONV_TMA
+#define LENSED_CONV_TMA 1         // input tiles by one cp.async.bulk.tensor per tile (0: cp.async per 16 bytes)
+#endif
 
 namespace lensed {
 
@@ -64,15 +76,26 @@ __constant__ unsigned long long c_taps[kTapPoolPairs];
 namespace {
 
 constexpr int kTR = 4;                 // output rows per thread (two pairs)
-constexpr int kNTX = 16, kNTY = 16;    // threads per block in x / y (warps are 8 x 4 threads)
-constexpr int kThreads = kNTX * kNTY;
-constexpr int kGroup = 4 * kNTX;       // 64: distance of a thread's two column groups
-constexpr int kTW = 2 * kGroup;        // 128 output columns per tile
+constexpr int kNTY = 16;               // threads per block in y (warps are 8 x 4 threads)
 constexpr int kTH = kTR * kNTY;        // 64 output rows per tile
 constexpr int kSlackRows = 2;          // rows past a staged tile the last loop body loads but never uses
 
+// Two block shapes (api.cu picks one per handle, ConvArgs::wide):
+//   wide   NTX = 16: 256 threads, 64 x 128 tile, one block per SM   -- large images, large PSFs
+//   narrow NTX =  8: 128 threads, 64 x 64 tile, two blocks per SM   -- small or masked images and
+//          small PSFs, where a tile's prologue (staging, barriers) and epilogue (reduction) are
+//          not small against its inner loop: the second block's inner loop hides them, and the
+//          64-column tiles waste less of a masked or small image.
+template <int NTX>
+struct Shape {
+    static constexpr int kThreads = NTX * kNTY;
+    static constexpr int kGroup = 4 * NTX;      // distance of a thread's two column groups
+    static constexpr int kTW = 2 * kGroup;      // output columns per tile
+};
+
 __device__ __forceinline__ f2 as_f2(unsigned long long v) { f2 r; r.v = v; return r; }
 
+#if !LENSED_CONV_TMA
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
 {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -81,22 +104,53 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+#endif
+
+// ---- TMA: one elected thread moves the whole (64 + KH - 1) x (tile width + 4 NC) box of the padded
+// frame with a single 3-D tensor copy (x, y, vector) that completes on an mbarrier.
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    const unsigned b = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile(
+        "{\n.reg .pred p;\nWAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(b), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void *smem, const CUtensorMap *map, unsigned long long *bar, int x, int y, int z)
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // earlier generic reads of this stage are done
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+                 ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(map), "r"((unsigned)__cvta_generic_to_shared(bar)),
+                   "r"(x), "r"(y), "r"(z) : "memory");
+}
 
 // The 16 input floats a thread needs from one staged row for one 4-tap chunk: columns
 // 4 tx + 4 c .. + 7 of both column groups.
 struct InRow { float4 a0, a1, b0, b1; };
 
+template <int NTX>
 __device__ __forceinline__ void load_row(InRow &x, const float4 *p)
 {
-    x.a0 = p[0]; x.a1 = p[1]; x.b0 = p[kGroup / 4]; x.b1 = p[kGroup / 4 + 1];
+    x.a0 = p[0]; x.a1 = p[1]; x.b0 = p[NTX]; x.b1 = p[NTX + 1];
 }
 
 // One step j of a 4-tap chunk: both row pairs against the SAME tap pairs Q[j][c][0..3]
 // (iq = their index in c_taps).  Pair 0 (output rows 0-1) takes input row j of the strip
 // (x0), pair 1 (rows 2-3) takes input row j + 2 (x1).  NT = taps of the chunk (4, or the
 // 1-3 of the last chunk when KW is not a multiple of 4: no multiply by a padded zero column).
-template <int NT>
-__device__ __forceinline__ void tap_step(f2 (&part)[2][8], const InRow &x0, const InRow &x1, int iq)
+// GT: the tap pairs come from global memory (gt) instead of the constant pool: the fallback
+// for handles that found the pool full (api.cu); same values, LDG through L1 instead of LDCU.
+template <int NT, bool GT>
+__device__ __forceinline__ void tap_step(f2 (&part)[2][8], const InRow &x0, const InRow &x1, int iq,
+                                         const unsigned long long *gt)
 {
     const float va0[8] = {x0.a0.x, x0.a0.y, x0.a0.z, x0.a0.w, x0.a1.x, x0.a1.y, x0.a1.z, x0.a1.w};
     const float vb0[8] = {x0.b0.x, x0.b0.y, x0.b0.z, x0.b0.w, x0.b1.x, x0.b1.y, x0.b1.z, x0.b1.w};
@@ -104,7 +158,7 @@ __device__ __forceinline__ void tap_step(f2 (&part)[2][8], const InRow &x0, cons
     const float vb1[8] = {x1.b0.x, x1.b0.y, x1.b0.z, x1.b0.w, x1.b1.x, x1.b1.y, x1.b1.z, x1.b1.w};
 #pragma unroll
     for (int k = 0; k < NT; ++k) {
-        const f2 q = as_f2(c_taps[iq + k]);
+        const f2 q = as_f2(GT ? __ldg(gt + iq + k) : c_taps[iq + k]);
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             part[0][e] = fma2(q, bc(va0[e + k]), part[0][e]);
@@ -118,9 +172,9 @@ __device__ __forceinline__ void tap_step(f2 (&part)[2][8], const InRow &x0, cons
 // One 4-tap chunk: steps j = 0 .. KH (tap pair rows Q[j], first pair at c_taps[iq]) into
 // `part`, then `acc += part`.  Four staged rows live in registers and change roles every two
 // steps without moves: the loop body is four steps.  in_r -> in[strip row 0][4 tx + 4 c].
-template <int NT>
+template <int NT, int NTX, bool GT>
 __device__ __forceinline__ void conv_chunk(f2 (&acc)[2][8], const float4 *in_r, int iq, int n4, bool tail2, int IW4,
-                                           int NC4)
+                                           int NC4, const unsigned long long *gt)
 {
     f2 part[2][8];
 #pragma unroll
@@ -128,27 +182,27 @@ __device__ __forceinline__ void conv_chunk(f2 (&acc)[2][8], const float4 *in_r, 
 #pragma unroll
         for (int e = 0; e < 8; ++e) part[p][e] = bc(0.0f);
     InRow A, B, C, D;
-    load_row(A, in_r);
-    load_row(B, in_r + IW4);
-    load_row(C, in_r + 2 * IW4);
-    load_row(D, in_r + 3 * IW4);
+    load_row<NTX>(A, in_r);
+    load_row<NTX>(B, in_r + IW4);
+    load_row<NTX>(C, in_r + 2 * IW4);
+    load_row<NTX>(D, in_r + 3 * IW4);
     in_r += 4 * IW4;
 #pragma unroll 1
     for (int j4 = 0; j4 < n4; ++j4) {
-        tap_step<NT>(part, A, C, iq);
-        load_row(A, in_r);
-        tap_step<NT>(part, B, D, iq + NC4);
-        load_row(B, in_r + IW4);
-        tap_step<NT>(part, C, A, iq + 2 * NC4);
-        load_row(C, in_r + 2 * IW4);
-        tap_step<NT>(part, D, B, iq + 3 * NC4);
-        load_row(D, in_r + 3 * IW4);
+        tap_step<NT, GT>(part, A, C, iq, gt);
+        load_row<NTX>(A, in_r);
+        tap_step<NT, GT>(part, B, D, iq + NC4, gt);
+        load_row<NTX>(B, in_r + IW4);
+        tap_step<NT, GT>(part, C, A, iq + 2 * NC4, gt);
+        load_row<NTX>(C, in_r + 2 * IW4);
+        tap_step<NT, GT>(part, D, B, iq + 3 * NC4, gt);
+        load_row<NTX>(D, in_r + 3 * IW4);
         in_r += 4 * IW4;
         iq += 4 * NC4;
     }
     if (tail2) {
-        tap_step<NT>(part, A, C, iq);
-        tap_step<NT>(part, B, D, iq + NC4);
+        tap_step<NT, GT>(part, A, C, iq, gt);
+        tap_step<NT, GT>(part, B, D, iq + NC4, gt);
     }
 #pragma unroll
     for (int p = 0; p < 2; ++p)
@@ -156,16 +210,29 @@ __device__ __forceinline__ void conv_chunk(f2 (&acc)[2][8], const float4 *in_r, 
         for (int e = 0; e < 8; ++e) acc[p][e] = add2(acc[p][e], part[p][e]);
 }
 
-template <bool RENDER>
-__global__ void __launch_bounds__(kThreads, 1) conv_kernel(ConvArgs a)
+template <bool RENDER, int NTX, bool GT>
+__global__ void __launch_bounds__(NTX * kNTY, NTX == 16 ? 1 : 2) conv_kernel(const __grid_constant__ ConvArgs a,
+                                                                             const __grid_constant__ CUtensorMap tmap)
 {
-    extern __shared__ float4 smem4[];
+    constexpr int kThreads = Shape<NTX>::kThreads, kGroup = Shape<NTX>::kGroup, kTW = Shape<NTX>::kTW;
+    const unsigned long long *gt = a.gtaps;
+    extern __shared__ __align__(128) float4 smem4[];
     const int IW4 = kTW / 4 + a.NC, IW = 4 * IW4;
     const int IH = kTH + a.KH - 1 + kSlackRows;
+    const int stage_floats = (IH * IW + 31) / 32 * 32;                    // stages start on 128-byte boundaries (TMA)
     float *s_stage = reinterpret_cast<float *>(smem4);                    // [n_stages][IH][IW]
-    float *s_d = s_stage + (size_t)a.n_stages * IH * IW;                  // [kTH][kTW] data      (loglike)
+    float *s_d = s_stage + (size_t)a.n_stages * stage_floats;             // [kTH][kTW] data      (loglike)
     float *s_w = s_d + kTH * kTW;                                         // [kTH][kTW] weights   (loglike)
     __shared__ double s_red[kThreads / 32];
+#if LENSED_CONV_TMA
+    __shared__ __align__(8) unsigned long long s_bar[2];
+    if (threadIdx.x == 0) {
+        mbar_init(&s_bar[0], 1);
+        mbar_init(&s_bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+#endif
 
     // this block's share of the (tile, vector) items, tile-major
     const long long n_items = (long long)a.n_tiles * a.nb;
@@ -173,21 +240,28 @@ __global__ void __launch_bounds__(kThreads, 1) conv_kernel(ConvArgs a)
     if (lo >= hi) return;
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int tx = (warp & 1) * 8 + (lane & 7);
-    const int ty = (warp >> 1) * 4 + (lane >> 3);
+    const int tx = NTX == 16 ? (warp & 1) * 8 + (lane & 7) : (lane & 7);
+    const int ty = (NTX == 16 ? (warp >> 1) : warp) * 4 + (lane >> 3);
 
-    // input tile of an item -> stage s (all threads; one commit group)
+    // input tile of an item -> stage s
     auto issue = [&](int item, int s) {
         const int t = item / a.nb, b = item - t * a.nb;
         const uint32_t tile = a.tiles[t];
         const int Y0 = a.oy + (int)(tile >> 16) * kTH, X0 = a.ox + (int)(tile & 0xffffu) * kTW;
+        float *dst = s_stage + (size_t)s * stage_floats;
+#if LENSED_CONV_TMA
+        if (threadIdx.x == 0) {                   // one thread, one copy; completion on the stage's mbarrier
+            mbar_expect_tx(&s_bar[s], (unsigned)((IH - kSlackRows) * IW * sizeof(float)));
+            tma_load_3d(dst, &tmap, &s_bar[s], X0, Y0, b);
+        }
+#else                                             // all threads; one commit group
         const float *src = a.Lp + (size_t)b * a.lp_stride + (size_t)Y0 * a.Wp + X0;
-        float *dst = s_stage + (size_t)s * IH * IW;
         for (int i = threadIdx.x; i < (IH - kSlackRows) * IW4; i += kThreads) {
             const int r = i / IW4, c4 = i - r * IW4;
             cp_async16(dst + r * IW + 4 * c4, src + (size_t)r * a.Wp + 4 * c4);
         }
         cp_async_commit();
+#endif
     };
 
     issue(lo, 0);
@@ -224,7 +298,11 @@ __global__ void __launch_bounds__(kThreads, 1) conv_kernel(ConvArgs a)
                 *reinterpret_cast<float4 *>(s_w + r * kTW + c) = make_float4(wv[0], wv[1], wv[2], wv[3]);
             }
         }
+#if LENSED_CONV_TMA
+        mbar_wait(&s_bar[s], a.n_stages == 2 ? (((item - lo) >> 1) & 1) : ((item - lo) & 1));
+#else
         if (a.n_stages == 2 && more) cp_async_wait<1>(); else cp_async_wait<0>();
+#endif
         __syncthreads();
 
         if (t != cur_t) {
@@ -251,19 +329,19 @@ __global__ void __launch_bounds__(kThreads, 1) conv_kernel(ConvArgs a)
             for (int e = 0; e < 8; ++e) acc[p][e] = bc(0.0f);
 
         if (warp_any) {
-            const float4 *in_base = reinterpret_cast<const float4 *>(s_stage + (size_t)s * IH * IW) +
+            const float4 *in_base = reinterpret_cast<const float4 *>(s_stage + (size_t)s * stage_floats) +
                                     (size_t)(ty * kTR) * IW4 + tx;
             const int last_taps = a.KW - 4 * (a.NC - 1);          // taps of the last chunk, 1..4
             const int n_full = last_taps == 4 ? a.NC : a.NC - 1;
 #pragma unroll 1
             for (int c = 0; c < n_full; ++c)
-                conv_chunk<4>(acc, in_base + c, a.tap_off + 4 * c, n4, tail2, IW4, NC4);
+                conv_chunk<4, NTX, GT>(acc, in_base + c, a.tap_off + 4 * c, n4, tail2, IW4, NC4, gt);
             if (last_taps != 4) {
                 const float4 *in_r = in_base + n_full;
                 const int iq = a.tap_off + 4 * n_full;
-                if (last_taps == 3) conv_chunk<3>(acc, in_r, iq, n4, tail2, IW4, NC4);
-                else if (last_taps == 2) conv_chunk<2>(acc, in_r, iq, n4, tail2, IW4, NC4);
-                else conv_chunk<1>(acc, in_r, iq, n4, tail2, IW4, NC4);
+                if (last_taps == 3) conv_chunk<3, NTX, GT>(acc, in_r, iq, n4, tail2, IW4, NC4, gt);
+                else if (last_taps == 2) conv_chunk<2, NTX, GT>(acc, in_r, iq, n4, tail2, IW4, NC4, gt);
+                else conv_chunk<1, NTX, GT>(acc, in_r, iq, n4, tail2, IW4, NC4, gt);
             }
         }
 
@@ -332,7 +410,7 @@ __global__ void final_kernel(FinalArgs a)
 
 }  // namespace
 
-void conv_tile_shape(int *tile_w, int *tile_h) { *tile_w = kTW; *tile_h = kTH; }
+void conv_tile_shape(bool wide, int *tile_w, int *tile_h) { *tile_w = wide ? Shape<16>::kTW : Shape<8>::kTW; *tile_h = kTH; }
 
 // rows x cols = the image rounded up to cover every tile of the grids in use (api.cu)
 void conv_padded_shape(int rows, int cols, int KH, int NC, int *Hp, int *Wp)
@@ -342,26 +420,51 @@ void conv_padded_shape(int rows, int cols, int KH, int NC, int *Hp, int *Wp)
 }
 
 namespace {
-constexpr size_t kSmemLimit = 226 * 1024;   // dynamic part; 227 KB per block minus the static s_red
-size_t stage_bytes(int KH, int NC) { return (size_t)(kTH + KH - 1 + kSlackRows) * (kTW + 4 * NC) * sizeof(float); }
-size_t dw_bytes(bool render) { return render ? 0 : (size_t)2 * kTH * kTW * sizeof(float); }
+// dynamic shared memory a block may take: 227 KB per SM minus the static arrays, per resident block
+size_t smem_limit(bool wide) { return wide ? 226 * 1024 : 112 * 1024; }
+size_t stage_bytes(int KH, int NC, bool wide)
+{
+    const size_t floats = (size_t)(kTH + KH - 1 + kSlackRows) * ((wide ? 128 : 64) + 4 * NC);
+    return (floats + 31) / 32 * 32 * sizeof(float);
+}
+size_t dw_bytes(bool render, bool wide) { return render ? 0 : (size_t)2 * kTH * (wide ? 128 : 64) * sizeof(float); }
 }  // namespace
 
-int conv_num_stages(int KH, int NC, bool render)
+int conv_num_stages(int KH, int NC, bool render, bool wide)
 {
-    return 2 * stage_bytes(KH, NC) + dw_bytes(render) <= kSmemLimit ? 2 : 1;
+    return 2 * stage_bytes(KH, NC, wide) + dw_bytes(render, wide) <= smem_limit(wide) ? 2 : 1;
 }
 
-size_t conv_smem_bytes(int KH, int NC, bool render)
+size_t conv_smem_bytes(int KH, int NC, bool render, bool wide)
 {
-    return conv_num_stages(KH, NC, render) * stage_bytes(KH, NC) + dw_bytes(render);
+    return conv_num_stages(KH, NC, render, wide) * stage_bytes(KH, NC, wide) + dw_bytes(render, wide);
 }
+
+// the narrow shape needs its single stage + d, w to fit twice per SM
+bool conv_narrow_fits(int KH, int NC) { return stage_bytes(KH, NC, false) + dw_bytes(false, false) <= smem_limit(false); }
+
+namespace {
+template <bool RENDER, int NTX, bool GT>
+cudaError_t set_attr()
+{
+    return cudaFuncSetAttribute(conv_kernel<RENDER, NTX, GT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)smem_limit(NTX == 16));
+}
+template <bool RENDER, int NTX, bool GT>
+void launch(const ConvArgs &a, const CUtensorMap &tmap, int grid, size_t smem, cudaStream_t st)
+{
+    conv_kernel<RENDER, NTX, GT><<<grid, NTX * kNTY, smem, st>>>(a, tmap);
+}
+}  // namespace
 
 cudaError_t conv_setup()
 {
-    cudaError_t e = cudaFuncSetAttribute(conv_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(conv_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemLimit);
+    cudaError_t e;
+#define LENSED_SET(R, N, G) if ((e = set_attr<R, N, G>()) != cudaSuccess) return e;
+    LENSED_SET(false, 16, false) LENSED_SET(true, 16, false) LENSED_SET(false, 8, false) LENSED_SET(true, 8, false)
+    LENSED_SET(false, 16, true) LENSED_SET(true, 16, true) LENSED_SET(false, 8, true) LENSED_SET(true, 8, true)
+#undef LENSED_SET
+    return cudaSuccess;
 }
 
 cudaError_t conv_upload_taps(const float *pairs, int n_pairs, int pool_offset)
@@ -370,16 +473,47 @@ cudaError_t conv_upload_taps(const float *pairs, int n_pairs, int pool_offset)
                               (size_t)pool_offset * sizeof(unsigned long long), cudaMemcpyHostToDevice);
 }
 
-// n_blocks: persistent blocks to launch (the SM count; fewer when there are fewer items)
-cudaError_t launch_conv(ConvArgs a, bool render, int n_blocks, cudaStream_t st)
+// Tensor map of the padded frames L[n_frames][Hp][Wp] for boxes of one input tile with its halo
+// (conv_kernel "issue").  out: 128 bytes, 64-byte aligned.  The encoder is a driver entry point
+// fetched through the runtime, so the library links against nothing but the static runtime.
+cudaError_t conv_make_tensor_map(void *out, const float *L, int Wp, int Hp, long long n_frames, int KH, int NC, bool wide)
 {
-    a.n_stages = conv_num_stages(a.KH, a.NC, render);
-    const size_t smem = conv_smem_bytes(a.KH, a.NC, render);
+    static PFN_cuTensorMapEncodeTiled_v12000 encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
+        if (e != cudaSuccess) return e;
+        if (!fn || qr != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+        encode = (PFN_cuTensorMapEncodeTiled_v12000)fn;
+    }
+    const cuuint64_t dims[3] = {(cuuint64_t)Wp, (cuuint64_t)Hp, (cuuint64_t)std::max<long long>(n_frames, 1)};
+    const cuuint64_t strides[2] = {(cuuint64_t)Wp * sizeof(float), (cuuint64_t)Wp * Hp * sizeof(float)};
+    const cuuint32_t box[3] = {(cuuint32_t)((wide ? 128 : 64) + 4 * NC), (cuuint32_t)(kTH + KH - 1), 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = encode((CUtensorMap *)out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)L, dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+// n_sm: persistent blocks = n_sm x (blocks per SM of the shape), fewer when there are fewer items
+cudaError_t launch_conv(ConvArgs a, const void *tensor_map, bool render, int n_sm, cudaStream_t st)
+{
+    const CUtensorMap &tmap = *reinterpret_cast<const CUtensorMap *>(tensor_map);
+    const bool wide = a.wide != 0, gt = a.gtaps != nullptr;
+    a.n_stages = conv_num_stages(a.KH, a.NC, render, wide);
+    const size_t smem = conv_smem_bytes(a.KH, a.NC, render, wide);
     const long long n_items = (long long)a.n_tiles * a.nb;
+    const long long n_blocks = (long long)n_sm * (wide ? 1 : 2);
     const int grid = (int)(n_items < n_blocks ? n_items : n_blocks);
     if (grid < 1) return cudaSuccess;
-    if (render) conv_kernel<true><<<grid, kThreads, smem, st>>>(a);
-    else conv_kernel<false><<<grid, kThreads, smem, st>>>(a);
+#define LENSED_GO(R, N, G) launch<R, N, G>(a, tmap, grid, smem, st)
+    if (wide) { if (render) { if (gt) LENSED_GO(true, 16, true); else LENSED_GO(true, 16, false); }
+                else        { if (gt) LENSED_GO(false, 16, true); else LENSED_GO(false, 16, false); } }
+    else      { if (render) { if (gt) LENSED_GO(true, 8, true); else LENSED_GO(true, 8, false); }
+                else        { if (gt) LENSED_GO(false, 8, true); else LENSED_GO(false, 8, false); } }
+#undef LENSED_GO
     return cudaGetLastError();
 }
 

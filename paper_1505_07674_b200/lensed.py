@@ -44,6 +44,10 @@ SYMBOLS = {
     "lensed_get_refined": (_i, [_p, _p]),
     "lensed_set_chunk_bytes": (_i, [_p, _ll]),
     "lensed_frame_bytes": (_ll, [_p]),
+    "lensed_set_conv_shape": (_i, [_p, _i]),
+    "lensed_get_conv_shape": (_i, [_p]),
+    "lensed_uses_global_taps": (_i, [_p]),
+    "lensed_debug_force_global_taps": (None, [_i]),
     "lensed_set_static_tracer": (_i, [_p, _i]),
     "lensed_get_static_tracer": (_i, [_p]),
     "lensed_ns_run": (_i, [_p, _p, _p, _p, _i, _p, _p, _p, _p, _p, _ll, _p]),
@@ -243,6 +247,22 @@ def lensed_set_chunk_bytes(h, nbytes):
 
 def lensed_frame_bytes(h):
     return lib().lensed_frame_bytes(h)
+
+
+def lensed_set_conv_shape(h, wide):
+    _check(lib().lensed_set_conv_shape(h, int(bool(wide))), h)
+
+
+def lensed_get_conv_shape(h):
+    return lib().lensed_get_conv_shape(h)
+
+
+def lensed_uses_global_taps(h):
+    return lib().lensed_uses_global_taps(h)
+
+
+def lensed_debug_force_global_taps(on):
+    lib().lensed_debug_force_global_taps(int(bool(on)))
 
 
 def lensed_set_static_tracer(h, on):

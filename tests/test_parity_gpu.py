@@ -328,32 +328,74 @@ def test_quadrature_error_map_of_the_gauss_kronrod_rule(L, n_kronrod):
             np.abs(err[b] - ref) / bound).max()
 
 
-def test_constant_tap_pool_is_shared_by_live_handles_and_released_on_destroy(L):
-    """The PSF taps of the live handles share 60 KB of constant memory (include/lensed.h):
-    two 63x63 PSFs (32.5 KB each) do not fit together; destroying one makes room; the
-    surviving handle still computes the right thing."""
+def test_full_constant_tap_pool_falls_back_to_global_memory_taps(L):
+    """The PSF taps of the live handles share 60 KB of constant memory (include/lensed.h).  Two
+    63x63 PSFs (32.5 KB each) do not fit together: the second handle keeps its taps in global
+    memory and must compute the same thing; so must the 9th .. 16th of sixteen live 31x31 handles
+    (8 KB each) -- a sampler fitting several images or bands at once."""
     rng = np.random.default_rng(7)
     psf = rng.uniform(0.1, 1.0, size=(63, 63))
     small = synth.shrunk(synth.get_config(1), 20, 24, 2)
     cfg = synth.Config(1, "pool", small.H, small.W, small.scale, small.models, small.quad, psf, None,
                        small.truth, 2, small._draw, 0.005, 2000.0)
     prob = Problem(cfg)
-    h1 = prob.create()
-    try:
-        with pytest.raises(L.LensedError) as e:
-            prob.create()
-        assert e.value.status == L.ENOMEM
-        logl1, _ = _gpu_eval(L, h1, cfg.batch(), cfg.H, cfg.W, render=False)
-    finally:
-        L.lensed_destroy(h1)
-    h2 = prob.create()                                    # room again
-    try:
-        logl2, _ = _gpu_eval(L, h2, cfg.batch(), cfg.H, cfg.W, render=False)
-    finally:
-        L.lensed_destroy(h2)
-    assert np.array_equal(logl1, logl2)
     logl_o = prob.oracle_loglike(cfg.batch())[0]
-    assert logl_errors(logl1, logl_o).max() <= LOGL_RTOL
+    h1 = prob.create()
+    h2 = prob.create()
+    try:
+        assert L.lensed_uses_global_taps(h1) == 0 and L.lensed_uses_global_taps(h2) == 1
+        for h in (h1, h2):
+            logl, _ = _gpu_eval(L, h, cfg.batch(), cfg.H, cfg.W, render=False)
+            assert logl_errors(logl, logl_o).max() <= LOGL_RTOL
+    finally:
+        L.lensed_destroy(h1); L.lensed_destroy(h2)
+    h3 = prob.create()                                    # room in the pool again
+    try:
+        assert L.lensed_uses_global_taps(h3) == 0
+    finally:
+        L.lensed_destroy(h3)
+
+    cfg = synth.shrunk(synth.get_config(4), 70, 90, 3)    # 31 x 31 PSF
+    prob = Problem(cfg)
+    params = cfg.batch()
+    logl_o, model_o = prob.oracle_loglike(params, want_model=True)
+    handles = [prob.create() for _ in range(16)]
+    try:
+        flags = [L.lensed_uses_global_taps(h) for h in handles]
+        assert flags[0] == 0 and flags[-1] == 1 and 7 <= flags.count(0) <= 8
+        for h in (handles[0], handles[8], handles[15]):
+            logl, model = _gpu_eval(L, h, params, cfg.H, cfg.W)
+            assert logl_errors(logl, logl_o).max() <= LOGL_RTOL
+            assert pixel_errors(model, model_o).max() <= PIXEL_RTOL
+    finally:
+        for h in handles:
+            L.lensed_destroy(h)
+
+
+@pytest.mark.parametrize("index,H,W,B", [(1, 90, 70, 12), (2, 75, 93, 8), (3, 70, 150, 6), (4, 101, 67, 4), (5, 60, 64, 6)])
+@pytest.mark.parametrize("global_taps", [False, True])
+def test_both_convolution_shapes_and_both_tap_paths(L, index, H, W, B, global_taps):
+    """wide (256 threads, 64 x 128 tiles) and narrow (128 threads, 64 x 64 tiles, two blocks per
+    SM) blocks, taps from the constant pool or from global memory: same results against the oracle."""
+    cfg = synth.shrunk(synth.get_config(index), H, W, B)
+    prob = Problem(cfg)
+    params = cfg.batch()
+    logl_o, model_o = prob.oracle_loglike(params, want_model=True)
+    L.lensed_debug_force_global_taps(global_taps)
+    try:
+        h = prob.create()
+    finally:
+        L.lensed_debug_force_global_taps(False)
+    try:
+        assert L.lensed_uses_global_taps(h) == int(global_taps)
+        for wide in (1, 0):
+            L.lensed_set_conv_shape(h, wide)
+            assert L.lensed_get_conv_shape(h) == wide
+            logl, model = _gpu_eval(L, h, params, cfg.H, cfg.W)
+            assert logl_errors(logl, logl_o).max() <= LOGL_RTOL
+            assert pixel_errors(model, model_o).max() <= PIXEL_RTOL
+    finally:
+        L.lensed_destroy(h)
 
 
 def test_largest_rule_and_longest_model_list(L):
