@@ -15,9 +15,10 @@
  * (a cudaStream_t passed as void*, NULL = the legacy default stream) and is asynchronous
  * with respect to the host unless stated otherwise.
  *
- * Thread-safety: a handle owns its scratch buffers, so calls on ONE handle must not
- * overlap in time (use one handle per stream / thread); different handles are
- * independent.
+ * Thread-safety: the problem data of a handle (image, weights, mask, pixel lists, PSF) is
+ * immutable after lensed_create; its scratch buffers and options are not, so calls on ONE
+ * handle must not overlap in time.  For several streams or threads on one problem use
+ * lensed_clone: clones share the immutable device arrays and own their scratch.
  */
 #ifndef LENSED_H
 #define LENSED_H
@@ -97,6 +98,14 @@ lensed_status lensed_create(int H, int W, double pixel_scale,
                             const int *models, int n_models,
                             double mag_zero_point, int device,
                             lensed_handle **out);
+
+/*
+ * lensed_clone -- a second handle on the same problem, for another stream or thread.  The
+ * large immutable device arrays (image, weights, pixel lists, PSF taps) are shared and
+ * reference-counted; the clone has its own scratch, options and profile, so calls on the two
+ * handles may overlap in time (one handle per stream).  Either may be destroyed first.
+ * Synchronous.  EINVAL for NULL; ENOMEM / ECUDA.                                          */
+lensed_status lensed_clone(const lensed_handle *h, lensed_handle **out);
 
 /* P, the length of one parameter vector for the handle's model list; -1 for NULL.       */
 int lensed_num_params(const lensed_handle *h);

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblensed_b200.so")
 SOURCES = ("api.cu", "prep.cu", "trace.cu", "trace_sig_a.cu", "trace_sig_b.cu", "trace_sig_c.cu",
-           "trace_sig_d.cu", "trace_sig_e.cu", "trace_sig_f.cu", "trace_sig_g.cu", "trace_sig_h.cu", "refine.cu", "deflect.cu", "nested.cu", "conv.cu",
+           "trace_sig_d.cu", "trace_sig_e.cu", "trace_sig_f.cu", "trace_sig_g.cu", "trace_sig_h.cu", "trace_sig_i.cu", "refine.cu", "deflect.cu", "nested.cu", "conv.cu",
            "peak.cu")
 HEADERS = tuple(os.path.join(CSRC, f) for f in ("lensed_internal.h", "f32x2.cuh", "trace_math.cuh",
                                                   "trace_block.cuh", "trace_static.cuh")) + (

@@ -10,6 +10,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <atomic>
 #include <mutex>
 #include <utility>
 #include <new>
@@ -28,7 +29,14 @@ struct EventPair { cudaEvent_t a, b; int phase; };
 
 }  // namespace
 
+// Reference count of what lensed_clone shares between handles: the large immutable device
+// arrays of a problem (d_image, d_wmask, d_pix_ll, d_pix_all, the tap range / d_gtaps).
+struct SharedArrays {
+    std::atomic<int> refs{1};
+};
+
 struct lensed_handle {
+    SharedArrays *shared = nullptr;
     int device = 0;
     int H = 0, W = 0;
     double scale = 0, zp = 0;
@@ -471,6 +479,8 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
 
     lensed_handle *h = new (std::nothrow) lensed_handle;
     if (!h) return fail(nullptr, LENSED_ENOMEM, "host allocation failed");
+    h->shared = new (std::nothrow) SharedArrays;
+    if (!h->shared) { delete h->shared; delete h; return fail(nullptr, LENSED_ENOMEM, "host allocation failed"); }
     lensed_status s = LENSED_OK;
 #define CREATE_FAIL(expr)                                             \
     do { s = (expr); if (s != LENSED_OK) { g_last_error = h->err.empty() ? g_last_error : h->err; lensed_destroy(h); return s; } } while (0)
@@ -483,7 +493,7 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     int P = 0, D = kHeaderFloats;
     for (int m = 0; m < n_models; ++m) {
         const int k = models[m];
-        if (k < 0 || k >= K_COUNT) { delete h; return fail(nullptr, LENSED_EINVAL, "models[%d] = %d is not a lensed_kind", m, k); }
+        if (k < 0 || k >= K_COUNT) { delete h->shared; delete h; return fail(nullptr, LENSED_EINVAL, "models[%d] = %d is not a lensed_kind", m, k); }
         pg.kind[m] = (uint8_t)k;
         pg.par_off[m] = (uint16_t)P;
         pg.der_off[m] = (uint16_t)D;
@@ -517,10 +527,10 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     double wsum = 0.0;
     for (int k = 0; k < n_quad; ++k) {
         for (int c = 0; c < 3; ++c)
-            if (!isfinite(quad[3 * k + c])) { delete h; return fail(nullptr, LENSED_EINVAL, "quad[%d] not finite", k); }
+            if (!isfinite(quad[3 * k + c])) { delete h->shared; delete h; return fail(nullptr, LENSED_EINVAL, "quad[%d] not finite", k); }
         wsum += (double)quad[3 * k + 2];
     }
-    if (!(fabs(wsum) > 0.0)) { delete h; return fail(nullptr, LENSED_EINVAL, "quadrature weights sum to zero"); }
+    if (!(fabs(wsum) > 0.0)) { delete h->shared; delete h; return fail(nullptr, LENSED_EINVAL, "quadrature weights sum to zero"); }
     h->n_quad = n_quad;
     h->R = trace_pick_R(n_quad);
     h->nq_pad = (n_quad + h->R - 1) / h->R * h->R;
@@ -538,10 +548,10 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     if (has_psf) {
         double fsum = 0.0;
         for (int t = 0; t < psf_h * psf_w; ++t) {
-            if (!isfinite(psf[t])) { delete h; return fail(nullptr, LENSED_EINVAL, "psf[%d] not finite", t); }
+            if (!isfinite(psf[t])) { delete h->shared; delete h; return fail(nullptr, LENSED_EINVAL, "psf[%d] not finite", t); }
             fsum += (double)psf[t];
         }
-        if (!(fabs(fsum) > 0.0)) { delete h; return fail(nullptr, LENSED_EINVAL, "PSF sums to zero"); }
+        if (!(fabs(fsum) > 0.0)) { delete h->shared; delete h; return fail(nullptr, LENSED_EINVAL, "PSF sums to zero"); }
         for (int ky = 0; ky < psf_h; ++ky)
             for (int kx = 0; kx < psf_w; ++kx)
                 G[(size_t)ky * psf_w + kx] =
@@ -567,25 +577,25 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     int ndev = 0;
     cudaError_t ce = cudaGetDeviceCount(&ndev);
     if (ce != cudaSuccess || ndev < 1) {
-        delete h;
+        delete h->shared; delete h;
         return fail(nullptr, LENSED_ECUDA, "no CUDA device (%s); there is no CPU fallback",
                     ce != cudaSuccess ? cudaGetErrorString(ce) : "device count 0");
     }
-    if (device < 0 || device >= ndev) { delete h; return fail(nullptr, LENSED_EINVAL, "device %d of %d", device, ndev); }
+    if (device < 0 || device >= ndev) { delete h->shared; delete h; return fail(nullptr, LENSED_EINVAL, "device %d of %d", device, ndev); }
     {
         cudaError_t e1 = cudaSetDevice(device);
-        if (e1 != cudaSuccess) { delete h; return fail(nullptr, LENSED_ECUDA, "cudaSetDevice: %s", cudaGetErrorString(e1)); }
+        if (e1 != cudaSuccess) { delete h->shared; delete h; return fail(nullptr, LENSED_ECUDA, "cudaSetDevice: %s", cudaGetErrorString(e1)); }
         cudaDeviceProp prop;
         e1 = cudaGetDeviceProperties(&prop, device);
-        if (e1 != cudaSuccess) { delete h; return fail(nullptr, LENSED_ECUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e1)); }
+        if (e1 != cudaSuccess) { delete h->shared; delete h; return fail(nullptr, LENSED_ECUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e1)); }
         if (prop.major != 10) {
-            delete h;
+            delete h->shared; delete h;
             return fail(nullptr, LENSED_ECUDA, "device %d is sm_%d%d; this library holds sm_100a code only",
                         device, prop.major, prop.minor);
         }
         h->n_sm = prop.multiProcessorCount;
         e1 = conv_setup();
-        if (e1 != cudaSuccess) { delete h; return fail(nullptr, LENSED_ECUDA, "conv_setup: %s", cudaGetErrorString(e1)); }
+        if (e1 != cudaSuccess) { delete h->shared; delete h; return fail(nullptr, LENSED_ECUDA, "conv_setup: %s", cudaGetErrorString(e1)); }
     }
     CREATE_FAIL(upload(h, &h->d_image, image, HW));
     CREATE_FAIL(upload(h, &h->d_wmask, wmask.data(), HW));
@@ -614,6 +624,40 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     CREATE_FAIL(upload(h, &h->d_pix_all, pix_all.data(), pix_all.size()));
     CREATE_FAIL(build_tiles(h, default_wide(h)));
 #undef CREATE_FAIL
+    *out = h;
+    return LENSED_OK;
+}
+
+lensed_status lensed_clone(const lensed_handle *src, lensed_handle **out)
+{
+    if (!out) return fail(nullptr, LENSED_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!src) return fail(nullptr, LENSED_EINVAL, "null handle");
+    lensed_handle *h = new (std::nothrow) lensed_handle;
+    if (!h) return fail(nullptr, LENSED_ENOMEM, "host allocation failed");
+    // the problem: geometry, program, rule, PSF layout, options; the big arrays are shared
+    h->shared = src->shared;
+    h->shared->refs.fetch_add(1);
+    h->device = src->device; h->H = src->H; h->W = src->W; h->scale = src->scale; h->zp = src->zp;
+    h->prog = src->prog;
+    h->n_quad = src->n_quad; h->R = src->R; h->nq_pad = src->nq_pad; h->h_quad = src->h_quad;
+    h->has_error_rule = src->has_error_rule;
+    h->KH = src->KH; h->KW = src->KW; h->NC = src->NC; h->n_sm = src->n_sm;
+    h->tap_off = src->tap_off; h->tap_pairs = src->tap_pairs; h->d_gtaps = src->d_gtaps;
+    h->counted = src->counted;
+    h->d_image = src->d_image; h->d_wmask = src->d_wmask; h->d_pix_ll = src->d_pix_ll; h->d_pix_all = src->d_pix_all;
+    h->npix_ll = src->npix_ll; h->npix_all = src->npix_all;
+    h->chunk_bytes = src->chunk_bytes; h->static_tracer = src->static_tracer; h->refine_gain = src->refine_gain;
+    lensed_status s = LENSED_OK;
+#define CLONE_FAIL(expr) do { s = (expr); if (s != LENSED_OK) { g_last_error = h->err; lensed_destroy(h); return s; } } while (0)
+    if (cudaSetDevice(h->device) != cudaSuccess) { lensed_destroy(h); return fail(nullptr, LENSED_ECUDA, "cudaSetDevice failed"); }
+    CLONE_FAIL(upload(h, &h->d_quad, h->h_quad.data(), h->h_quad.size()));
+    const unsigned long long zero = 0;
+    const unsigned zero32 = 0;
+    CLONE_FAIL(upload(h, &h->d_refined, &zero, 1));
+    CLONE_FAIL(upload(h, &h->d_queue_count, &zero32, 1));
+    CLONE_FAIL(build_tiles(h, src->wide));
+#undef CLONE_FAIL
     *out = h;
     return LENSED_OK;
 }
@@ -864,12 +908,16 @@ void lensed_destroy(lensed_handle *h)
     cudaDeviceSynchronize();
     for (EventPair &ep : h->used) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (EventPair &ep : h->pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
-    cudaFree(h->d_image); cudaFree(h->d_wmask); cudaFree(h->d_quad);
-    if (h->tap_off >= 0) g_tap_pool.give(h->device, h->tap_off);
-    cudaFree(h->d_pix_ll); cudaFree(h->d_pix_all); cudaFree(h->d_tiles_ll); cudaFree(h->d_tiles_all);
+    cudaFree(h->d_quad); cudaFree(h->d_tiles_ll); cudaFree(h->d_tiles_all);
+    if (h->shared && h->shared->refs.fetch_sub(1) == 1) {       // the last handle of this problem
+        // the pointers of the handle are the shared ones unless create failed half-way
+        cudaFree(h->d_image); cudaFree(h->d_wmask); cudaFree(h->d_pix_ll); cudaFree(h->d_pix_all); cudaFree(h->d_gtaps);
+        if (h->tap_off >= 0) g_tap_pool.give(h->device, h->tap_off);
+        delete h->shared;
+    }
     cudaFree(h->d_derived); cudaFree(h->d_L); cudaFree(h->d_partial);
     cudaFree(h->d_derived64); cudaFree(h->d_fixmask); cudaFree(h->d_refined);
-    cudaFree(h->d_queue); cudaFree(h->d_queue_count); cudaFree(h->d_gtaps);
+    cudaFree(h->d_queue); cudaFree(h->d_queue_count);
     cudaFree(h->d_stage_in); cudaFree(h->d_stage_out);
     delete h;
 }

@@ -43,6 +43,7 @@ LENSED_DECLARE_STATIC_TRACER(trace_static_e)
 LENSED_DECLARE_STATIC_TRACER(trace_static_f)
 LENSED_DECLARE_STATIC_TRACER(trace_static_g)
 LENSED_DECLARE_STATIC_TRACER(trace_static_h)
+LENSED_DECLARE_STATIC_TRACER(trace_static_i)
 
 namespace {
 
@@ -201,7 +202,8 @@ namespace {
 typedef bool (*StaticTracer)(const int (&)[K_COUNT], const Program &, const TraceArgs &, int, int, cudaStream_t,
                              cudaError_t *);
 const StaticTracer kStaticTracers[] = {trace_static_a, trace_static_b, trace_static_c, trace_static_d,
-                                       trace_static_e, trace_static_f, trace_static_g, trace_static_h};
+                                       trace_static_e, trace_static_f, trace_static_g, trace_static_h,
+                                       trace_static_i};
 
 void count_kinds(const Program &prog, int (&counts)[K_COUNT])
 {

@@ -25,6 +25,7 @@ PHASES = ("prep", "trace", "refine", "conv", "final")
 _c, _i, _d, _p, _ll = ctypes.c_char_p, ctypes.c_int, ctypes.c_double, ctypes.c_void_p, ctypes.c_longlong
 SYMBOLS = {
     "lensed_create": (_i, [_i, _i, _d, _p, _p, _p, _p, _i, _i, _p, _i, _p, _i, _d, _i, _p]),
+    "lensed_clone": (_i, [_p, _p]),
     "lensed_num_params": (_i, [_p]),
     "lensed_num_traced": (_i, [_p]),
     "lensed_num_pixels": (_i, [_p]),
@@ -122,6 +123,13 @@ def lensed_create(image, weight, mask, psf, quad, models, pixel_scale, mag_zero_
                              float(mag_zero_point), int(device), ctypes.byref(h))
     _check(st)
     return h
+
+
+def lensed_clone(h):
+    """-> a second handle on the same problem (shared immutable arrays, own scratch)."""
+    out = ctypes.c_void_p()
+    _check(lib().lensed_clone(h, ctypes.byref(out)))
+    return out
 
 
 def lensed_num_params(h):

@@ -234,6 +234,43 @@ _MULTI_TRUTH = [0.02, -0.03, 1.2, 0.75, 35.0, 1.4, -0.9, 0.4, 0.85, 110.0,
                 0.02, -0.03, 1.0, mag_of_flux(2000.0), 4.0, 0.8, 30.0, 0.01]
 
 
+J0808_MODELS = ("sie", "sie", "fg_sersic", "fg_sersic", "fg_sersic", "src_sersic", "src_sersic", "sky")
+_J0808_TRUTH = [0.0, 0.0, 1.17, 0.80, 9.4,                       # main lens (Table 3: b, q, PA)
+                0.9, -0.7, 0.33, 0.99, 111.0,                    # companion
+                0.0, 0.0, 0.9, mag_of_flux(2500.0), 4.0, 0.8, 10.0,
+                0.0, 0.0, 0.25, mag_of_flux(600.0), 1.2, 0.7, 15.0,
+                0.9, -0.7, 0.3, mag_of_flux(400.0), 2.5, 0.9, 100.0,
+                0.12, 0.08, 0.12, mag_of_flux(25.0), 1.5, 0.6, 60.0,
+                0.05, 0.15, 0.07, mag_of_flux(10.0), 1.0, 0.8, 140.0, 0.005]
+
+
+def _draw_j0808(rng, B):
+    """two SIEs, two + one foreground Sersic components, two source components.
+    Priors a few tenths around the stand-in truth; the companion is nearly round (Table 3)."""
+    t = np.tile(np.array(_J0808_TRUTH), (B, 1))
+    t[:, [0, 1, 5, 6, 10, 11, 17, 18, 24, 25]] += rng.uniform(-0.05, 0.05, size=(B, 10))
+    t[:, 2] = rng.uniform(0.9, 1.4, size=B)
+    t[:, 3] = rng.uniform(0.5, 1.0, size=B)
+    t[:, 4] = rng.uniform(0.0, 180.0, size=B)
+    t[:, 7] = rng.uniform(0.2, 0.5, size=B)
+    t[:, 8] = rng.uniform(0.8, 1.0, size=B)
+    t[:, 9] = rng.uniform(0.0, 180.0, size=B)
+    for o, nmax in ((10, 6.0), (17, 3.0), (24, 4.0)):
+        t[:, o + 2] *= rng.uniform(0.8, 1.25, size=B)
+        t[:, o + 4] = rng.uniform(0.8, nmax, size=B)
+        t[:, o + 5] = rng.uniform(0.5, 1.0, size=B)
+        t[:, o + 6] = rng.uniform(0.0, 180.0, size=B)
+    for o in (31, 38):
+        sx, sy = _disc(rng, 0.4, B)
+        t[:, o], t[:, o + 1] = sx, sy
+        t[:, o + 2] = rng.uniform(0.05, 0.25, size=B)
+        t[:, o + 4] = rng.uniform(0.5, 4.0, size=B)
+        t[:, o + 5] = rng.uniform(0.3, 1.0, size=B)
+        t[:, o + 6] = rng.uniform(0.0, 180.0, size=B)
+    t[:, 45] = rng.uniform(0.0, 0.01, size=B)
+    return t
+
+
 class Config:
     """One synthetic workload: geometry, model list, rule, PSF, mask, truth, batch draw."""
 
@@ -341,7 +378,14 @@ def get_config(index):
         # container: a 15x15 Moffat (beta = 3, FWHM 0.1") stands in for it.
         return Config(5, "mock", 120, 120, 0.05, MOCK_MODELS, gauss_kronrod_rule(7),
                       moffat_psf(15, 2.0, 3.0), None, _MOCK_TRUTH, 4096, _draw_mock, 0.005, 2000.0)
-    raise ValueError("config index 0..5")
+    if index == 6:
+        # The paper's largest fitted model, SDSS J0808+4706: two SIEs, three
+        # foreground and two source Sersic components, sky -- 46 parameters here (the paper ties
+        # centres and counts 35).  5" cut-out at 0.05"/px (Fig. 5), sub4 rule, a
+        # 15x15 Moffat standing in for the HST PSF.  Context row, not one of BASELINE.json's.
+        return Config(6, "j0808", 100, 100, 0.05, J0808_MODELS, subsample_rule(4),
+                      moffat_psf(15, 2.0, 3.0), None, _J0808_TRUTH, 2048, _draw_j0808, 0.005, 2000.0)
+    raise ValueError("config index 0..6")
 
 
 def shrunk(cfg, H, W, B):

@@ -77,7 +77,7 @@ def test_shrunk_configs_span_tiles_and_ragged_tails(L, index, H, W, B):
 
 
 @pytest.mark.parametrize("index,H,W,B", [(0, 32, 32, 16), (1, 90, 70, 24), (2, 75, 93, 12), (3, 70, 80, 8), (4, 101, 67, 6),
-                                         (5, 60, 64, 6)])
+                                         (5, 60, 64, 6), (6, 64, 70, 8)])
 @pytest.mark.parametrize("static", [True, False])
 def test_both_tracers_on_every_config_list(L, index, H, W, B, static):
     """The model lists of BASELINE.json's configs have a compile-time specialised tracer; the
@@ -125,7 +125,8 @@ def test_paper_mock_scenario_gauss_kronrod_rule(L):
 
 
 # ------------------------------------------------- full sizes, bench launch configuration
-@pytest.mark.parametrize("index,B,n_sample", [(1, 1024, 128), (2, 4096, 96), (3, 4096, 64), (4, 16384, 64), (5, 4096, 128)])
+@pytest.mark.parametrize("index,B,n_sample", [(1, 1024, 128), (2, 4096, 96), (3, 4096, 64), (4, 16384, 64), (5, 4096, 128),
+                                              (6, 2048, 64)])
 def test_full_size_configs_on_sampled_vectors(L, index, B, n_sample):
     """BASELINE.json's full sizes in the launch configuration bench.py times; 64-128 vectors per
     config spread over the batch, each against the oracle on every pixel, so that the test sees
@@ -270,6 +271,40 @@ def test_host_buffer_calls_match_device_calls_and_chunking_does_not_change_resul
     assert np.array_equal(logl_dev, logl_chunked) and np.array_equal(model_dev, model_chunked)
     assert n == {"prep": 1, "trace": 14, "refine": 28, "conv": 14, "final": 1}
     assert all(v > 0 for v in ms.values())
+
+
+def test_clones_share_the_problem_and_run_concurrently_on_their_own_streams(L):
+    """the problem data is immutable after create and usable from several streams:
+    lensed_clone gives each stream its own scratch on the shared arrays.  Three handles, three
+    streams, overlapping calls with different batches; then the original is destroyed first and
+    the clones still work."""
+    import torch
+    cfg = synth.shrunk(synth.get_config(2), 80, 72, 8)
+    prob = Problem(cfg)
+    batches = [cfg.batch(200, stream=10 + i) for i in range(3)]
+    h0 = prob.create()
+    handles = [h0, L.lensed_clone(h0), L.lensed_clone(h0)]
+    streams = [torch.cuda.Stream() for _ in handles]
+    ps = [torch.from_numpy(b).cuda() for b in batches]
+    outs = [torch.empty(200, dtype=torch.float32, device="cuda") for _ in handles]
+    torch.cuda.synchronize()
+    try:
+        for rep in range(3):                                   # overlapping launches, repeated
+            for h, st, p, o in zip(handles, streams, ps, outs):
+                L.lensed_loglike(h, p, o, stream=st.cuda_stream)
+        torch.cuda.synchronize()
+        got = [o.cpu().numpy() for o in outs]
+        L.lensed_destroy(handles[0])                           # the original goes first
+        again = torch.empty(200, dtype=torch.float32, device="cuda")
+        L.lensed_loglike(handles[2], ps[2], again)
+        torch.cuda.synchronize()
+        assert np.array_equal(again.cpu().numpy(), got[2])
+    finally:
+        for h in handles:
+            L.lensed_destroy(h)
+    for b, g in zip(batches, got):
+        ref = prob.oracle_loglike(b[::8], want_model=False)
+        assert logl_errors(g[::8], ref).max() <= LOGL_RTOL
 
 
 def test_create_rejects_bad_arguments_on_the_gpu_box_too(L):
@@ -440,7 +475,7 @@ def test_largest_rule_and_longest_model_list(L):
 
 
 @pytest.mark.parametrize("static", [True, False])
-@pytest.mark.parametrize("index,H,W", [(1, 48, 40), (2, 64, 56), (3, 56, 48), (4, 60, 52), (5, 60, 64)])
+@pytest.mark.parametrize("index,H,W", [(1, 48, 40), (2, 64, 56), (3, 56, 48), (4, 60, 52), (5, 60, 64), (6, 56, 60)])
 def test_every_one_of_192_draws_of_the_prior_meets_the_tolerances(L, index, H, W, static):
     """192 draws per prior -- BASELINE.json's four and the paper's own mock prior (n <= 8,
     q_S >= 0.1) -- on shrunk images, both tracers: EVERY vector inside north_star's
