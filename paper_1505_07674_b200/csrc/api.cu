@@ -68,6 +68,9 @@ struct lensed_handle {
     unsigned *d_queue_count = nullptr;
     unsigned long long *d_refined = nullptr;   // pixels refined in FP64 since the last profile reset
     double refine_gain = 1.0;                  // lensed_set_refine
+    double fgx_tau = 0.15;                     // lensed_set_fg_expansion (0 = off)
+    bool rule_symmetric = true;                // odd moments of the rule vanish: the expansion may be used
+    double rule_radius = 0.0;                  // farthest rule point from the pixel centre, pixels
     float *d_L = nullptr; size_t cap_L = 0;
     alignas(64) unsigned char tmap_L[128] = {};    // CUtensorMap of d_L for the convolution's tile loads (conv.cu)
     double *d_partial = nullptr; size_t cap_partial = 0;
@@ -344,7 +347,9 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
     if (refine && (s = grow(h, &h->d_queue, &h->cap_queue, queue_cap, st)) != LENSED_OK) return s;
 
     PrepArgs pa{params_dev, h->d_derived, h->d_derived64, B,
-                h->refine_gain > 0.0 ? h->refine_gain : (double)INFINITY, h->scale, h->zp, 0.5 * (h->W - 1), 0.5 * (h->H - 1)};
+                h->refine_gain > 0.0 ? h->refine_gain : (double)INFINITY,
+                h->rule_symmetric && h->static_tracer ? h->fgx_tau : 0.0, h->rule_radius,
+                h->scale, h->zp, 0.5 * (h->W - 1), 0.5 * (h->H - 1)};
     if ((s = timed_begin(h, PH_PREP, st)) != LENSED_OK) return s;
     CU(h, launch_prep(prog, pa, st));
     if ((s = timed_end(h, st)) != LENSED_OK) return s;
@@ -537,6 +542,20 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     std::vector<float4> hq(h->nq_pad, make_float4(0.f, 0.f, 0.f, 0.f));
     for (int k = 0; k < n_quad; ++k)
         hq[k] = make_float4(quad[3 * k], quad[3 * k + 1], (float)((double)quad[3 * k + 2] / wsum), 0.f);
+    {
+        // first and third moments of the rule: the foreground expansion (trace_static.cuh) drops
+        // them, so it is used only when they vanish (every Cartesian-product rule of the paper does)
+        double m1[2] = {0, 0}, m3[4] = {0, 0, 0, 0}, rad = 0.0;
+        for (int k = 0; k < n_quad; ++k) {
+            const double x = quad[3 * k], y = quad[3 * k + 1], w = (double)quad[3 * k + 2] / wsum;
+            m1[0] += w * x; m1[1] += w * y;
+            m3[0] += w * x * x * x; m3[1] += w * x * x * y; m3[2] += w * x * y * y; m3[3] += w * y * y * y;
+            rad = std::max(rad, sqrt(x * x + y * y));
+        }
+        h->rule_radius = rad;
+        h->rule_symmetric = fabs(m1[0]) < 1e-7 && fabs(m1[1]) < 1e-7 && fabs(m3[0]) < 1e-8 && fabs(m3[1]) < 1e-8 &&
+                            fabs(m3[2]) < 1e-8 && fabs(m3[3]) < 1e-8;
+    }
 
     // PSF: normalise in double, flip (eq. 15 uses F_{-k,-l}) -> G[KH][KW]; the convolution
     // reads tap PAIRS  Q[j][c][k] = (G[j][4c+k], G[j-1][4c+k]),  j = 0..KH, G[-1] = G[KH] = 0,
@@ -648,6 +667,7 @@ lensed_status lensed_clone(const lensed_handle *src, lensed_handle **out)
     h->d_image = src->d_image; h->d_wmask = src->d_wmask; h->d_pix_ll = src->d_pix_ll; h->d_pix_all = src->d_pix_all;
     h->npix_ll = src->npix_ll; h->npix_all = src->npix_all;
     h->chunk_bytes = src->chunk_bytes; h->static_tracer = src->static_tracer; h->refine_gain = src->refine_gain;
+    h->fgx_tau = src->fgx_tau; h->rule_symmetric = src->rule_symmetric; h->rule_radius = src->rule_radius;
     lensed_status s = LENSED_OK;
 #define CLONE_FAIL(expr) do { s = (expr); if (s != LENSED_OK) { g_last_error = h->err; lensed_destroy(h); return s; } } while (0)
     if (cudaSetDevice(h->device) != cudaSuccess) { lensed_destroy(h); return fail(nullptr, LENSED_ECUDA, "cudaSetDevice failed"); }
@@ -715,8 +735,8 @@ lensed_status lensed_render_error(lensed_handle *h, const float *params_dev, int
     lensed_status s;
     if ((s = grow(h, &h->d_derived, &h->cap_derived, (size_t)B * prog.D, st)) != LENSED_OK) return s;
     if ((s = grow(h, &h->d_derived64, &h->cap_derived64, (size_t)B * prog.n_models * kD64PerModel, st)) != LENSED_OK) return s;
-    PrepArgs pa{params_dev, h->d_derived, h->d_derived64, B, (double)INFINITY, h->scale, h->zp, 0.5 * (h->W - 1),
-                0.5 * (h->H - 1)};
+    PrepArgs pa{params_dev, h->d_derived, h->d_derived64, B, (double)INFINITY, 0.0, h->rule_radius, h->scale, h->zp,
+                0.5 * (h->W - 1), 0.5 * (h->H - 1)};
     if ((s = timed_begin(h, PH_PREP, st)) != LENSED_OK) return s;
     CU(h, launch_prep(prog, pa, st));
     if ((s = timed_end(h, st)) != LENSED_OK) return s;
@@ -830,6 +850,14 @@ lensed_status lensed_set_refine(lensed_handle *h, double gain)
     if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
     if (gain != gain) return fail(h, LENSED_EINVAL, "gain is NaN");
     h->refine_gain = gain > 0.0 ? gain : 0.0;
+    return LENSED_OK;
+}
+
+lensed_status lensed_set_fg_expansion(lensed_handle *h, double tau)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (tau != tau || tau > 0.5) return fail(h, LENSED_EINVAL, "tau = %g outside [0, 0.5]", tau);
+    h->fgx_tau = tau > 0.0 ? tau : 0.0;
     return LENSED_OK;
 }
 

@@ -24,9 +24,13 @@ namespace lensed {
 //         A = b sqrt(q)/q' with q' floored at 1e-4, l = ln(2)/2 (trace.cu lens_sie)
 //  POINT  [c0][thetaE^2, 0, 0, 0]                                       8
 //  SHEAR  [g1, g2, 0, 0]                                                4
-//  SERSIC [c0][a1, a2, a3, a4][log2 I0, b_n*log2(e), 1/(2n), T2]        12
+//  SERSIC [c0][a1, a2, a3, a4][log2 I0, b_n*log2(e), 1/(2n), T2][s_lo, s_hi, s_lo2, s_hi2]   16
 //         T2 = squared scaled radius inside which a source's pixels are refined in FP64
-//         (prep.cu "refinement threshold"; 0 for foregrounds and n <= 1)
+//         (prep.cu "refinement threshold"; 0 for foregrounds and n <= 1);
+//         [s_lo, s_hi] (foregrounds): range of the squared scaled radius of a pixel centre in
+//         which the pixel integral of the profile is taken from its moment expansion instead
+//         of the per-ray sum (trace_static.cuh "foreground expansion"; empty range = never);
+//         inside [s_lo2, s_hi2] its second-order terms are enough
 //         (u', v') = (a1 dx + a2 dy, a3 dx + a4 dy) = rotated, q-stretched offset / r_S,
 //         so that u'^2 + v'^2 = (R / r_S)^2 with R of PAPER.md:250 eq. 23
 //  GAUSS  [c0][a1, a2, a3, a4][log2 I0, log2(e)/2, 0, 0]                12   (offset / sigma)
@@ -66,7 +70,8 @@ __host__ __device__ constexpr int kind_num_params(int k) {
 }
 __host__ __device__ constexpr int kind_num_derived(int k) {
     return k == K_SIS ? 8 : k == K_SIE ? 12 : k == K_POINT ? 8 : k == K_SHEAR ? 4
-         : (k >= K_SRC_SERSIC && k <= K_FG_GAUSS) ? 12 : k == K_SKY ? 4 : -1;
+         : (k == K_SRC_SERSIC || k == K_FG_SERSIC) ? 16 : (k == K_SRC_GAUSS || k == K_FG_GAUSS) ? 12
+         : k == K_SKY ? 4 : -1;
 }
 
 // The model list compiled to two flat programs (lenses first, then lights); passed to the
@@ -90,6 +95,8 @@ struct PrepArgs {
     double *derived64;     // [B][n_models][kD64PerModel]
     int B;
     double refine_gain;    // scales the refinement threshold G (1 = default; prep.cu)
+    double fgx_tau;        // foreground expansion: largest expansion parameter tau (0 = off; prep.cu)
+    double rule_radius;    // largest distance of a rule point from the pixel centre, pixels
     double scale, zp;      // arcsec per pixel, magnitude zero point
     double cxh, cyh;       // (W-1)/2, (H-1)/2
 };

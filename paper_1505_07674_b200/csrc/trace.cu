@@ -175,7 +175,7 @@ size_t trace_smem_bytes(const Program &prog, int nq_pad)
 {
     const size_t n_slots = 1 + prog.n_lens + prog.n_light;
     const size_t nq4 = ((size_t)nq_pad + 3) / 4 * 4;          // keeps the float4 scratch after the tables aligned
-    return (size_t)prog.D * sizeof(float) + (n_slots * 2 + 2) * nq4 * sizeof(float) + (size_t)prog.n_light * sizeof(float4);
+    return (size_t)prog.D * sizeof(float) + (n_slots * 2 + 2) * nq4 * sizeof(float) + (size_t)prog.n_light * (sizeof(float4) + 8 * sizeof(float));
 }
 
 // Rays carried per thread, R = 2 NP in {2, 4, 6, 8, 10}: least padded rule length, weighted

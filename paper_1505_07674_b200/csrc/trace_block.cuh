@@ -12,7 +12,12 @@
 
 namespace lensed {
 
-constexpr int kTraceThreads = 256;
+struct FgMoments;
+
+#ifndef LENSED_TRACE_THREADS
+#define LENSED_TRACE_THREADS 256          // tuning builds: 128 with twice the resident blocks
+#endif
+constexpr int kTraceThreads = LENSED_TRACE_THREADS;
 
 struct TraceBlock {
     const float4 *sder;   // derived constants of the vector
@@ -20,6 +25,7 @@ struct TraceBlock {
     const float *sw;      // rule weights
     const float *sdw;     // rule weights minus the embedded rule's (error estimate, trace.cu)
     float4 *smat;         // [n_light] scratch matrices (trace_static.cuh "direct frames")
+    struct FgMoments *sfgx; // [n_light] rule moments per foreground Sersic (trace_static.cuh "foreground expansion")
     float sky;            // summed sky levels
     bool valid;
 };
@@ -39,7 +45,8 @@ __device__ __forceinline__ TraceBlock trace_prologue(const Program &prog, const 
     __syncthreads();
     float *sdw = sw + nq;
     float4 *smat = reinterpret_cast<float4 *>(sdw + nq);      // nq is even and the tables are 16-byte aligned
-    TraceBlock tb{sder, stab, sw, sdw, smat, 0.0f, sder[0].x != 0.0f};
+    TraceBlock tb{sder, stab, sw, sdw, smat, reinterpret_cast<struct FgMoments *>(smat + prog.n_light), 0.0f,
+                  sder[0].x != 0.0f};
     if (!tb.valid) return tb;                     // vector outside the model domain: block-uniform
     for (int m = 0; m < prog.n_light; ++m)
         if (prog.light_kind[m] == K_SKY) tb.sky += sder[prog.light_off[m] >> 2].x;

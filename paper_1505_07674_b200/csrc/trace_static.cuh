@@ -36,6 +36,51 @@ struct TraceSig {
     }
 };
 
+// ---- foreground expansion ------------------------------------------------------------------
+// A foreground Sersic (eqs. 22-23) is evaluated at the image-plane point
+// itself (eq. 2), so over one pixel its argument moves over a known patch of its own frame:
+// y = y0 + M delta_k with y0 = M (pixel centre - c) and delta_k the rule offsets.  Away from
+// its centre the profile I = exp(h(s)), s = |y|^2, h = ln I0 - b_n s^(1/2n), is smooth on that
+// scale, and the rule sum of eq. 14 follows from its Taylor series in
+// Delta = s - s0 = L + Q,  L = 2 y0 . M delta,  Q = |M delta|^2,  to fourth order in delta:
+//   sum_k w_k I(y0 + M delta_k) = F0 + F1 E[Q] + F2/2 (E[L^2] + E[Q^2]) + F3/2 E[L^2 Q] + F4/24 E[L^4],
+// Fj = d^j exp(h)/ds^j at s0, where E[.] = sum_k w_k (.) are second and fourth moments of the
+// rule in the light's frame (the odd ones vanish for a symmetric rule; api.cu checks).  The
+// block prologue sums them from the SAME frame table the per-ray path reads, so the expansion
+// reproduces the rule's own sum -- not the exact integral -- to 0.016 tau^6 (prep.cu
+// "foreground expansion" derives the range of s0 where tau <= fgx_tau; default 0.15: 2e-7).
+// Cost: 4 MUFU + ~70 flops per PIXEL instead of 3 MUFU + 17 flops per RAY; pixels outside the
+// range (the few around the profile's centre) take the per-ray sum.
+struct FgMoments { float S11, S12, S22, T0, T1, T2, T3, T4; };       // E[d_i d_j], E[d1^(4-i) d2^i]
+
+// full: fourth-order form; else the second-order terms only (valid on the narrower range d[3].zw)
+__device__ __forceinline__ float fg_expansion(const float4 *d, const FgMoments &m, float a, float b, float s0, bool full)
+{
+    const float4 c2 = d[2];                              // log2 I0, b_n log2 e, 1/(2n)
+    const float c = c2.z;
+    const float e = mufu_ex2(c * mufu_lg2(s0));          // s0^c
+    const float F = mufu_ex2(fmaf(-c2.y, e, c2.x));
+    const float is = mufu_rcp(s0);
+    const float h1 = -(c2.y * 0.69314718056f) * c * e * is;           // dh/ds = -b_n c s^(c-1)
+    const float h2 = h1 * (c - 1.0f) * is;
+    const float h11 = h1 * h1;
+    if (!full) {
+        const float el2 = 4.0f * (a * a * m.S11 + 2.0f * a * b * m.S12 + b * b * m.S22);
+        return fmaf(F, fmaf(h1, m.S11 + m.S22, 0.5f * (h11 + h2) * el2), F);
+    }
+    const float h3 = h2 * (c - 2.0f) * is, h4 = h3 * (c - 3.0f) * is;
+    const float F1 = h1, F2 = h11 + h2, F3 = h1 * (h11 + 3.0f * h2) + h3;
+    const float F4 = h11 * (h11 + 6.0f * h2) + 3.0f * h2 * h2 + 4.0f * h1 * h3 + h4;
+    const float aa = a * a, ab = a * b, bb = b * b;
+    const float EQ = m.S11 + m.S22;
+    const float EL2 = 4.0f * (aa * m.S11 + 2.0f * ab * m.S12 + bb * m.S22);
+    const float EQ2 = m.T0 + 2.0f * m.T2 + m.T4;
+    const float EL2Q = 4.0f * (aa * (m.T0 + m.T2) + 2.0f * ab * (m.T1 + m.T3) + bb * (m.T2 + m.T4));
+    const float EL4 = 16.0f * (aa * (aa * m.T0 + 4.0f * ab * m.T1 + 6.0f * bb * m.T2) + bb * (4.0f * ab * m.T3 + bb * m.T4));
+    const float corr = F1 * EQ + 0.5f * F2 * (EL2 + EQ2) + 0.5f * F3 * EL2Q + (1.0f / 24.0f) * F4 * EL4;
+    return fmaf(F, corr, F);
+}
+
 template <int NP, class S, int MODE>
 __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArgs &a, const TraceBlock &tb, float *Lb)
 {
@@ -83,6 +128,32 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
             }
         }
 
+        // foreground Sersics: moment expansion where it holds, else their own per-ray sum
+        float fg = 0.0f;
+#pragma unroll
+        for (int i = 0; i < S::n_fs; ++i) {
+            const float4 *d = sder + (prog.light_off[G_FS + i] >> 2);
+            const float s0 = fmaf(gu[G_FS + i], gu[G_FS + i], gv[G_FS + i] * gv[G_FS + i]);
+            const float4 rng = d[3];
+            if (s0 >= rng.x && s0 <= rng.y) {
+                fg += fg_expansion(d, tb.sfgx[i], gu[G_FS + i], gv[G_FS + i], s0, !(s0 >= rng.z && s0 <= rng.w));
+            } else {
+                f2 accf = bc(0.0f);
+#pragma unroll 1
+                for (int q0 = 0; q0 < nq; q0 += R) {
+                    Rays<NP> rf_;
+                    light_profile<NP, false, false, true>(d, gtab + (size_t)(2 * (G_FS + i)) * nq + q0,
+                                                          gtab + (size_t)(2 * (G_FS + i) + 1) * nq + q0, gu[G_FS + i],
+                                                          gv[G_FS + i], rf_, nullptr, rdummy);
+                    f2 w[NP];
+                    load_pairs<NP>(tb.sw + q0, w);
+#pragma unroll
+                    for (int k = 0; k < NP; ++k) accf = fma2(w[k], rf_.I[k], accf);
+                }
+                fg += lo2(accf) + hi2(accf);
+            }
+        }
+
         f2 acc = bc(0.0f);
 #pragma unroll 1
         for (int q0 = 0; q0 < nq; q0 += R) {
@@ -112,25 +183,21 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
                 const int m = L_PT + i;
                 lens_circular<NP, true>(sder + (prog.lens_off[m] >> 2), tb.stab + q0, tb.stab + nq + q0, lu[m], lv[m], r);
             }
-            if (NPOS == 0) {
+            if (NPOS - S::n_fs == 0) {                    // no light left in the ray loop
 #pragma unroll
                 for (int k = 0; k < NP; ++k) r.I[k] = bc(0.0f);
             }
-            // foreground lights first: they do not wait for the deflection
+            // foreground lights first: they do not wait for the deflection (foreground Sersics
+            // are not in this loop: "foreground expansion" above)
 #define LENSED_LIGHT(m, SRC, GAUSS, INIT)                                                                     \
     light_profile<NP, SRC, GAUSS, INIT>(sder + (prog.light_off[m] >> 2), gtab + (size_t)(2 * (m)) * nq + q0, \
                                         gtab + (size_t)(2 * (m) + 1) * nq + q0, gu[m], gv[m], r,              \
                                         (SRC) && S::direct ? tb.smat + (m) : nullptr,                         \
                                         (SRC) && !(GAUSS) ? rmin[(m) < S::n_ss ? (m) : 0] : rdummy)
-            constexpr bool fg_first = S::n_fs + S::n_fg > 0;
-#pragma unroll
-            for (int i = 0; i < S::n_fs; ++i) {
-                if (i == 0) LENSED_LIGHT(G_FS + i, false, false, true);
-                else LENSED_LIGHT(G_FS + i, false, false, false);
-            }
+            constexpr bool fg_first = S::n_fg > 0;
 #pragma unroll
             for (int i = 0; i < S::n_fg; ++i) {
-                if (i == 0 && S::n_fs == 0) LENSED_LIGHT(G_FG + i, false, true, true);
+                if (i == 0) LENSED_LIGHT(G_FG + i, false, true, true);
                 else LENSED_LIGHT(G_FG + i, false, true, false);
             }
 #pragma unroll
@@ -149,7 +216,7 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
 #pragma unroll
             for (int k = 0; k < NP; ++k) acc = fma2(w[k], r.I[k], acc);
         }
-        store_pixel(a, Lb, row, col, (lo2(acc) + hi2(acc)) + tb.sky);
+        store_pixel(a, Lb, row, col, ((lo2(acc) + hi2(acc)) + fg) + tb.sky);
 #pragma unroll
         for (int i = 0; i < S::n_ss; ++i)
             if (rmin[i] < sder[(prog.light_off[i] >> 2) + 2].w) flags |= bit;
@@ -160,7 +227,7 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
 // MINB = resident blocks per SM the register budget is cut for (3 -> 80 registers, 2 -> 128):
 // chosen per signature where it was measured (profiles/r1f.md)
 template <int NP, class S, int MINB>
-__global__ void __launch_bounds__(kTraceThreads, MINB) trace_static_kernel(Program prog, TraceArgs a)
+__global__ void __launch_bounds__(kTraceThreads, MINB * (256 / kTraceThreads)) trace_static_kernel(Program prog, TraceArgs a)
 {
     extern __shared__ float4 smem4[];
     const TraceBlock tb = trace_prologue(prog, a, smem4);
@@ -187,6 +254,23 @@ __global__ void __launch_bounds__(kTraceThreads, MINB) trace_static_kernel(Progr
             const float4 c2 = tb.sder[(prog.lens_off[S::n_shear] >> 2) + 2];  // (cs A, sn A, cs A l, -sn A l)
             tb.smat[threadIdx.x] = make_float4(fmaf(M.x, c2.x, M.y * c2.y), fmaf(M.x, c2.w, M.y * c2.z),
                                                fmaf(M.z, c2.x, M.w * c2.y), fmaf(M.z, c2.w, M.w * c2.z));
+        }
+        __syncthreads();
+    }
+    if constexpr (S::n_fs > 0) {
+        // rule moments in the frame of every foreground Sersic ("foreground expansion"), from the
+        // table the per-ray path reads (padding entries have zero weight)
+        if (threadIdx.x < S::n_fs) {
+            const int nq = a.nq_pad;
+            const int m = S::n_ss + S::n_sg + threadIdx.x;
+            const float *tu = tb.stab + (size_t)(2 * (1 + S::n_lens + m)) * nq, *tv = tu + nq;
+            FgMoments mo{0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+            for (int k = 0; k < nq; ++k) {
+                const float w = tb.sw[k], d1 = tu[k], d2 = tv[k], w11 = w * d1 * d1, w12 = w * d1 * d2, w22 = w * d2 * d2;
+                mo.S11 += w11; mo.S12 += w12; mo.S22 += w22;
+                mo.T0 += w11 * d1 * d1; mo.T1 += w11 * d1 * d2; mo.T2 += w11 * d2 * d2; mo.T3 += w12 * d2 * d2; mo.T4 += w22 * d2 * d2;
+            }
+            tb.sfgx[threadIdx.x] = mo;
         }
         __syncthreads();
     }

@@ -42,6 +42,7 @@ SYMBOLS = {
     "lensed_get_profile": (_i, [_p, _p, _p]),
     "lensed_reset_profile": (_i, [_p]),
     "lensed_set_refine": (_i, [_p, _d]),
+    "lensed_set_fg_expansion": (_i, [_p, _d]),
     "lensed_get_refined": (_i, [_p, _p]),
     "lensed_set_chunk_bytes": (_i, [_p, _ll]),
     "lensed_frame_bytes": (_ll, [_p]),
@@ -240,6 +241,10 @@ def lensed_reset_profile(h):
 
 def lensed_set_refine(h, gain):
     _check(lib().lensed_set_refine(h, float(gain)), h)
+
+
+def lensed_set_fg_expansion(h, tau):
+    _check(lib().lensed_set_fg_expansion(h, float(tau)), h)
 
 
 def lensed_get_refined(h):

@@ -530,6 +530,52 @@ def test_refinement_switch(L):
     assert out[0.0][1] == 0 and out[0.0][0].max() > 3 * LOGL_RTOL
 
 
+@pytest.mark.parametrize("rule", ["sub4", "gl3", "g3k7", "lopsided"])
+def test_foreground_expansion_reproduces_the_rule_sum(L, rule):
+    """The specialised tracers take a foreground Sersic's pixel integral from its fourth-order
+    moment expansion where tau <= 0.15 (trace_static.cuh "foreground expansion").  Unlensed
+    foreground components over their whole parameter range -- n from 0.3 (steeper than a Gaussian
+    outside, range bounded ABOVE) to 8, axis ratios to 0.2, radii from 1.5 pixels up -- against the
+    oracle with the expansion on (default), off, and at the loosest setting the API takes; the
+    lopsided rule has odd moments, so the library must not use the expansion at all."""
+    import torch
+    quad = {"sub4": synth.subsample_rule(4), "gl3": synth.gauss_legendre_rule(3), "g3k7": synth.gauss_kronrod_rule(7),
+            "lopsided": np.array([[0.3, 0.1, 0.5], [-0.2, 0.25, 0.2], [-0.1, -0.3, 0.3]])}[rule]
+    models = ("sie", "src_sersic", "fg_sersic", "sky")
+    rng = np.random.default_rng(21)
+    rows = []
+    for n in (0.3, 0.5, 0.8, 1.0, 1.5, 2.5, 4.0, 6.0, 8.0):
+        for _ in range(3):
+            rows.append([0.0, 0.0, 0.3, 0.8, 20.0, 0.2, 0.1, 0.1, synth.mag_of_flux(20.0), 1.5, 0.7, 30.0,
+                         rng.uniform(-0.3, 0.3), rng.uniform(-0.3, 0.3), np.exp(rng.uniform(np.log(0.075), np.log(1.5))),
+                         synth.mag_of_flux(2000.0), n, rng.uniform(0.2, 1.0), rng.uniform(0, 180), 0.01])
+    params = np.array(rows, dtype=np.float32)
+    cfg = _mini(models, rows[0], H=60, W=56, psf=synth.gaussian_psf(5, 1.7), quad=quad)
+    prob = Problem(cfg)
+    logl_o, model_o = prob.oracle_loglike(params, want_model=True)
+    h = prob.create()
+    try:
+        assert L.lensed_get_static_tracer(h) == 1
+        out = {}
+        for tau in (0.15, 0.0, 0.5):
+            L.lensed_set_fg_expansion(h, tau)
+            logl, model = _gpu_eval(L, h, params, cfg.H, cfg.W)
+            out[tau] = (logl, model)
+            if tau < 0.5:
+                assert logl_errors(logl, logl_o).max() <= LOGL_RTOL
+                assert pixel_errors(model, model_o).max() <= PIXEL_RTOL
+        with pytest.raises(L.LensedError):
+            L.lensed_set_fg_expansion(h, 0.7)
+    finally:
+        L.lensed_destroy(h)
+    d = np.abs(out[0.15][1] - out[0.0][1]).max() / np.abs(model_o).max()
+    if rule == "lopsided":
+        assert np.array_equal(out[0.15][1], out[0.0][1]) and np.array_equal(out[0.5][1], out[0.0][1])
+    else:
+        assert 0 < d < 3e-6                                  # used, and as accurate as derived
+        assert pixel_errors(out[0.5][1], model_o).max() < 20 * PIXEL_RTOL   # tau = 0.5: 0.016 tau^6 = 2.5e-4
+
+
 @pytest.mark.parametrize("static", [True, False])
 def test_two_sies_in_different_modes_one_flat_one_round(L, static):
     """The SIE mode is per vector (the most general one any of its SIEs needs).  A flat SIE
