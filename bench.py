@@ -172,6 +172,129 @@ def run_reference(args, cfg, B):
         "gpu_launches": 0}))
 
 
+
+
+class Bench:
+    """One handle on one config with its device buffers; `run` times K steps of lensed_loglike."""
+
+    def __init__(self, lensed, torch, index, B, local, rank, args=None):
+        self.L, self.torch, self.index, self.B, self.local = lensed, torch, index, B, local
+        self.cfg = cfg = synth.get_config(index)
+        self.dev = torch.device("cuda", local)
+        self.image, self.weight = make_observation_cuda(cfg, local)
+        self.h = lensed.lensed_create(self.image, self.weight, cfg.mask, cfg.psf, cfg.quad,
+                                      synth.kind_ids(cfg.models), cfg.scale, cfg.zp, local)
+        if args is not None and args.interpreter:
+            lensed.lensed_set_static_tracer(self.h, 0)
+        if args is not None and args.conv_shape != "auto":
+            lensed.lensed_set_conv_shape(self.h, args.conv_shape == "wide")
+        self.tracer_kind = "static" if lensed.lensed_get_static_tracer(self.h) == 1 else "interpreter"
+        self.conv_shape = "wide" if lensed.lensed_get_conv_shape(self.h) else "narrow"
+        self.n_traced = cfg.n_traced()                       # m_d, the required set (SURVEY.md 8(d))
+        assert self.n_traced <= lensed.lensed_num_traced(self.h)
+        self.n_counted = int(cfg.H * cfg.W if cfg.mask is None else cfg.mask.sum())
+        self.params = cfg.batch(B, stream=2 + rank)          # this rank's shard of the global batch
+        self.p_dev = torch.from_numpy(self.params).to(self.dev)
+        self.logl = torch.empty(B, dtype=torch.float32, device=self.dev)
+
+    def close(self):
+        self.L.lensed_destroy(self.h)
+
+    def run(self, steps, warmup, flush, barrier=None):
+        """-> (ms of every timed step, per-phase ms, per-phase launches, wall t0, t1)"""
+        L, torch, h = self.L, self.torch, self.h
+        stream = torch.cuda.current_stream()
+        for _ in range(warmup):
+            L.lensed_loglike(h, self.p_dev, self.logl)
+        L.lensed_set_profiling(h, True)
+        L.lensed_reset_profile(h)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        (barrier or torch.cuda.synchronize)()
+        t0 = time.perf_counter()
+        for a, b in ev:
+            flush.zero_()                                    # L2 flush between timed iterations (untimed)
+            a.record(stream)
+            L.lensed_loglike(h, self.p_dev, self.logl)
+            b.record(stream)
+        (barrier or torch.cuda.synchronize)()
+        t1 = time.perf_counter()
+        ms = [a.elapsed_time(b) for a, b in ev]
+        phase_ms, phase_n = L.lensed_get_profile(h)
+        L.lensed_set_profiling(h, False)
+        return ms, phase_ms, phase_n, t0, t1
+
+    def flop_model(self, steps, phase_n):
+        """algorithmic flops of ONE launch of the tracer / the convolution, averaged over its launches"""
+        cfg = self.cfg
+        return {"trace": flops_per_ray(cfg.models) * len(cfg.quad) * self.n_traced * self.B * steps / max(phase_n["trace"], 1),
+                "conv": flops_per_conv_pixel(cfg) * self.n_counted * self.B * steps / max(phase_n["conv"], 1)}
+
+    def kernels(self, steps, phase_ms, phase_n):
+        per_launch = self.flop_model(steps, phase_n)
+        out = {}
+        for k in self.L.PHASES:
+            tf = None
+            if k in per_launch and phase_ms[k] > 0:
+                tf = per_launch[k] * phase_n[k] / (phase_ms[k] * 1e-3) / 1e12
+            out[k] = {"ms_per_step": phase_ms[k] / steps, "launches_per_step": phase_n[k] / steps, "tflops": tf,
+                      "frac": tf / NOMINAL_FP32_TFLOPS if tf else None}
+        return out
+
+    def summary(self, steps, warmup, flush):
+        """short row for the per-config table of the bench line"""
+        ms, phase_ms, phase_n, _, _ = self.run(steps, warmup, flush)
+        cfg = self.cfg
+        value = self.B * steps / (sum(ms) * 1e-3)
+        per_launch = self.flop_model(steps, phase_n)
+        k = self.kernels(steps, phase_ms, phase_n)
+        whole = (per_launch["trace"] * phase_n["trace"] + per_launch["conv"] * phase_n["conv"]) / (sum(ms) * 1e-3) / 1e12
+        return {"config": self.index, "workload": workload_name(cfg, self.B), "logl_per_s": value,
+                "rays_per_s": value * self.n_traced * len(cfg.quad), "ms_per_step": sum(ms) / steps, "steps": steps,
+                "tracer": self.tracer_kind, "conv_shape": self.conv_shape,
+                "trace_ms": k["trace"]["ms_per_step"], "trace_frac": k["trace"]["frac"],
+                "conv_ms": k["conv"]["ms_per_step"], "conv_frac": k["conv"]["frac"],
+                "other_ms": sum(k[p]["ms_per_step"] for p in ("prep", "refine", "final")),
+                "whole_step_frac": whole / NOMINAL_FP32_TFLOPS}
+
+
+def nested_row(lensed, torch, local, rounds=40, n_live=1024, batch=1024):
+    """The batched likelihood inside its caller: a fixed number of rounds of the
+    device-resident nested sampler on the HST config at full size, six free parameters in a box
+    around the truth.  Likelihood evaluations per second of wall time, everything included
+    (proposals, lensed_loglike, replacement, evidence); the call is synchronous."""
+    b = Bench(lensed, torch, 1, 1, local, 0)
+    t = b.cfg.truth.astype(np.float64)
+    lo, hi = t.copy(), t.copy()
+    lo[2], hi[2] = t[2] - 0.03, t[2] + 0.03                  # Einstein radius
+    lo[3], hi[3] = t[3] - 0.05, t[3] + 0.05                  # lens axis ratio
+    lo[7:9], hi[7:9] = t[7:9] - 0.03, t[7:9] + 0.03          # source position
+    lo[9], hi[9] = 0.8 * t[9], 1.25 * t[9]                   # source radius
+    lo[10], hi[10] = t[10] - 0.3, t[10] + 0.3                # source magnitude
+    kw = dict(n_live=n_live, batch=batch, tol=1e-30, enlarge=1.2, seed=5)
+    lensed.lensed_ns_run(b.h, lo, hi, max_rounds=3, **kw)    # warm-up: allocations, first launches
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    res = lensed.lensed_ns_run(b.h, lo, hi, max_rounds=rounds, **kw)
+    dt = time.perf_counter() - t0
+    b.close()
+    return {"workload": workload_name(b.cfg, batch) + ", %d live points, 6 free parameters" % n_live,
+            "rounds": int(res["n_rounds"]), "likelihood_calls": int(res["n_likelihood"]),
+            "likelihood_per_s": res["n_likelihood"] / dt, "rounds_per_s": res["n_rounds"] / dt,
+            "dead_points": int(res["n_dead"]), "wall_s": dt, "timing": "host wall clock around the synchronous call"}
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` with no launcher around it: start the N ranks ourselves, the
+    way the driver's torchrun line does (one process per GPU, NCCL rendezvous on 127.0.0.1)."""
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    os.execv(sys.executable, cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -181,6 +304,8 @@ def main():
     ap.add_argument("--config", type=int, default=DEFAULT_CONFIG)
     ap.add_argument("--batch", type=int, default=0, help="vectors per GPU per step (0 = the config's)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the batch sweep of the Euclid config")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip the per-config rows (configs 0-3, 5) and the nested-sampling row")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--conv-shape", default="auto", choices=("auto", "wide", "narrow"),
                     help="convolution block shape (include/lensed.h); auto = what lensed_create picks")
@@ -191,6 +316,8 @@ def main():
     B = args.batch or cfg.B
     if args.impl == "reference":
         return run_reference(args, cfg, B)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return respawn_under_torchrun(args)
 
     import torch
     import torch.distributed as dist
@@ -201,29 +328,12 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py --impl ours needs a CUDA device: the library has no CPU fallback")
+    if local >= torch.cuda.device_count():
+        raise SystemExit("bench.py --gpus %d: rank %d has no GPU (%d visible)" % (world, local, torch.cuda.device_count()))
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
-
-    image, weight = make_observation_cuda(cfg, local)
-    kinds = synth.kind_ids(cfg.models)
-    h = lensed.lensed_create(image, weight, cfg.mask, cfg.psf, cfg.quad, kinds, cfg.scale, cfg.zp, local)
-    if args.interpreter:
-        lensed.lensed_set_static_tracer(h, 0)
-    if args.conv_shape != "auto":
-        lensed.lensed_set_conv_shape(h, args.conv_shape == "wide")
-    tracer_kind = "static" if lensed.lensed_get_static_tracer(h) == 1 else "interpreter"
-    conv_shape = "wide" if lensed.lensed_get_conv_shape(h) else "narrow"
-    n_traced = cfg.n_traced()                               # m_d, the required set
-    assert n_traced <= lensed.lensed_num_traced(h)
-    n_counted = int(cfg.H * cfg.W if cfg.mask is None else cfg.mask.sum())
-
-    params = cfg.batch(B, stream=2 + rank)                 # this rank's shard of the global batch
-    p_dev = torch.from_numpy(params).to(dev)
-    logl = torch.empty(B, dtype=torch.float32, device=dev)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
-    stream = torch.cuda.current_stream()
 
     def barrier():
         torch.cuda.synchronize()
@@ -231,30 +341,22 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    def max_over_ranks(x):
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+    bench = Bench(lensed, torch, args.config, B, local, rank, args)
+    h, params, logl = bench.h, bench.params, bench.logl
+    n_traced = bench.n_traced
+
     # ---------------------------------------------------------------- device-resident timing
-    for _ in range(args.warmup):
-        lensed.lensed_loglike(h, p_dev, logl)
-    lensed.lensed_set_profiling(h, True)
-    lensed.lensed_reset_profile(h)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
     clocks = ClockSampler(local)
-    t_wall0 = time.perf_counter()
-    for a, b in ev:
-        flush.zero_()                                       # L2 flush between timed iterations (untimed)
-        a.record(stream)
-        lensed.lensed_loglike(h, p_dev, logl)
-        b.record(stream)
-    barrier()
-    t_wall1 = time.perf_counter()
+    ms_steps, phase_ms, phase_n, t_wall0, t_wall1 = bench.run(args.steps, args.warmup, flush, barrier)
     clock_info = clocks.stop(t_wall0, t_wall1)
-    ms_steps = [a.elapsed_time(b) for a, b in ev]
-    phase_ms, phase_n = lensed.lensed_get_profile(h)
-    lensed.lensed_set_profiling(h, False)
-    t_dev = torch.tensor([sum(ms_steps)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t_dev, op=dist.ReduceOp.MAX)
-    total_ms = float(t_dev.item())
+    total_ms = max_over_ranks(sum(ms_steps))
     value = world * B * args.steps / (total_ms * 1e-3)
     rays_per_s = value * n_traced * len(cfg.quad)
 
@@ -266,46 +368,43 @@ def main():
     t0 = time.perf_counter()
     for _ in range(args.steps):
         lensed.lensed_loglike_host(h, p_host, l_host)       # H2D + path + D2H + stream sync, every step
-    t_e2e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
-    e2e_value = world * B * args.steps / float(t_e2e.item())
+    e2e_value = world * B * args.steps / max_over_ranks(time.perf_counter() - t0)
     assert np.array_equal(l_host.numpy(), logl.cpu().numpy())
 
     # ------------------------------------------------------------------------------ roofline
-    fpr = flops_per_ray(cfg.models)
-    per_launch = {   # algorithmic flops of one launch of each kernel, averaged over its launches
-        "trace": fpr * len(cfg.quad) * n_traced * B * args.steps / max(phase_n["trace"], 1),
-        "conv": flops_per_conv_pixel(cfg) * n_counted * B * args.steps / max(phase_n["conv"], 1),
-    }
+    per_launch = bench.flop_model(args.steps, phase_n)
+    kern = bench.kernels(args.steps, phase_ms, phase_n)
     dom = max(("trace", "conv"), key=lambda k: phase_ms[k])
     avg_ms = phase_ms[dom] / max(phase_n[dom], 1)
     achieved = per_launch[dom] / (avg_ms * 1e-3) / 1e12
-    kern = {k: {"ms_per_step": phase_ms[k] / args.steps, "launches_per_step": phase_n[k] / args.steps,
-                "tflops": (per_launch[k] * phase_n[k] / (phase_ms[k] * 1e-3) / 1e12) if k in per_launch and phase_ms[k] > 0 else None}
-            for k in lensed.PHASES}
     try:
         measured_ffma = lensed.lensed_fma_peak(local, 2048)
     except lensed.LensedError:
         measured_ffma = None
-    traffic = None
+    traffic = traffic_src = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per vector from the ncu capture
     if os.path.exists(tpath):
         with open(tpath) as fh:
             t = json.load(fh).get("%s:%d" % (dom, args.config))
             if t:                                            # per vector in the capture -> per launch of this run
                 traffic = int(t["bytes_per_vector"] * B * args.steps / max(phase_n[dom], 1))
+                traffic_src = t["capture"]
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS,
                 "unit": "TFLOP/s", "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": traffic,
+                "traffic_source": traffic_src,
                 "peak_source": "nominal 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)",
                 "measured_ffma_tflops": measured_ffma,
                 "frac_of_measured_ffma": achieved / measured_ffma if measured_ffma else None,
                 "whole_step_tflops": (per_launch["trace"] * phase_n["trace"] + per_launch["conv"] * phase_n["conv"])
                 / (total_ms * 1e-3) / 1e12 if world == 1 else None,
-                "flops_per_ray": fpr, "flops_per_conv_pixel": flops_per_conv_pixel(cfg), "kernels": kern}
+                "flops_per_ray": flops_per_ray(cfg.models), "flops_per_conv_pixel": flops_per_conv_pixel(cfg),
+                "kernels": kern}
+    if roofline["whole_step_tflops"]:
+        roofline["whole_step_frac"] = roofline["whole_step_tflops"] / NOMINAL_FP32_TFLOPS
 
     # -------------------------------------------------------------- batch sweep (config 4 only)
     sweep = None
+    stream = torch.cuda.current_stream()
     if args.config == 4 and not args.no_sweep and world == 1:
         sweep = []
         for Bs in (256, 1024, 4096, 16384):
@@ -322,11 +421,22 @@ def main():
     # ---------------------------------------------------------------------------- cpu baseline
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, cores, n, dt = time_oracle(cfg, image, weight, params, 15.0)
+        v, cores, n, dt = time_oracle(cfg, bench.image, bench.weight, params, 15.0)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": "%d of the %d vectors, full image, %.1f s" % (n, B, dt)}
+    gpu_launches = int(sum(phase_n.values()))
+    bench.close()
 
-    lensed.lensed_destroy(h)
+    # ------------------------------- the other configs and the sampler row (short, rank 0, N = 1)
+    per_config = nested = None
+    if args.config == DEFAULT_CONFIG and not args.no_extras and world == 1 and not args.batch:
+        per_config = []
+        for c, steps in ((0, 20), (1, 20), (2, 10), (3, 5), (5, 10)):
+            b = Bench(lensed, torch, c, synth.get_config(c).B, local, rank, args)
+            per_config.append(b.summary(steps, 3, flush))
+            b.close()
+        nested = nested_row(lensed, torch, local)
+
     if rank == 0:
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -335,16 +445,19 @@ def main():
             "config": {"workload": workload_name(cfg, B), "batch_per_gpu": B, "global_batch": B * world,
                        "traced_pixels": n_traced, "rays_per_step": B * world * n_traced * len(cfg.quad),
                        "parallelism": "batch-sharded x%d, no collective" % world,
-                       "tracer": tracer_kind, "conv_shape": conv_shape,
+                       "tracer": bench.tracer_kind, "conv_shape": bench.conv_shape,
                        "timing": "CUDA events per step, L2 flushed (256 MB write) between steps, max over ranks"},
             "rays_per_sec": rays_per_s,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(params.nbytes),
                     "d2h_bytes_per_step": int(B * 4)},
-            "gpu_launches": int(sum(phase_n.values())),
+            "gpu_launches": gpu_launches,
             "clocks": clock_info, "roofline": roofline, "cpu_baseline": cpu,
         }
         if sweep is not None:
             out["sweep"] = sweep
+        if per_config is not None:
+            out["per_config"] = per_config
+            out["nested_sampling"] = nested
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
