@@ -64,6 +64,7 @@ struct lensed_handle {
     float *d_derived = nullptr; size_t cap_derived = 0;
     double *d_derived64 = nullptr; size_t cap_derived64 = 0;
     uint32_t *d_fixmask = nullptr; size_t cap_fixmask = 0;
+    int *d_order = nullptr; size_t cap_order = 0;          // tracer block order (prep.cu order_kernel)
     uint2 *d_queue = nullptr; size_t cap_queue = 0;      // refine.cu: flagged pixels of one chunk
     unsigned *d_queue_count = nullptr;
     unsigned long long *d_refined = nullptr;   // pixels refined in FP64 since the last profile reset
@@ -350,14 +351,20 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
                 h->refine_gain > 0.0 ? h->refine_gain : (double)INFINITY,
                 h->rule_symmetric && h->static_tracer ? h->fgx_tau : 0.0, h->rule_radius,
                 h->scale, h->zp, 0.5 * (h->W - 1), 0.5 * (h->H - 1)};
+    bool has_sie = false;                     // only the SIE has per-mode code paths worth sorting for
+    for (int m = 0; m < prog.n_lens; ++m) has_sie = has_sie || prog.lens_kind[m] == K_SIE;
+    const bool sorted = has_sie && npix > 0 && B > 1;
+    if (sorted && (s = grow(h, &h->d_order, &h->cap_order, (size_t)B, st)) != LENSED_OK) return s;
     if ((s = timed_begin(h, PH_PREP, st)) != LENSED_OK) return s;
     CU(h, launch_prep(prog, pa, st));
+    if (sorted) CU(h, launch_order(h->d_derived, prog.D, B, Bc, h->d_order, st));
     if ((s = timed_end(h, st)) != LENSED_OK) return s;
 
     for (int b0 = 0; b0 < B; b0 += Bc) {
         const int nb = std::min(Bc, B - b0);
         if (npix > 0) {
             TraceArgs ta{};
+            ta.order = sorted ? h->d_order + b0 : nullptr;
             ta.derived = h->d_derived + (size_t)b0 * prog.D;
             ta.pix = render ? h->d_pix_all : h->d_pix_ll;
             ta.quad = h->d_quad;
@@ -944,7 +951,7 @@ void lensed_destroy(lensed_handle *h)
         delete h->shared;
     }
     cudaFree(h->d_derived); cudaFree(h->d_L); cudaFree(h->d_partial);
-    cudaFree(h->d_derived64); cudaFree(h->d_fixmask); cudaFree(h->d_refined);
+    cudaFree(h->d_derived64); cudaFree(h->d_fixmask); cudaFree(h->d_order); cudaFree(h->d_refined);
     cudaFree(h->d_queue); cudaFree(h->d_queue_count);
     cudaFree(h->d_stage_in); cudaFree(h->d_stage_out);
     delete h;

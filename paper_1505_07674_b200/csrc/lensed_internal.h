@@ -103,6 +103,9 @@ struct PrepArgs {
 
 struct TraceArgs {
     const float *derived;  // [.][D], already offset to the chunk's first vector
+    const int *order;      // [nvec] or NULL: block row y works on vector order[y] of the chunk -- the chunk's
+                           // vectors sorted by SIE mode (prep.cu order_kernel), so that the blocks resident at
+                           // one time run the same specialised code path (instruction cache)
     const uint32_t *pix;   // [npix] packed (row << 16) | column
     const float4 *quad;    // [nq_pad] (xi, eta, w, w - w'), zero-weight padding up to a multiple of R (even);
                            // w' = embedded rule of lensed_set_error_rule (0 before it is set)
@@ -160,6 +163,8 @@ struct FinalArgs {
 
 // launchers (each returns the cudaGetLastError of its launch)
 cudaError_t launch_prep(const Program &prog, const PrepArgs &a, cudaStream_t st);
+// order[c * Bc + i] = index within chunk c of its i-th vector by (SIE mode, index); invalid vectors last
+cudaError_t launch_order(const float *derived, int D, int B, int Bc, int *order, cudaStream_t st);
 // allow_static: use the compile-time-specialised kernel when the list has one (trace.cu)
 cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nvec, bool allow_static, cudaStream_t st);
 inline int trace_blocks_per_vector(const TraceArgs &a) { return (a.npix + a.pix_per_block - 1) / a.pix_per_block; }

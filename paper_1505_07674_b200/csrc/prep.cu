@@ -254,12 +254,70 @@ __global__ void __launch_bounds__(kMaxModels * kPrepVec) prep_kernel(Program pro
     }
 }
 
+
+// Block order of the ray tracer: the vectors of each batch chunk sorted by (SIE mode, index),
+// vectors outside the model domain last.  The specialised tracers hold one straight-line copy of
+// the ray loop per mode (trace_static.cuh); with the vectors of a launch in arbitrary order the
+// blocks resident at one time run all six copies and miss the instruction cache (HST config:
+// `no_instruction` 2.8 stall cycles per issue, profiles/r2c.md).  Stable counting sort, one block
+// per chunk: the order is a function of the inputs.  It only changes which block works on which
+// vector -- every vector's result is what it was.
+constexpr int kOrderKeys = 7;                   // SIE modes 0..5, 6 = invalid
+__global__ void __launch_bounds__(256) order_kernel(const float *derived, int D, int B, int Bc, int *order)
+{
+    __shared__ int s_run[kOrderKeys + 1];       // next free slot per key
+    __shared__ int s_warp[8][kOrderKeys];       // per warp, per key: count within the current tile
+    const int b0 = blockIdx.x * Bc, n = min(Bc, B - b0);
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    auto key_of = [&](int i) {
+        const float *hdr = derived + (size_t)(b0 + i) * D;
+        return hdr[0] != 0.0f ? min(max((int)hdr[1], 0), kOrderKeys - 2) : kOrderKeys - 1;
+    };
+    if (t <= kOrderKeys) s_run[t] = 0;
+    __syncthreads();
+    for (int i = t; i < n; i += 256) atomicAdd(&s_run[key_of(i) + 1], 1);      // totals (integers: order-free)
+    __syncthreads();
+    if (t == 0)
+        for (int k = 1; k <= kOrderKeys; ++k) s_run[k] += s_run[k - 1];        // s_run[k] = first slot of key k
+    __syncthreads();
+    for (int base = 0; base < n; base += 256) {
+        const int i = base + t;
+        const int key = i < n ? key_of(i) : kOrderKeys;
+        int rank = 0;
+#pragma unroll
+        for (int k = 0; k < kOrderKeys; ++k) {
+            const unsigned m = __ballot_sync(0xffffffffu, key == k);
+            if (key == k) rank = __popc(m & ((1u << lane) - 1u));
+            if (lane == 0) s_warp[warp][k] = __popc(m);
+        }
+        __syncthreads();
+        if (key < kOrderKeys) {
+            int off = s_run[key] + rank;
+            for (int w = 0; w < warp; ++w) off += s_warp[w][key];
+            order[b0 + off] = i;
+        }
+        __syncthreads();
+        if (t < kOrderKeys) {
+            int c = 0;
+            for (int w = 0; w < 8; ++w) c += s_warp[w][t];
+            s_run[t] += c;
+        }
+        __syncthreads();
+    }
+}
+
 }  // namespace
 
 cudaError_t launch_prep(const Program &prog, const PrepArgs &a, cudaStream_t st)
 {
     const dim3 block(kMaxModels, kPrepVec);
     prep_kernel<<<(a.B + kPrepVec - 1) / kPrepVec, block, 0, st>>>(prog, a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_order(const float *derived, int D, int B, int Bc, int *order, cudaStream_t st)
+{
+    order_kernel<<<(B + Bc - 1) / Bc, 256, 0, st>>>(derived, D, B, Bc, order);
     return cudaGetLastError();
 }
 

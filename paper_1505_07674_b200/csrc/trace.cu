@@ -6,7 +6,7 @@
 //   I   = sum_src I_S(y_k) + sum_fg I_L(x_k) + sky           PAPER.md:59-63  eq. 2
 //   L_i = sum_k w_k I                                        PAPER.md:155-157 eq. 14
 //
-// Layout.  blockIdx.y = parameter vector, blockIdx.x = chunk of the traced-pixel list.  A
+// Layout.  blockIdx.y -> parameter vector (TraceArgs::order), blockIdx.x = chunk of the traced-pixel list.  A
 // thread owns one pixel at a time and carries R = 2 NP rays (rule points) in registers, as
 // NP packed FP32 pairs (f32x2.cuh), through the model list.  No per-ray value ever goes to
 // memory; one float per traced pixel is written.
@@ -73,14 +73,15 @@ __global__ void __launch_bounds__(kTraceThreads, LENSED_MINB_GENERIC) trace_kern
 {
     constexpr int R = 2 * NP;
     extern __shared__ float4 smem4[];
-    const TraceBlock tb = trace_prologue(prog, a, smem4);
+    const int vec = trace_vector(a);
+    const TraceBlock tb = trace_prologue(prog, a, smem4, vec);
     if (!tb.valid) {
-        if (!ERR && a.fixmask) a.fixmask[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = 0;
+        if (!ERR && a.fixmask) a.fixmask[((size_t)vec * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = 0;
         if (ERR) {
             const int base = blockIdx.x * a.pix_per_block, end = min(base + a.pix_per_block, a.npix);
             for (int ip = base + threadIdx.x; ip < end; ip += kTraceThreads) {
                 const uint32_t rc = a.pix[ip];
-                a.err[(size_t)blockIdx.y * a.H * a.W + (size_t)(rc >> 16) * a.W + (rc & 0xffffu)] = nanf("");
+                a.err[(size_t)vec * a.H * a.W + (size_t)(rc >> 16) * a.W + (rc & 0xffffu)] = nanf("");
             }
         }
         return;
@@ -89,7 +90,7 @@ __global__ void __launch_bounds__(kTraceThreads, LENSED_MINB_GENERIC) trace_kern
     const float *stab = tb.stab;
     const int nq = a.nq_pad;
     const int mode = (int)sder[0].y;
-    float *Lb = a.L + (size_t)blockIdx.y * a.l_stride;
+    float *Lb = a.L + (size_t)vec * a.l_stride;
 
     const int base = blockIdx.x * a.pix_per_block;
     const int end = min(base + a.pix_per_block, a.npix);
@@ -162,11 +163,11 @@ __global__ void __launch_bounds__(kTraceThreads, LENSED_MINB_GENERIC) trace_kern
 #pragma unroll
             for (int k = 0; k < NP; ++k) acc = fma2(w[k], r.I[k], acc);
         }
-        if (ERR) a.err[(size_t)blockIdx.y * a.H * a.W + (size_t)row * a.W + col] = fabsf(lo2(acc) + hi2(acc));
+        if (ERR) a.err[(size_t)vec * a.H * a.W + (size_t)row * a.W + col] = fabsf(lo2(acc) + hi2(acc));
         else store_pixel(a, Lb, row, col, (lo2(acc) + hi2(acc)) + tb.sky);
         if (flag) flags |= 1u << ((ip - base) >> 8);
     }
-    if (!ERR && a.fixmask) a.fixmask[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = flags;
+    if (!ERR && a.fixmask) a.fixmask[((size_t)vec * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = flags;
 }
 
 }  // namespace

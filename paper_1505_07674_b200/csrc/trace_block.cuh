@@ -30,8 +30,11 @@ struct TraceBlock {
     bool valid;
 };
 
+// the chunk-local parameter vector of this block (TraceArgs::order)
+__device__ __forceinline__ int trace_vector(const TraceArgs &a) { return a.order ? a.order[blockIdx.y] : (int)blockIdx.y; }
+
 // Must be called by all threads of the block; ends with a barrier.
-__device__ __forceinline__ TraceBlock trace_prologue(const Program &prog, const TraceArgs &a, float4 *smem4)
+__device__ __forceinline__ TraceBlock trace_prologue(const Program &prog, const TraceArgs &a, float4 *smem4, int vec)
 {
     float4 *sder = smem4;
     float *stab = reinterpret_cast<float *>(smem4 + prog.D / 4);
@@ -39,7 +42,7 @@ __device__ __forceinline__ TraceBlock trace_prologue(const Program &prog, const 
     const int n_slots = 1 + prog.n_lens + prog.n_light;
     float *sw = stab + (size_t)n_slots * 2 * nq;
     {
-        const float4 *g = reinterpret_cast<const float4 *>(a.derived + (size_t)blockIdx.y * prog.D);
+        const float4 *g = reinterpret_cast<const float4 *>(a.derived + (size_t)vec * prog.D);
         for (int i = threadIdx.x; i < prog.D / 4; i += kTraceThreads) sder[i] = g[i];
     }
     __syncthreads();

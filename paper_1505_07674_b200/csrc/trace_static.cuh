@@ -82,7 +82,7 @@ __device__ __forceinline__ float fg_expansion(const float4 *d, const FgMoments &
 }
 
 template <int NP, class S, int MODE>
-__device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArgs &a, const TraceBlock &tb, float *Lb)
+__device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArgs &a, const TraceBlock &tb, float *Lb, int vec)
 {
     constexpr int R = 2 * NP;
     constexpr int NL = S::n_lens, NPOS = S::n_pos;
@@ -221,7 +221,7 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
         for (int i = 0; i < S::n_ss; ++i)
             if (rmin[i] < sder[(prog.light_off[i] >> 2) + 2].w) flags |= bit;
     }
-    if (a.fixmask) a.fixmask[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = flags;
+    if (a.fixmask) a.fixmask[((size_t)vec * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = flags;
 }
 
 // MINB = resident blocks per SM the register budget is cut for (3 -> 80 registers, 2 -> 128):
@@ -230,9 +230,10 @@ template <int NP, class S, int MINB>
 __global__ void __launch_bounds__(kTraceThreads, MINB * (256 / kTraceThreads)) trace_static_kernel(Program prog, TraceArgs a)
 {
     extern __shared__ float4 smem4[];
-    const TraceBlock tb = trace_prologue(prog, a, smem4);
+    const int vec = trace_vector(a);
+    const TraceBlock tb = trace_prologue(prog, a, smem4, vec);
     if (!tb.valid) {
-        if (a.fixmask) a.fixmask[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = 0;
+        if (a.fixmask) a.fixmask[((size_t)vec * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = 0;
         return;
     }
     if constexpr (S::direct) {
@@ -274,17 +275,17 @@ __global__ void __launch_bounds__(kTraceThreads, MINB * (256 / kTraceThreads)) t
         }
         __syncthreads();
     }
-    float *Lb = a.L + (size_t)blockIdx.y * a.l_stride;
+    float *Lb = a.L + (size_t)vec * a.l_stride;
     if constexpr (S::n_sie == 0) {
-        trace_pixels<NP, S, 0>(prog, a, tb, Lb);
+        trace_pixels<NP, S, 0>(prog, a, tb, Lb, vec);
     } else {
         switch ((int)tb.sder[0].y) {              // SieMode of the vector (prep.cu), block-uniform
-        case 0: trace_pixels<NP, S, 0>(prog, a, tb, Lb); break;
-        case 1: trace_pixels<NP, S, 1>(prog, a, tb, Lb); break;
-        case 2: trace_pixels<NP, S, 2>(prog, a, tb, Lb); break;
-        case 3: trace_pixels<NP, S, 3>(prog, a, tb, Lb); break;
-        case 4: trace_pixels<NP, S, 4>(prog, a, tb, Lb); break;
-        default: trace_pixels<NP, S, 5>(prog, a, tb, Lb); break;
+        case 0: trace_pixels<NP, S, 0>(prog, a, tb, Lb, vec); break;
+        case 1: trace_pixels<NP, S, 1>(prog, a, tb, Lb, vec); break;
+        case 2: trace_pixels<NP, S, 2>(prog, a, tb, Lb, vec); break;
+        case 3: trace_pixels<NP, S, 3>(prog, a, tb, Lb, vec); break;
+        case 4: trace_pixels<NP, S, 4>(prog, a, tb, Lb, vec); break;
+        default: trace_pixels<NP, S, 5>(prog, a, tb, Lb, vec); break;
         }
     }
 }
