@@ -187,9 +187,9 @@ class Bench:
         if args is not None and args.interpreter:
             lensed.lensed_set_static_tracer(self.h, 0)
         if args is not None and args.conv_shape != "auto":
-            lensed.lensed_set_conv_shape(self.h, args.conv_shape == "wide")
+            lensed.lensed_set_conv_shape(self.h, lensed.CONV_SHAPES.index(args.conv_shape))
         self.tracer_kind = "static" if lensed.lensed_get_static_tracer(self.h) == 1 else "interpreter"
-        self.conv_shape = "wide" if lensed.lensed_get_conv_shape(self.h) else "narrow"
+        self.conv_shape = lensed.CONV_SHAPES[lensed.lensed_get_conv_shape(self.h)]
         self.n_traced = cfg.n_traced()                       # m_d, the required set
         assert self.n_traced <= lensed.lensed_num_traced(self.h)
         self.n_counted = int(cfg.H * cfg.W if cfg.mask is None else cfg.mask.sum())
@@ -307,8 +307,8 @@ def main():
     ap.add_argument("--no-extras", action="store_true",
                     help="skip the per-config rows (configs 0-3, 5) and the nested-sampling row")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--conv-shape", default="auto", choices=("auto", "wide", "narrow"),
-                    help="convolution block shape (include/lensed.h); auto = what lensed_create picks")
+    ap.add_argument("--conv-shape", default="auto", choices=("auto", "wide", "narrow", "strip"),
+                    help="convolution shape (include/lensed.h); auto = what lensed_create picks")
     ap.add_argument("--interpreter", action="store_true",
                     help="run the interpreting tracer instead of the compile-time specialised one")
     args = ap.parse_args()

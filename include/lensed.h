@@ -225,13 +225,19 @@ lensed_status lensed_set_fg_expansion(lensed_handle *h, double tau);
 lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes);
 long long lensed_frame_bytes(const lensed_handle *h);
 
-/* Convolution block shape.  The convolution exists in two shapes (same arithmetic): "wide",
- * 256 threads on 64 x 128 output tiles, one block per SM, and "narrow", 128 threads on 64 x 64
- * tiles, two blocks per SM (small or masked images, small PSFs).  lensed_create picks one;
- * lensed_set_conv_shape(h, 1 / 0) forces wide / narrow (it rebuilds the tile lists and the frame
- * layout and synchronises the device; LENSED_EUNSUPPORTED if the PSF is too large for the narrow
- * shape's shared memory).  lensed_get_conv_shape: 1 / 0, -1 for NULL.  Results do not depend on
- * the shape beyond the order of the per-tile chi-square partials.
+/* Convolution shape.  The convolution exists in three shapes (same per-pixel arithmetic):
+ *   2 "strip"   one block of 8 INDEPENDENT warps per SM, each on its own 16 x 64 output strip with
+ *               its own shared-memory stage: nothing is lost at block barriers, masked images skip
+ *               whole strips; needs 8 stages of (16 + psf_h - 1) x (64 + 4 ceil(psf_w / 4)) floats
+ *               (PSFs up to about 37 rows)
+ *   1 "wide"    256 threads on 64 x 128 output tiles, one block per SM: any PSF
+ *   0 "narrow"  128 threads on 64 x 64 tiles, two blocks per SM: small or masked images
+ * lensed_create picks one (wide for full images; narrow or strip where a mask or a small image
+ * makes their tile list compute at least 15 % fewer pixels); lensed_set_conv_shape(h, shape) forces one (it
+ * rebuilds the tile lists and the frame layout and synchronises the device; EINVAL for another
+ * value, LENSED_EUNSUPPORTED if the PSF is too large for that shape's shared memory).
+ * lensed_get_conv_shape: 2 / 1 / 0, -1 for NULL.  Rendered pixels do not depend on the shape at
+ * all; logL only through the order in which the per-tile chi-square partials are summed.
  *
  * PSF taps.  The taps of a handle normally sit in a 60 KB pool of constant memory shared by
  * the live handles of a device ((psf_h + 1) * 4 ceil(psf_w / 4) * 8 bytes each: 8 KB for 31 x 31,
@@ -239,7 +245,7 @@ long long lensed_frame_bytes(const lensed_handle *h);
  * and runs a variant of the convolution that reads them from there (same results, somewhat
  * slower); lensed_uses_global_taps tells (1 / 0, -1 for NULL).
  * lensed_debug_force_global_taps(1) makes every later lensed_create take that path (tests).   */
-lensed_status lensed_set_conv_shape(lensed_handle *h, int wide);
+lensed_status lensed_set_conv_shape(lensed_handle *h, int shape);
 int lensed_get_conv_shape(const lensed_handle *h);
 int lensed_uses_global_taps(const lensed_handle *h);
 void lensed_debug_force_global_taps(int on);

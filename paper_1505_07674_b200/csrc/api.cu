@@ -51,7 +51,7 @@ struct lensed_handle {
     int n_sm = 1;
     int tap_off = -1, tap_pairs = 0; // this handle's range of the constant tap pool
     unsigned long long *d_gtaps = nullptr;   // the taps in global memory instead, when the pool was full
-    bool wide = true;               // convolution block shape (conv.cu "Two block shapes")
+    int shape = 1;                  // convolution shape: 0 narrow, 1 wide, 2 strip (conv.cu)
     std::vector<uint8_t> counted;   // host copy of the counted-pixel map (lensed_set_conv_shape rebuilds the tiles)
 
     // device, immutable after create
@@ -245,11 +245,11 @@ bool g_force_global_taps = false;     // lensed_debug_force_global_taps (tests)
 // (its layout changes).  Loglike tiles start at the corner of the counted pixels' bounding box
 // (x rounded down to a 16-byte boundary for cp.async): a mask that is not tile-aligned costs
 // fewer tiles.  The render grid starts at (0, 0).
-lensed_status build_tiles(lensed_handle *h, bool wide)
+lensed_status build_tiles(lensed_handle *h, int shape)
 {
     const int H = h->H, W = h->W;
-    h->wide = wide;
-    conv_tile_shape(wide, &h->tile_w, &h->tile_h);
+    h->shape = shape;
+    conv_tile_shape(shape, &h->tile_w, &h->tile_h);
     std::vector<uint8_t> all((size_t)H * W, 1);
     std::vector<uint32_t> tiles_ll, tiles_all;
     int x0 = W, y0 = H;
@@ -275,28 +275,31 @@ lensed_status build_tiles(lensed_handle *h, bool wide)
     return upload(h, &h->d_tiles_all, tiles_all.data(), tiles_all.size());
 }
 
-// Block shape lensed_create picks.  Measured on the configs (profiles/r2b.md): with full tiles
-// the wide shape is as fast (small PSFs) or faster (31 x 31: 32.9 against 35.7 ms per 4096
-// Euclid vectors); the narrow one wins where its 64-column tiles cover a masked image with
-// fewer pixels (SLACS annulus: 9 x 4096 against 6 x 8192 pixels per vector, 2.58 -> 2.21 ms).
-bool default_wide(const lensed_handle *h)
+// Shape lensed_create picks, from the pixels each shape's tile list computes (tiles x tile area)
+// and what was measured on the configs (profiles/r2b.md, r2e.md).  With full tiles the wide shape
+// is the fastest (31 x 31 PSF, 4096 Euclid vectors: wide 32.5, narrow 35.0, strip 35.3 ms: the
+// strip shape's unsynchronised warps miss the constant cache on the taps more often than a
+// block's lock-step warps).  A masked or small image goes to the shape that computes at least
+// 15 % fewer pixels: narrow's 64-column tiles, or the 16 x 64 strips (SLACS annulus: 25 strips =
+// 25.6 k pixels against 8 narrow tiles = 32.8 k; 1.72 against 2.10 ms per 4096 vectors).
+int default_shape(const lensed_handle *h)
 {
-#ifdef LENSED_CONV_FORCE_WIDE
-    return LENSED_CONV_FORCE_WIDE != 0;
+#ifdef LENSED_CONV_FORCE_SHAPE
+    return LENSED_CONV_FORCE_SHAPE;
 #endif
-    if (!conv_narrow_fits(h->KH, h->NC)) return true;
-    long long px[2];
-    for (int wide = 0; wide < 2; ++wide) {
+    long long px[3];
+    for (int shape = 0; shape < 3; ++shape) {
         int tw, th, ny, nx, x0 = h->W, y0 = h->H;
-        conv_tile_shape(wide != 0, &tw, &th);
+        conv_tile_shape(shape, &tw, &th);
         for (int i = 0; i < h->H; ++i)
             for (int j = 0; j < h->W; ++j)
                 if (h->counted[(size_t)i * h->W + j]) { x0 = std::min(x0, j); y0 = std::min(y0, i); }
         std::vector<uint32_t> tiles;
         tile_list(h->counted, h->H, h->W, tw, th, x0 < h->W ? x0 / 4 * 4 : 0, y0 < h->H ? y0 : 0, tiles, &ny, &nx);
-        px[wide] = (long long)tiles.size() * tw * th;
+        px[shape] = conv_shape_fits(h->KH, h->NC, shape) ? (long long)tiles.size() * tw * th : (1LL << 60);
     }
-    return !(px[0] * 100 <= px[1] * 85);
+    const int block = px[0] * 100 <= px[1] * 85 ? 0 : 1;
+    return px[2] * 100 <= px[block] * 85 ? 2 : block;
 }
 
 // Pixels of the traced list one tracer block walks: it amortises its prologue (constants +
@@ -336,7 +339,7 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
         // pad cells no pixel clamps to (tile overhang) are read, never written: keep them zero
         if ((s = grow(h, &h->d_L, &h->cap_L, (size_t)Bc * HWp, st)) != LENSED_OK) return s;
         CU(h, cudaMemsetAsync(h->d_L, 0, (size_t)Bc * HWp * sizeof(float), st));
-        CU(h, conv_make_tensor_map(h->tmap_L, h->d_L, h->Wp, h->Hp, Bc, h->KH, h->NC, h->wide));
+        CU(h, conv_make_tensor_map(h->tmap_L, h->d_L, h->Wp, h->Hp, Bc, h->KH, h->NC, h->shape));
     }
     if (!render && (s = grow(h, &h->d_partial, &h->cap_partial, (size_t)B * std::max(n_tiles, 1), st)) != LENSED_OK)
         return s;
@@ -401,7 +404,7 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
             ca.D = prog.D;
             ca.H = h->H; ca.W = h->W; ca.Wp = h->Wp; ca.KH = h->KH; ca.KW = h->KW; ca.NC = h->NC;
             ca.n_tiles = n_tiles; ca.nb = nb;
-            ca.tap_off = h->d_gtaps ? 0 : h->tap_off; ca.gtaps = h->d_gtaps; ca.wide = h->wide ? 1 : 0;
+            ca.tap_off = h->d_gtaps ? 0 : h->tap_off; ca.gtaps = h->d_gtaps; ca.shape = h->shape;
             ca.ox = render ? 0 : h->ox_ll; ca.oy = render ? 0 : h->oy_ll;
             if ((s = timed_begin(h, PH_CONV, st)) != LENSED_OK) return s;
             CU(h, launch_conv(ca, h->tmap_L, render, h->n_sm, st));
@@ -502,37 +505,40 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     // model list -> program
     Program &pg = h->prog;
     pg.n_models = n_models;
-    int P = 0, D = kHeaderFloats;
+    int P = 0;
     for (int m = 0; m < n_models; ++m) {
         const int k = models[m];
         if (k < 0 || k >= K_COUNT) { delete h->shared; delete h; return fail(nullptr, LENSED_EINVAL, "models[%d] = %d is not a lensed_kind", m, k); }
         pg.kind[m] = (uint8_t)k;
         pg.par_off[m] = (uint16_t)P;
-        pg.der_off[m] = (uint16_t)D;
-        if (k <= K_SHEAR) { pg.lens_kind[pg.n_lens] = (uint8_t)k; pg.lens_off[pg.n_lens++] = (uint16_t)D; }
-        else { pg.light_kind[pg.n_light] = (uint8_t)k; pg.light_off[pg.n_light++] = (uint16_t)D; }
         P += kind_num_params(k);
-        D += kind_num_derived(k);
     }
-    pg.P = P; pg.D = D;
     // canonical order (stable within a kind): lenses shear, SIE, SIS, point mass -- the first
     // shear initialises alpha in the tracer; lights source Sersic, source Gaussian, foreground
     // Sersic, foreground Gaussian, sky.  The sums over lenses and over lights do not depend on
-    // the order beyond rounding; the static tracer kernels index the lists by it (trace_static.cuh).
+    // the order beyond rounding.  The derived vector is laid out in that order too (header,
+    // lenses, lights), so a static tracer signature fixes every block's offset at compile time
+    // (trace_static.cuh TraceSig::lens_off4 / light_off4).
+    int D = kHeaderFloats;
     {
         static const int lens_order[] = {K_SHEAR, K_SIE, K_SIS, K_POINT};
         static const int light_order[] = {K_SRC_SERSIC, K_SRC_GAUSS, K_FG_SERSIC, K_FG_GAUSS, K_SKY};
-        uint8_t kk[kMaxModels]; uint16_t oo[kMaxModels]; int n = 0;
         for (int kind : lens_order)
-            for (int m = 0; m < pg.n_lens; ++m)
-                if (pg.lens_kind[m] == kind) { kk[n] = pg.lens_kind[m]; oo[n++] = pg.lens_off[m]; }
-        for (int m = 0; m < pg.n_lens; ++m) { pg.lens_kind[m] = kk[m]; pg.lens_off[m] = oo[m]; }
-        n = 0;
+            for (int m = 0; m < n_models; ++m)
+                if (pg.kind[m] == kind) {
+                    pg.der_off[m] = (uint16_t)D;
+                    pg.lens_kind[pg.n_lens] = (uint8_t)kind; pg.lens_off[pg.n_lens++] = (uint16_t)D;
+                    D += kind_num_derived(kind);
+                }
         for (int kind : light_order)
-            for (int m = 0; m < pg.n_light; ++m)
-                if (pg.light_kind[m] == kind) { kk[n] = pg.light_kind[m]; oo[n++] = pg.light_off[m]; }
-        for (int m = 0; m < pg.n_light; ++m) { pg.light_kind[m] = kk[m]; pg.light_off[m] = oo[m]; }
+            for (int m = 0; m < n_models; ++m)
+                if (pg.kind[m] == kind) {
+                    pg.der_off[m] = (uint16_t)D;
+                    pg.light_kind[pg.n_light] = (uint8_t)kind; pg.light_off[pg.n_light++] = (uint16_t)D;
+                    D += kind_num_derived(kind);
+                }
     }
+    pg.P = P; pg.D = D;
     h->static_tracer = trace_has_static(pg);
 
     // rule: weights to unit sum in double, padded with zero-weight points to a multiple of R
@@ -648,7 +654,7 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     h->h_quad = hq;
     CREATE_FAIL(upload(h, &h->d_pix_ll, pix_ll.data(), pix_ll.size()));
     CREATE_FAIL(upload(h, &h->d_pix_all, pix_all.data(), pix_all.size()));
-    CREATE_FAIL(build_tiles(h, default_wide(h)));
+    CREATE_FAIL(build_tiles(h, default_shape(h)));
 #undef CREATE_FAIL
     *out = h;
     return LENSED_OK;
@@ -683,7 +689,7 @@ lensed_status lensed_clone(const lensed_handle *src, lensed_handle **out)
     const unsigned zero32 = 0;
     CLONE_FAIL(upload(h, &h->d_refined, &zero, 1));
     CLONE_FAIL(upload(h, &h->d_queue_count, &zero32, 1));
-    CLONE_FAIL(build_tiles(h, src->wide));
+    CLONE_FAIL(build_tiles(h, src->shape));
 #undef CLONE_FAIL
     *out = h;
     return LENSED_OK;
@@ -895,15 +901,17 @@ lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes)
     return LENSED_OK;
 }
 
-lensed_status lensed_set_conv_shape(lensed_handle *h, int wide)
+lensed_status lensed_set_conv_shape(lensed_handle *h, int shape)
 {
     if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
-    if (!wide && !conv_narrow_fits(h->KH, h->NC))
-        return fail(h, LENSED_EUNSUPPORTED, "a %d x %d PSF does not fit the narrow block shape", h->KH, h->KW);
-    return build_tiles(h, wide != 0);
+    if (shape < 0 || shape > 2) return fail(h, LENSED_EINVAL, "shape = %d is not 0 (narrow), 1 (wide) or 2 (strip)", shape);
+    if (!conv_shape_fits(h->KH, h->NC, shape))
+        return fail(h, LENSED_EUNSUPPORTED, "a %d x %d PSF does not fit the %s shape's shared memory", h->KH, h->KW,
+                    shape == 0 ? "narrow" : "strip");
+    return build_tiles(h, shape);
 }
 
-int lensed_get_conv_shape(const lensed_handle *h) { return h ? (h->wide ? 1 : 0) : -1; }
+int lensed_get_conv_shape(const lensed_handle *h) { return h ? h->shape : -1; }
 
 void lensed_debug_force_global_taps(int on) { g_force_global_taps = on != 0; }
 

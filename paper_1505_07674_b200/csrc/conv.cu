@@ -63,6 +63,7 @@
 #include <cuda.h>                 // CUtensorMap (types only; the encoder is fetched from the driver at run time)
 #include <cudaTypedefs.h>
 #include <algorithm>
+#include <stdlib.h>
 
 #ifndef LENSED_CONV_TMA
 #define LENSED_CONV_TMA 1         // input tiles by one cp.async.bulk.tensor per tile (0: cp.async per 16 bytes)
@@ -397,6 +398,166 @@ __global__ void __launch_bounds__(NTX * kNTY, NTX == 16 ? 1 : 2) conv_kernel(con
     }
 }
 
+
+// ---- "strip" shape: every warp is its own worker ---------------------------------------------
+// Eight ONE-WARP blocks per SM and no block-level step at all: a work item is (16 x 64 output
+// strip, parameter vector), items are ordered strip-major and split evenly over all warps of the
+// grid, and a warp owns its input stage(s) in shared memory, its mbarrier(s) and its TMA copies
+// (lane 0 issues; box = (16 + KH - 1) rows x (64 + 4 NC) floats).  One warp per block: all loop
+// indices derive from blockIdx, and the kernel is declared __launch_bounds__(32) WITHOUT a
+// minimum block count -- with (32, 8) ptxas keeps the tap pairs in vector registers (LDC + MOV
+// instead of LDCU + UR operands: 327 instead of 305 instructions per loop body, 25 % slower);
+// eight blocks per SM are resident because 8 x (registers, shared memory) fit.
+// What the block shapes above
+// lose at their barriers -- the tile prologue (wait for the copy), the epilogue (chi-square
+// reduction) and the ramps of the chunk loops, during which a block's warps all leave the FMA pipe
+// together -- a warp here loses alone, while the other warp of its scheduler keeps the pipe busy.
+// Masked images skip work per strip instead of per tile (SLACS annulus: 62 % of the computed
+// pixels are counted instead of 49 %).  The per-thread arithmetic (thread tile 4 x 8, tap pairs,
+// rotating rows, blocked summation) is the code of the block shapes, so the results agree with
+// theirs bit for bit per pixel; the chi-square partials are per strip.
+// Data d and weights w of the strip are read from global memory in the epilogue (L2 hits: the
+// same strip is reused for many vectors); stages are double buffered when 16 of them fit.
+constexpr int kSH = 16, kSW = 64;      // strip: the 4 x 8 lanes of a warp on 4 x 8 thread tiles
+constexpr int kStripWarps = 8;
+
+template <bool RENDER, bool GT>
+__global__ void __launch_bounds__(32) conv_strip_kernel(const __grid_constant__ ConvArgs a,
+                                                                         const __grid_constant__ CUtensorMap tmap)
+{
+    constexpr int NTX = 8, kGroup = 32;
+    const unsigned long long *gt = a.gtaps;
+    extern __shared__ __align__(128) float4 smem4[];
+    __shared__ __align__(8) unsigned long long s_bar[2];
+    const int lane = threadIdx.x;
+    const int IW4 = kSW / 4 + a.NC, IW = 4 * IW4;
+    const int IH = kSH + a.KH - 1 + kSlackRows;
+    const int stage_floats = (IH * IW + 31) / 32 * 32;
+    float *s_stage = reinterpret_cast<float *>(smem4);
+    if (lane == 0) {
+        mbar_init(&s_bar[0], 1);
+        mbar_init(&s_bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+
+    const long long n_items = (long long)a.n_tiles * a.nb;
+    const int lo = (int)(n_items * blockIdx.x / gridDim.x), hi = (int)(n_items * (blockIdx.x + 1) / gridDim.x);
+    if (lo >= hi) return;
+    const int tx = lane & 7, ty = lane >> 3;
+
+    auto issue = [&](int item, int s) {
+        if (lane == 0) {
+            const int t = item / a.nb, b = item - t * a.nb;
+            const uint32_t tile = a.tiles[t];
+            mbar_expect_tx(&s_bar[s], (unsigned)((IH - kSlackRows) * IW * sizeof(float)));
+            tma_load_3d(s_stage + (size_t)s * stage_floats, &tmap, &s_bar[s], a.ox + (int)(tile & 0xffffu) * kSW,
+                        a.oy + (int)(tile >> 16) * kSH, b);
+        }
+    };
+
+    issue(lo, 0);
+    int cur_t = -1;
+    bool warp_any = true;
+    const int NC4 = 4 * a.NC;
+    const int n4 = (a.KH + 1) >> 2;
+    const bool tail2 = ((a.KH + 1) & 2) != 0;
+
+#pragma unroll 1
+    for (int item = lo; item < hi; ++item) {
+        const int s = a.n_stages == 2 ? ((item - lo) & 1) : 0;
+        const int t = item / a.nb, b = item - t * a.nb;
+        const uint32_t tile = a.tiles[t];
+        const int oy = a.oy + (int)(tile >> 16) * kSH + ty * kTR, ox = a.ox + (int)(tile & 0xffffu) * kSW + tx * 4;
+        const bool more = item + 1 < hi;
+        if (a.n_stages == 2 && more) issue(item + 1, s ^ 1);      // its last readers passed the __syncwarp below
+
+        if (!RENDER && t != cur_t) {
+            // warps whose strip is fully masked never get here (api.cu lists strips with a counted
+            // pixel); the test stays for the strips of a render-sized list used by loglike
+            cur_t = t;
+            bool any = false;
+#pragma unroll
+            for (int o = 0; o < kTR; ++o)
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
+                    const float wv = (y < a.H && x < a.W) ? __ldg(a.wmask + (size_t)y * a.W + x) : 0.0f;
+                    any = any | (wv != 0.0f);
+                }
+            warp_any = __any_sync(0xffffffffu, any);
+        }
+        mbar_wait(&s_bar[s], a.n_stages == 2 ? (((item - lo) >> 1) & 1) : ((item - lo) & 1));
+        __syncwarp();              // lanes leave the wait loop one by one
+
+        f2 acc[2][8];
+#pragma unroll
+        for (int p = 0; p < 2; ++p)
+#pragma unroll
+            for (int e = 0; e < 8; ++e) acc[p][e] = bc(0.0f);
+        if (warp_any) {
+            const float4 *in_base = reinterpret_cast<const float4 *>(s_stage + (size_t)s * stage_floats) +
+                                    (size_t)(ty * kTR) * IW4 + tx;
+            const int last_taps = a.KW - 4 * (a.NC - 1);
+            const int n_full = last_taps == 4 ? a.NC : a.NC - 1;
+#pragma unroll 1
+            for (int c = 0; c < n_full; ++c)
+                conv_chunk<4, NTX, GT>(acc, in_base + c, a.tap_off + 4 * c, n4, tail2, IW4, NC4, gt);
+            if (last_taps != 4) {
+                const float4 *in_r = in_base + n_full;
+                const int iq = a.tap_off + 4 * n_full;
+                if (last_taps == 3) conv_chunk<3, NTX, GT>(acc, in_r, iq, n4, tail2, IW4, NC4, gt);
+                else if (last_taps == 2) conv_chunk<2, NTX, GT>(acc, in_r, iq, n4, tail2, IW4, NC4, gt);
+                else conv_chunk<1, NTX, GT>(acc, in_r, iq, n4, tail2, IW4, NC4, gt);
+            }
+        }
+        float out[kTR][8];
+#pragma unroll
+        for (int p = 0; p < 2; ++p)
+#pragma unroll
+            for (int e = 0; e < 8; ++e) un2(acc[p][e], out[2 * p][e], out[2 * p + 1][e]);
+
+        if (RENDER) {
+            const bool valid = a.derived[(size_t)b * a.D] != 0.0f;
+            float *mb = a.model + (size_t)b * a.H * a.W;
+#pragma unroll
+            for (int o = 0; o < kTR; ++o)
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
+                    if (y < a.H && x < a.W) mb[(size_t)y * a.W + x] = valid ? out[o][e] : nanf("");
+                }
+        } else {
+            float part = 0.0f;
+            if (warp_any) {
+#pragma unroll
+                for (int o = 0; o < kTR; ++o) {
+                    float wv[8], dv[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
+                        const bool in = y < a.H && x < a.W;
+                        wv[e] = in ? __ldg(a.wmask + (size_t)y * a.W + x) : 0.0f;
+                        dv[e] = in ? __ldg(a.image + (size_t)y * a.W + x) : 0.0f;
+                    }
+#pragma unroll
+                    for (int e = 0; e < 8; ++e)
+                        if (wv[e] != 0.0f) {               // masked pixels may see untraced L: never touch them
+                            const float diff = dv[e] - out[o][e];
+                            part = fmaf(wv[e] * diff, diff, part);
+                        }
+                }
+            }
+            double sum = (double)part;
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
+            if (lane == 0) a.partial[(size_t)b * a.n_tiles + t] = sum;
+        }
+        __syncwarp();              // every lane is done with stage s
+        if (a.n_stages == 1 && more) issue(item + 1, 0);
+    }
+}
+
 // logL[b] = -1/2 sum over tiles, in tile order; -inf for vectors outside the model domain
 __global__ void final_kernel(FinalArgs a)
 {
@@ -410,7 +571,12 @@ __global__ void final_kernel(FinalArgs a)
 
 }  // namespace
 
-void conv_tile_shape(bool wide, int *tile_w, int *tile_h) { *tile_w = wide ? Shape<16>::kTW : Shape<8>::kTW; *tile_h = kTH; }
+// shape: 0 = narrow, 1 = wide, 2 = strip (ConvArgs::shape)
+void conv_tile_shape(int shape, int *tile_w, int *tile_h)
+{
+    *tile_w = shape == 1 ? Shape<16>::kTW : shape == 0 ? Shape<8>::kTW : kSW;
+    *tile_h = shape == 2 ? kSH : kTH;
+}
 
 // rows x cols = the image rounded up to cover every tile of the grids in use (api.cu)
 void conv_padded_shape(int rows, int cols, int KH, int NC, int *Hp, int *Wp)
@@ -421,39 +587,55 @@ void conv_padded_shape(int rows, int cols, int KH, int NC, int *Hp, int *Wp)
 
 namespace {
 // dynamic shared memory a block may take: 227 KB per SM minus the static arrays, per resident block
-size_t smem_limit(bool wide) { return wide ? 226 * 1024 : 112 * 1024; }
-size_t stage_bytes(int KH, int NC, bool wide)
+size_t smem_limit(int shape) { return shape == 0 ? 112 * 1024 : shape == 2 ? 28 * 1024 : 226 * 1024; }   // strip: 8 blocks per SM
+size_t stage_bytes(int KH, int NC, int shape)
 {
-    const size_t floats = (size_t)(kTH + KH - 1 + kSlackRows) * ((wide ? 128 : 64) + 4 * NC);
+    int tw, th;
+    conv_tile_shape(shape, &tw, &th);
+    const size_t floats = (size_t)(th + KH - 1 + kSlackRows) * (tw + 4 * NC);
     return (floats + 31) / 32 * 32 * sizeof(float);
 }
-size_t dw_bytes(bool render, bool wide) { return render ? 0 : (size_t)2 * kTH * (wide ? 128 : 64) * sizeof(float); }
+// d and w of a tile staged in shared memory (block shapes, loglike); the strip shape reads them from global memory
+size_t dw_bytes(bool render, int shape) { return render || shape == 2 ? 0 : (size_t)2 * kTH * (shape == 1 ? 128 : 64) * sizeof(float); }
 }  // namespace
 
-int conv_num_stages(int KH, int NC, bool render, bool wide)
+int conv_num_stages(int KH, int NC, bool render, int shape)
 {
-    return 2 * stage_bytes(KH, NC, wide) + dw_bytes(render, wide) <= smem_limit(wide) ? 2 : 1;
+    return 2 * stage_bytes(KH, NC, shape) + dw_bytes(render, shape) <= smem_limit(shape) ? 2 : 1;
 }
 
-size_t conv_smem_bytes(int KH, int NC, bool render, bool wide)
+size_t conv_smem_bytes(int KH, int NC, bool render, int shape)
 {
-    return conv_num_stages(KH, NC, render, wide) * stage_bytes(KH, NC, wide) + dw_bytes(render, wide);
+    return conv_num_stages(KH, NC, render, shape) * stage_bytes(KH, NC, shape) + dw_bytes(render, shape);
 }
 
-// the narrow shape needs its single stage + d, w to fit twice per SM
-bool conv_narrow_fits(int KH, int NC) { return stage_bytes(KH, NC, false) + dw_bytes(false, false) <= smem_limit(false); }
+// the narrow shape needs its single stage + d, w to fit twice per SM; the strip shape one stage eight times
+bool conv_shape_fits(int KH, int NC, int shape)
+{
+    return shape == 1 || stage_bytes(KH, NC, shape) + dw_bytes(false, shape) <= smem_limit(shape);
+}
 
 namespace {
 template <bool RENDER, int NTX, bool GT>
 cudaError_t set_attr()
 {
     return cudaFuncSetAttribute(conv_kernel<RENDER, NTX, GT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)smem_limit(NTX == 16));
+                                (int)smem_limit(NTX == 16 ? 1 : 0));
+}
+template <bool RENDER, bool GT>
+cudaError_t set_attr_strip()
+{
+    return cudaFuncSetAttribute(conv_strip_kernel<RENDER, GT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024);
 }
 template <bool RENDER, int NTX, bool GT>
 void launch(const ConvArgs &a, const CUtensorMap &tmap, int grid, size_t smem, cudaStream_t st)
 {
     conv_kernel<RENDER, NTX, GT><<<grid, NTX * kNTY, smem, st>>>(a, tmap);
+}
+template <bool RENDER, bool GT>
+void launch_strip(const ConvArgs &a, const CUtensorMap &tmap, int grid, size_t smem, cudaStream_t st)
+{
+    conv_strip_kernel<RENDER, GT><<<grid, 32, smem, st>>>(a, tmap);
 }
 }  // namespace
 
@@ -463,6 +645,9 @@ cudaError_t conv_setup()
 #define LENSED_SET(R, N, G) if ((e = set_attr<R, N, G>()) != cudaSuccess) return e;
     LENSED_SET(false, 16, false) LENSED_SET(true, 16, false) LENSED_SET(false, 8, false) LENSED_SET(true, 8, false)
     LENSED_SET(false, 16, true) LENSED_SET(true, 16, true) LENSED_SET(false, 8, true) LENSED_SET(true, 8, true)
+#undef LENSED_SET
+#define LENSED_SET(R, G) if ((e = set_attr_strip<R, G>()) != cudaSuccess) return e;
+    LENSED_SET(false, false) LENSED_SET(true, false) LENSED_SET(false, true) LENSED_SET(true, true)
 #undef LENSED_SET
     return cudaSuccess;
 }
@@ -476,7 +661,7 @@ cudaError_t conv_upload_taps(const float *pairs, int n_pairs, int pool_offset)
 // Tensor map of the padded frames L[n_frames][Hp][Wp] for boxes of one input tile with its halo
 // (conv_kernel "issue").  out: 128 bytes, 64-byte aligned.  The encoder is a driver entry point
 // fetched through the runtime, so the library links against nothing but the static runtime.
-cudaError_t conv_make_tensor_map(void *out, const float *L, int Wp, int Hp, long long n_frames, int KH, int NC, bool wide)
+cudaError_t conv_make_tensor_map(void *out, const float *L, int Wp, int Hp, long long n_frames, int KH, int NC, int shape)
 {
     static PFN_cuTensorMapEncodeTiled_v12000 encode = nullptr;
     if (!encode) {
@@ -489,7 +674,9 @@ cudaError_t conv_make_tensor_map(void *out, const float *L, int Wp, int Hp, long
     }
     const cuuint64_t dims[3] = {(cuuint64_t)Wp, (cuuint64_t)Hp, (cuuint64_t)std::max<long long>(n_frames, 1)};
     const cuuint64_t strides[2] = {(cuuint64_t)Wp * sizeof(float), (cuuint64_t)Wp * Hp * sizeof(float)};
-    const cuuint32_t box[3] = {(cuuint32_t)((wide ? 128 : 64) + 4 * NC), (cuuint32_t)(kTH + KH - 1), 1};
+    int tw, th;
+    conv_tile_shape(shape, &tw, &th);
+    const cuuint32_t box[3] = {(cuuint32_t)(tw + 4 * NC), (cuuint32_t)(th + KH - 1), 1};
     const cuuint32_t estr[3] = {1, 1, 1};
     const CUresult r = encode((CUtensorMap *)out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)L, dims, strides, box, estr,
                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
@@ -501,10 +688,26 @@ cudaError_t conv_make_tensor_map(void *out, const float *L, int Wp, int Hp, long
 cudaError_t launch_conv(ConvArgs a, const void *tensor_map, bool render, int n_sm, cudaStream_t st)
 {
     const CUtensorMap &tmap = *reinterpret_cast<const CUtensorMap *>(tensor_map);
-    const bool wide = a.wide != 0, gt = a.gtaps != nullptr;
-    a.n_stages = conv_num_stages(a.KH, a.NC, render, wide);
-    const size_t smem = conv_smem_bytes(a.KH, a.NC, render, wide);
+    const bool gt = a.gtaps != nullptr;
+    a.n_stages = conv_num_stages(a.KH, a.NC, render, a.shape);
+    size_t smem = conv_smem_bytes(a.KH, a.NC, render, a.shape);
     const long long n_items = (long long)a.n_tiles * a.nb;
+    if (a.shape == 2) {
+        // k one-warp blocks per SM: the request is padded so that exactly k fit (228 KB per SM, 1 KB
+        // reserved per block) -- otherwise the block scheduler packs up to 12 on some SMs and leaves
+        // others empty
+        int k = kStripWarps;
+        if (const char *e = getenv("LENSED_STRIP_WARPS")) k = atoi(e);       // tuning
+        k = std::max(1, std::min(k, (int)((228 * 1024) / (smem + 1024 + 64))));
+        smem = std::max(smem, (size_t)((228 * 1024) / k - 1024 - 64) / 128 * 128);
+        const long long n_warps = (long long)n_sm * k;
+        const int grid = (int)(n_items < n_warps ? n_items : n_warps);
+        if (grid < 1) return cudaSuccess;
+        if (render) { if (gt) launch_strip<true, true>(a, tmap, grid, smem, st); else launch_strip<true, false>(a, tmap, grid, smem, st); }
+        else        { if (gt) launch_strip<false, true>(a, tmap, grid, smem, st); else launch_strip<false, false>(a, tmap, grid, smem, st); }
+        return cudaGetLastError();
+    }
+    const bool wide = a.shape == 1;
     const long long n_blocks = (long long)n_sm * (wide ? 1 : 2);
     const int grid = (int)(n_items < n_blocks ? n_items : n_blocks);
     if (grid < 1) return cudaSuccess;

@@ -148,7 +148,8 @@ struct ConvArgs {
     int nb;                // vectors in this launch
     const unsigned long long *gtaps;   // the handle's tap pairs in global memory when the constant pool was
                            // full (then tap_off = 0), else NULL
-    int wide;              // block shape: 1 = 256 threads, 64 x 128 tiles; 0 = 128 threads, 64 x 64 tiles
+    int shape;             // 1 = 256 threads, 64 x 128 tiles; 0 = 128 threads, 64 x 64 tiles; 2 = independent
+                           // warps on 16 x 64 strips (conv.cu)
     int tap_off;           // first tap pair of this handle in c_taps: Q[j][c][k] at tap_off + (j NC + c) 4 + k,
                            // Q[j][c][k] = (G[j][4c+k], G[j-1][4c+k]), j = 0..KH, G = flipped normalised PSF
     int n_stages;          // input-tile buffers in shared memory (set by launch_conv)
@@ -171,7 +172,7 @@ inline int trace_blocks_per_vector(const TraceArgs &a) { return (a.npix + a.pix_
 cudaError_t launch_refine(const Program &prog, const RefineArgs &a, int n_sm, cudaStream_t st);
 bool trace_has_static(const Program &prog);
 cudaError_t launch_conv(ConvArgs a, const void *tensor_map, bool render, int n_sm, cudaStream_t st);
-cudaError_t conv_make_tensor_map(void *out, const float *L, int Wp, int Hp, long long n_frames, int KH, int NC, bool wide);
+cudaError_t conv_make_tensor_map(void *out, const float *L, int Wp, int Hp, long long n_frames, int KH, int NC, int shape);
 cudaError_t conv_upload_taps(const float *pairs, int n_pairs, int pool_offset);
 void conv_padded_shape(int rows, int cols, int KH, int NC, int *Hp, int *Wp);
 cudaError_t launch_final(const FinalArgs &a, cudaStream_t st);
@@ -183,9 +184,11 @@ cudaError_t launch_image_plane_prior(const Program &prog, const int *par_offs, i
 cudaError_t conv_setup();                 // one-time function attributes
 int trace_pick_R(int n_quad);             // rays per register block for an n_quad-point rule
 size_t trace_smem_bytes(const Program &prog, int nq_pad);
-void conv_tile_shape(bool wide, int *tile_w, int *tile_h);
-size_t conv_smem_bytes(int KH, int NC, bool render, bool wide);
-bool conv_narrow_fits(int KH, int NC);
+// shape: 0 narrow (128 threads, 64 x 64 tiles, 2 blocks per SM), 1 wide (256 threads, 64 x 128), 2 strip
+// (8 independent warps, 16 x 64 strips)
+void conv_tile_shape(int shape, int *tile_w, int *tile_h);
+size_t conv_smem_bytes(int KH, int NC, bool render, int shape);
+bool conv_shape_fits(int KH, int NC, int shape);
 cudaError_t run_fma_peak(int iters, double *tflops);
 
 // for the clients of the handle outside api.cu (nested.cu): error text on the handle, its device

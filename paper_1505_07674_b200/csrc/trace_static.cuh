@@ -29,6 +29,21 @@ struct TraceSig {
     // and the SIE leaves its two raw functions in (ax, ay).  Saves the two packed adds of the
     // shear and the four packed FMAs of the SIE's accumulation per pair of rays.
     static constexpr bool direct = NSIE == 1 && NSIS == 0 && NPOINT == 0 && NSS + NSG >= 1;
+    // float4 index of the derived block of lens / light m (canonical order) in the vector's derived
+    // constants: api.cu lays them out header, lenses, lights in that order, so for a signature the
+    // offsets are compile-time constants (blocks: shear 1, SIE 3, SIS / point 2 | Sersic 4, Gaussian 3)
+    __host__ __device__ static constexpr int lens_off4(int m)
+    {
+        return 1 + (m < NSHEAR ? m : NSHEAR + (m < NSHEAR + NSIE ? 3 * (m - NSHEAR) : 3 * NSIE + 2 * (m - NSHEAR - NSIE)));
+    }
+    __host__ __device__ static constexpr int light_off4(int m)
+    {
+        return lens_off4(n_lens) +
+               (m < NSS ? 4 * m
+                        : 4 * NSS + (m < NSS + NSG ? 3 * (m - NSS)
+                                                   : 3 * NSG + (m < NSS + NSG + NFS ? 4 * (m - NSS - NSG)
+                                                                                    : 4 * NFS + 3 * (m - NSS - NSG - NFS))));
+    }
     static bool matches(const int (&c)[K_COUNT])
     {
         return c[K_SHEAR] == NSHEAR && c[K_SIE] == NSIE && c[K_SIS] == NSIS && c[K_POINT] == NPOINT &&
@@ -110,29 +125,36 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
 
         // frame origins of this pixel
         float lu[NL > 0 ? NL : 1], lv[NL > 0 ? NL : 1], gu[NPOS > 0 ? NPOS : 1], gv[NPOS > 0 ? NPOS : 1];
-        if (S::n_shear) shear_origin(sder + (prog.lens_off[0] >> 2), jf, rf, a.cxh, a.cyh, lu[0], lv[0]);
+        if (S::n_shear) shear_origin(sder + S::lens_off4(0), jf, rf, a.cxh, a.cyh, lu[0], lv[0]);
 #pragma unroll
         for (int i = 0; i < S::n_sie; ++i)
-            sie_origin(sder + (prog.lens_off[L_SIE + i] >> 2), jf, rf, lu[L_SIE + i], lv[L_SIE + i]);
+            sie_origin(sder + S::lens_off4(L_SIE + i), jf, rf, lu[L_SIE + i], lv[L_SIE + i]);
 #pragma unroll
         for (int i = 0; i < S::n_sis + S::n_point; ++i)
-            circular_origin(sder + (prog.lens_off[L_SIS + i] >> 2), jf, rf, lu[L_SIS + i], lv[L_SIS + i]);
+            circular_origin(sder + S::lens_off4(L_SIS + i), jf, rf, lu[L_SIS + i], lv[L_SIS + i]);
 #pragma unroll
-        for (int i = 0; i < NPOS; ++i) light_origin(sder + (prog.light_off[i] >> 2), jf, rf, gu[i], gv[i]);
+        for (int i = 0; i < NPOS; ++i) light_origin(sder + S::light_off4(i), jf, rf, gu[i], gv[i]);
         if (S::direct && S::n_shear) {
 #pragma unroll
             for (int i = 0; i < S::n_src; ++i) {              // sources come first among the lights
-                const float4 M = sder[(prog.light_off[i] >> 2) + 1];
+                const float4 M = sder[S::light_off4(i) + 1];
                 gu[i] -= fmaf(M.x, lu[0], M.y * lv[0]);
                 gv[i] -= fmaf(M.z, lu[0], M.w * lv[0]);
             }
         }
 
+        // the origins are per-pixel values: an empty asm that "writes" them keeps ptxas from
+        // recomputing them inside the ray loop to save registers (it did: +13 instructions per pass)
+#pragma unroll
+        for (int i = 0; i < NL; ++i) { asm volatile("" : "+f"(lu[i]), "+f"(lv[i])); }
+#pragma unroll
+        for (int i = 0; i < S::n_src; ++i) { asm volatile("" : "+f"(gu[i]), "+f"(gv[i])); }
+
         // foreground Sersics: moment expansion where it holds, else their own per-ray sum
         float fg = 0.0f;
 #pragma unroll
         for (int i = 0; i < S::n_fs; ++i) {
-            const float4 *d = sder + (prog.light_off[G_FS + i] >> 2);
+            const float4 *d = sder + S::light_off4(G_FS + i);
             const float s0 = fmaf(gu[G_FS + i], gu[G_FS + i], gv[G_FS + i] * gv[G_FS + i]);
             const float4 rng = d[3];
             if (s0 >= rng.x && s0 <= rng.y) {
@@ -169,19 +191,19 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
 #pragma unroll
             for (int i = 0; i < S::n_sie; ++i) {
                 const int m = L_SIE + i;
-                lens_sie<NP, MODE, S::direct>(sder + (prog.lens_off[m] >> 2), ltab + (size_t)(2 * m) * nq + q0,
+                lens_sie<NP, MODE, S::direct>(sder + S::lens_off4(m), ltab + (size_t)(2 * m) * nq + q0,
                                               ltab + (size_t)(2 * m + 1) * nq + q0, lu[m], lv[m], r);
             }
             // SIS / point mass: identity frame = slot 0
 #pragma unroll
             for (int i = 0; i < S::n_sis; ++i) {
                 const int m = L_SIS + i;
-                lens_circular<NP, false>(sder + (prog.lens_off[m] >> 2), tb.stab + q0, tb.stab + nq + q0, lu[m], lv[m], r);
+                lens_circular<NP, false>(sder + S::lens_off4(m), tb.stab + q0, tb.stab + nq + q0, lu[m], lv[m], r);
             }
 #pragma unroll
             for (int i = 0; i < S::n_point; ++i) {
                 const int m = L_PT + i;
-                lens_circular<NP, true>(sder + (prog.lens_off[m] >> 2), tb.stab + q0, tb.stab + nq + q0, lu[m], lv[m], r);
+                lens_circular<NP, true>(sder + S::lens_off4(m), tb.stab + q0, tb.stab + nq + q0, lu[m], lv[m], r);
             }
             if (NPOS - S::n_fs == 0) {                    // no light left in the ray loop
 #pragma unroll
@@ -190,7 +212,7 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
             // foreground lights first: they do not wait for the deflection (foreground Sersics
             // are not in this loop: "foreground expansion" above)
 #define LENSED_LIGHT(m, SRC, GAUSS, INIT)                                                                     \
-    light_profile<NP, SRC, GAUSS, INIT>(sder + (prog.light_off[m] >> 2), gtab + (size_t)(2 * (m)) * nq + q0, \
+    light_profile<NP, SRC, GAUSS, INIT>(sder + S::light_off4(m), gtab + (size_t)(2 * (m)) * nq + q0, \
                                         gtab + (size_t)(2 * (m) + 1) * nq + q0, gu[m], gv[m], r,              \
                                         (SRC) && S::direct ? tb.smat + (m) : nullptr,                         \
                                         (SRC) && !(GAUSS) ? rmin[(m) < S::n_ss ? (m) : 0] : rdummy)
@@ -219,7 +241,7 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
         store_pixel(a, Lb, row, col, ((lo2(acc) + hi2(acc)) + fg) + tb.sky);
 #pragma unroll
         for (int i = 0; i < S::n_ss; ++i)
-            if (rmin[i] < sder[(prog.light_off[i] >> 2) + 2].w) flags |= bit;
+            if (rmin[i] < sder[S::light_off4(i) + 2].w) flags |= bit;
     }
     if (a.fixmask) a.fixmask[((size_t)vec * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = flags;
 }
@@ -244,15 +266,15 @@ __global__ void __launch_bounds__(kTraceThreads, MINB * (256 / kTraceThreads)) t
         if (S::n_shear) {
             for (int i = threadIdx.x; i < S::n_src * nq; i += kTraceThreads) {
                 const int m = i / nq, k = i - m * nq;
-                const float4 M = tb.sder[(prog.light_off[m] >> 2) + 1];
+                const float4 M = tb.sder[S::light_off4(m) + 1];
                 const float su = stab[2 * nq + k], sv = stab[3 * nq + k];     // shear = lens 0
                 gtab[(size_t)(2 * m) * nq + k] -= fmaf(M.x, su, M.y * sv);
                 gtab[(size_t)(2 * m + 1) * nq + k] -= fmaf(M.z, su, M.w * sv);
             }
         }
         if (threadIdx.x < S::n_src) {
-            const float4 M = tb.sder[(prog.light_off[threadIdx.x] >> 2) + 1];
-            const float4 c2 = tb.sder[(prog.lens_off[S::n_shear] >> 2) + 2];  // (cs A, sn A, cs A l, -sn A l)
+            const float4 M = tb.sder[S::light_off4(threadIdx.x) + 1];
+            const float4 c2 = tb.sder[S::lens_off4(S::n_shear) + 2];  // (cs A, sn A, cs A l, -sn A l)
             tb.smat[threadIdx.x] = make_float4(fmaf(M.x, c2.x, M.y * c2.y), fmaf(M.x, c2.w, M.y * c2.z),
                                                fmaf(M.z, c2.x, M.w * c2.y), fmaf(M.z, c2.w, M.w * c2.z));
         }

@@ -262,8 +262,11 @@ def lensed_frame_bytes(h):
     return lib().lensed_frame_bytes(h)
 
 
-def lensed_set_conv_shape(h, wide):
-    _check(lib().lensed_set_conv_shape(h, int(bool(wide))), h)
+CONV_SHAPES = ("narrow", "wide", "strip")     # lensed_set_conv_shape / lensed_get_conv_shape: 0, 1, 2
+
+
+def lensed_set_conv_shape(h, shape):
+    _check(lib().lensed_set_conv_shape(h, int(shape)), h)
 
 
 def lensed_get_conv_shape(h):

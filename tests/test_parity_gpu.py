@@ -409,9 +409,12 @@ def test_full_constant_tap_pool_falls_back_to_global_memory_taps(L):
 
 @pytest.mark.parametrize("index,H,W,B", [(1, 90, 70, 12), (2, 75, 93, 8), (3, 70, 150, 6), (4, 101, 67, 4), (5, 60, 64, 6)])
 @pytest.mark.parametrize("global_taps", [False, True])
-def test_both_convolution_shapes_and_both_tap_paths(L, index, H, W, B, global_taps):
-    """wide (256 threads, 64 x 128 tiles) and narrow (128 threads, 64 x 64 tiles, two blocks per
-    SM) blocks, taps from the constant pool or from global memory: same results against the oracle."""
+def test_all_convolution_shapes_and_both_tap_paths(L, index, H, W, B, global_taps):
+    """strip (8 independent warps per SM on 16 x 64 strips), wide (256 threads, 64 x 128 tiles) and
+    narrow (128 threads, 64 x 64 tiles, two blocks per SM), taps from the constant pool or from
+    global memory: same results against the oracle, and the rendered images of the three shapes
+    agree bit for bit (same per-pixel arithmetic; only the chi-square partials are grouped
+    differently)."""
     cfg = synth.shrunk(synth.get_config(index), H, W, B)
     prob = Problem(cfg)
     params = cfg.batch()
@@ -423,12 +426,40 @@ def test_both_convolution_shapes_and_both_tap_paths(L, index, H, W, B, global_ta
         L.lensed_debug_force_global_taps(False)
     try:
         assert L.lensed_uses_global_taps(h) == int(global_taps)
-        for wide in (1, 0):
-            L.lensed_set_conv_shape(h, wide)
-            assert L.lensed_get_conv_shape(h) == wide
+        models = []
+        for shape in (2, 1, 0):
+            L.lensed_set_conv_shape(h, shape)
+            assert L.lensed_get_conv_shape(h) == shape
             logl, model = _gpu_eval(L, h, params, cfg.H, cfg.W)
             assert logl_errors(logl, logl_o).max() <= LOGL_RTOL
             assert pixel_errors(model, model_o).max() <= PIXEL_RTOL
+            models.append(model)
+        assert np.array_equal(models[0], models[1]) and np.array_equal(models[0], models[2])
+        with pytest.raises(L.LensedError) as e:
+            L.lensed_set_conv_shape(h, 3)
+        assert e.value.status == L.EINVAL
+    finally:
+        L.lensed_destroy(h)
+
+
+def test_shape_picked_at_create_and_shared_memory_limits(L):
+    """lensed_create: wide for a full image, strip for the SLACS annulus (its strips compute 22 %
+    fewer pixels than the narrow tiles); a 63 x 63 PSF does not fit the strip shape's eight stages."""
+    for index, want in ((4, 1), (2, 2)):
+        h = Problem(synth.get_config(index), image=np.zeros((synth.get_config(index).H, synth.get_config(index).W), np.float32),
+                    weight=np.ones((synth.get_config(index).H, synth.get_config(index).W), np.float32)).create()
+        try:
+            assert L.lensed_get_conv_shape(h) == want
+        finally:
+            L.lensed_destroy(h)
+    cfg = synth.shrunk(synth.get_config(1), 40, 36, 2)
+    cfg.psf = synth.moffat_psf(63, 3.0, 2.5)
+    h = Problem(cfg, image=np.zeros((40, 36), np.float32), weight=np.ones((40, 36), np.float32)).create()
+    try:
+        assert L.lensed_get_conv_shape(h) in (0, 1)
+        with pytest.raises(L.LensedError) as e:
+            L.lensed_set_conv_shape(h, 2)
+        assert e.value.status == L.EUNSUPPORTED
     finally:
         L.lensed_destroy(h)
 
