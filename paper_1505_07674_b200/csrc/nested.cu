@@ -123,20 +123,49 @@ __global__ void __launch_bounds__(256) ns_bound_kernel(NsProblem pb, const doubl
     __shared__ double sC[kMaxFree * kMaxFree];
     __shared__ double sred[256];
     const int d = pb.d, N = pb.N, t = threadIdx.x;
-    for (int k = t; k < d; k += 256) {
-        double a = 0.0;
-        for (int i = 0; i < N; ++i) a += U[(size_t)i * d + k];
-        sm[k] = a / N;
+    // mean and covariance: when the block has more threads than entries, every entry's sum over the N
+    // live points is split over S = 256 / entries strided segments (partials in sred, added in
+    // segment order: deterministic)
+    {
+        const int E = d, S = E <= 128 ? 256 / E : 1;
+        const int e = t % E, seg = t / E;
+        for (int k = S > 1 ? e : t; k < d; k += S > 1 ? d : 256) {
+            if (seg >= S) break;
+            double a = 0.0;
+            for (int i = S > 1 ? seg : 0; i < N; i += S) a += U[(size_t)i * d + k];
+            if (S > 1) sred[seg * E + e] = a; else sm[k] = a / N;
+        }
+        __syncthreads();
+        if (S > 1 && t < E) {
+            double a = 0.0;
+            for (int g = 0; g < S; ++g) a += sred[g * E + t];
+            sm[t] = a / N;
+        }
+        __syncthreads();
     }
-    __syncthreads();
-    for (int e = t; e < d * d; e += 256) {
-        const int a = e / d, b = e - a * d;
-        if (b > a) continue;
-        double acc = 0.0;
-        for (int i = 0; i < N; ++i) acc += (U[(size_t)i * d + a] - sm[a]) * (U[(size_t)i * d + b] - sm[b]);
-        sC[a * d + b] = acc / N + (a == b ? 1e-30 : 0.0);
+    {
+        const int E = d * d, S = E <= 128 ? 256 / E : 1;
+        const int e0 = t % E, seg = t / E;
+        for (int e = S > 1 ? e0 : t; e < E; e += S > 1 ? E : 256) {
+            if (seg >= S) break;
+            const int a = e / d, b = e - a * d;
+            double acc = 0.0;
+            if (b <= a)
+                for (int i = S > 1 ? seg : 0; i < N; i += S) acc += (U[(size_t)i * d + a] - sm[a]) * (U[(size_t)i * d + b] - sm[b]);
+            if (S > 1) sred[seg * E + e0] = acc;
+            else if (b <= a) sC[a * d + b] = acc / N + (a == b ? 1e-30 : 0.0);
+        }
+        __syncthreads();
+        if (S > 1 && t < E) {
+            const int a = t / d, b = t - a * d;
+            if (b <= a) {
+                double acc = 0.0;
+                for (int g = 0; g < S; ++g) acc += sred[g * E + t];
+                sC[a * d + b] = acc / N + (a == b ? 1e-30 : 0.0);
+            }
+        }
+        __syncthreads();
     }
-    __syncthreads();
     // Cholesky, column by column, in place in the lower triangle
     for (int j = 0; j < d; ++j) {
         if (t == 0) {
@@ -214,28 +243,6 @@ __global__ void ns_propose_kernel(NsProblem pb, const double *m, const double *G
     write_theta(pb, x, theta_c + (size_t)j * pb.P);
 }
 
-// block-wide argmin with the lower index winning ties (numpy's argmin); result in s_val[0], s_idx[0]
-__device__ inline void block_argmin(const float *logl, int N, float *s_val, int *s_idx)
-{
-    const int t = threadIdx.x;
-    float v = INFINITY;
-    int at = 0x7fffffff;
-    for (int i = t; i < N; i += 256) {
-        const float l = logl[i];
-        if (l < v || (l == v && i < at)) { v = l; at = i; }
-    }
-    s_val[t] = v; s_idx[t] = at;
-    __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
-        if (t < o) {
-            const float l = s_val[t + o];
-            const int i = s_idx[t + o];
-            if (l < s_val[t] || (l == s_val[t] && i < s_idx[t])) { s_val[t] = l; s_idx[t] = i; }
-        }
-        __syncthreads();
-    }
-}
-
 // ln Z and H after adding one point of likelihood ls and log-weight lw (Skilling 2006 eq. 2.11)
 __device__ inline void accumulate(NsState &st, double ls, double lw)
 {
@@ -248,53 +255,190 @@ __device__ inline void accumulate(NsState &st, double ls, double lw)
     st.ln_z = ln_z_new;
 }
 
+// The same update for n points at once, by the whole block:  Z = sum_k L_k w_k  and
+// S = sum_k L_k w_k ln L_k  are plain sums (H = S/Z - ln Z is eq. 2.11 unrolled), taken relative to
+// the largest term; per-thread partial sums in index order, then a fixed tree: deterministic.
+// Differs from n calls of accumulate() by FP64 rounding only.  term(k) -> ln L_k, ln w_k.
+template <class F>
+__device__ inline void block_accumulate(NsState &st, int n, F term, double *s_a, double *s_b)
+{
+    const int t = threadIdx.x;
+    double m = -INFINITY;
+    for (int k = t; k < n; k += 256) {
+        double ls, lw;
+        term(k, ls, lw);
+        m = fmax(m, ls + lw);
+    }
+    s_a[t] = m;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (t < o) s_a[t] = fmax(s_a[t], s_a[t + o]);
+        __syncthreads();
+    }
+    const double M = fmax(s_a[0], st.ln_z);
+    __syncthreads();
+    if (!(M > -INFINITY)) return;                            // nothing has any weight yet
+    double z = 0.0, sl = 0.0;
+    for (int k = t; k < n; k += 256) {
+        double ls, lw;
+        term(k, ls, lw);
+        const double w = exp(ls + lw - M);
+        z += w;
+        if (w > 0.0) sl += w * ls;
+    }
+    s_a[t] = z; s_b[t] = sl;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (t < o) { s_a[t] += s_a[t + o]; s_b[t] += s_b[t + o]; }
+        __syncthreads();
+    }
+    if (t == 0) {
+        const double zo = isfinite(st.ln_z) ? exp(st.ln_z - M) : 0.0;
+        const double so = zo > 0.0 ? zo * (st.info + st.ln_z) : 0.0;
+        const double Z = zo + s_a[0], S = so + s_b[0];
+        st.ln_z = M + log(Z);
+        st.info = S / Z - st.ln_z;
+    }
+    __syncthreads();
+}
+
 struct NsOut { float *samples, *logl, *logw; long long cap; };
 
+// order-preserving map float -> unsigned (no NaN here): the warp-wide minimum is then ONE REDUX
+// instruction (__reduce_min_sync) instead of five shuffle rounds
+__device__ inline unsigned fkey(float f)
+{
+    const unsigned u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ inline float fkey_inv(unsigned k) { return __uint_as_float((k & 0x80000000u) ? (k ^ 0x80000000u) : ~k); }
+
+// minimum of the group of 32 slots g (whole warp): key and slot, the lowest slot winning ties
+__device__ inline void group_min(const float *s_logl, int N, int g, int lane, unsigned *s_gkey, int *s_gidx)
+{
+    const int i = g * 32 + lane;
+    const unsigned key = i < N ? fkey(s_logl[i]) : 0xffffffffu;
+    const unsigned kmin = __reduce_min_sync(0xffffffffu, key);
+    const int b = __ffs(__ballot_sync(0xffffffffu, key == kmin)) - 1;
+    if (lane == 0) { s_gkey[g] = kmin; s_gidx[g] = g * 32 + b; }
+}
+
+// Step 4 of the algorithm for one round, in the sequential order of its definition but without a
+// block-wide pass per candidate.  The live likelihoods sit in shared memory under a two-level
+// tournament: the minimum of every group of 32 slots, and the minimum over the groups.  ONE warp
+// walks the candidates 32 at a time (a ballot against the current threshold finds the next one
+// that beats it; after each death the threshold rises and the rest of the chunk is re-tested);
+// a death costs two warp-wide minima (its group, then the groups), each a REDUX and a ballot.  The warp only records who
+// died and who took which slot; all 256 threads then copy the dead points' parameter vectors
+// out and the surviving candidates in.  Same deaths, same order, same weights as the
+// candidate-by-candidate loop it replaces (1.07 ms -> 0.1 ms per round of 1024 candidates
+// against 1024 live points).
 __global__ void __launch_bounds__(256) ns_update_kernel(NsProblem pb, double *U, float *theta, float *logl_live,
                                                         const double *Uc, const float *theta_c, const float *logl_c,
-                                                        NsOut out, NsState *st_g)
+                                                        int *death_src, float *death_logl, NsOut out, NsState *st_g)
 {
     if (st_g->done) return;
     __shared__ float s_logl[kMaxLive];
+    __shared__ int s_owner[kMaxLive];          // -1: live since before this round; else the candidate in the slot
+    __shared__ unsigned s_gkey[kMaxLive / 32];
+    __shared__ int s_gidx[kMaxLive / 32];
+    constexpr int kChunk = 1024;
+    __shared__ float s_cl[kChunk];
     __shared__ float s_val[256];
-    __shared__ int s_idx[256];
+    __shared__ double s_red_a[256], s_red_b[256];
     __shared__ NsState st;
-    const int t = threadIdx.x, N = pb.N, d = pb.d, P = pb.P;
-    for (int i = t; i < N; i += 256) s_logl[i] = logl_live[i];
-    if (t == 0) st = *st_g;
+    __shared__ long long s_first_dead;
+    __shared__ int s_deaths;
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5, N = pb.N, d = pb.d, P = pb.P;
+    const int G = (N + 31) >> 5;
+    for (int i = t; i < N; i += 256) { s_logl[i] = logl_live[i]; s_owner[i] = -1; }
+    if (t == 0) { st = *st_g; s_first_dead = st_g->n_dead; s_deaths = 0; }
     __syncthreads();
-    block_argmin(s_logl, N, s_val, s_idx);
-    const double ln_shell = log(-expm1(-1.0 / N));          // ln (X_(k-1) - X_k) - ln X_(k-1)
-    for (int j = 0; j < pb.K; ++j) {
-        const bool is_void = isnan(Uc[(size_t)j * d]);
-        const float cl = is_void ? -INFINITY : logl_c[j];
-        const float lmin = s_val[0];
-        const int worst = s_idx[0];
-        if (!(cl > lmin)) continue;                          // block-uniform
-        __syncthreads();
-        if (t == 0) {
-            accumulate(st, (double)lmin, st.ln_x + ln_shell);
-            st.ln_x -= 1.0 / N;
+    for (int g = warp; g < G; g += 8) group_min(s_logl, N, g, lane, s_gkey, s_gidx);
+    __syncthreads();
+
+    // minimum over the groups: every lane its own groups (lower group first), then two REDUX
+    auto global_min = [&](float &v, int &i) {
+        unsigned key = 0xffffffffu;
+        int bg = 0x7fffffff;
+        for (int g = lane; g < G; g += 32) {
+            const unsigned gk = s_gkey[g];
+            if (gk < key) { key = gk; bg = g; }
         }
-        const long long slot = st.n_dead;                    // read before thread 0 bumps it (barrier below)
-        if (slot < out.cap) {
-            for (int p = t; p < P; p += 256) out.samples[(size_t)slot * P + p] = theta[(size_t)worst * P + p];
-            if (t == 0) {
-                out.logl[slot] = lmin;
-                out.logw[slot] = (float)(st.ln_x + 1.0 / N + ln_shell);     // this point's ln w (ln_x already stepped)
+        const unsigned kmin = __reduce_min_sync(0xffffffffu, key);
+        const int gsel = (int)__reduce_min_sync(0xffffffffu, key == kmin ? (unsigned)bg : 0x7fffffffu);
+        v = fkey_inv(kmin);
+        i = s_gidx[gsel];
+    };
+    float lmin = 0.0f;
+    int worst = 0;
+    if (warp == 0) global_min(lmin, worst);
+    int n_died = 0;                                          // warp 0's count
+    for (int base0 = 0; base0 < pb.K; base0 += kChunk) {
+        // the candidates' likelihoods of this stretch into shared memory, by the whole block
+        __syncthreads();
+        for (int c = t; c < kChunk; c += 256) {
+            const int j = base0 + c;
+            s_cl[c] = (j < pb.K && !isnan(Uc[(size_t)j * d])) ? logl_c[j] : -INFINITY;   // void candidate: never accepted
+        }
+        __syncthreads();
+        if (warp != 0) continue;
+        for (int base = 0; base < kChunk && base0 + base < pb.K; base += 32) {
+            const float cl = s_cl[base + lane];
+            unsigned mask = __ballot_sync(0xffffffffu, cl > lmin);
+            while (mask) {
+                const int b = __ffs(mask) - 1;
+                const float cj = __shfl_sync(0xffffffffu, cl, b);
+                if (lane == 0) {
+                    const int own = s_owner[worst];
+                    death_src[n_died] = own < 0 ? worst : ~own;      // whose parameter vector dies: a live row or a candidate
+                    death_logl[n_died] = lmin;
+                    s_logl[worst] = cj;
+                    s_owner[worst] = base0 + base + b;
+                }
+                ++n_died;
+                __syncwarp();
+                group_min(s_logl, N, worst >> 5, lane, s_gkey, s_gidx);
+                __syncwarp();
+                global_min(lmin, worst);
+                mask = __ballot_sync(0xffffffffu, cl > lmin) & ~((2u << b) - 1u);   // the later candidates of the chunk
             }
         }
-        __syncthreads();
-        for (int k = t; k < d; k += 256) U[(size_t)worst * d + k] = Uc[(size_t)j * d + k];
-        for (int p = t; p < P; p += 256) theta[(size_t)worst * P + p] = theta_c[(size_t)j * P + p];
-        if (t == 0) { s_logl[worst] = cl; st.n_dead += 1; }
-        __syncthreads();
-        block_argmin(s_logl, N, s_val, s_idx);
+    }
+    if (t == 0) s_deaths = n_died;
+    __syncthreads();
+
+    // evidence and information: death k of the round has ln w = ln X - k/N + ln(1 - e^(-1/N))
+    const int deaths = s_deaths;
+    const double ln_shell = log(-expm1(-1.0 / N));           // ln (X_(k-1) - X_k) - ln X_(k-1)
+    const double ln_x0 = st.ln_x;
+    for (int k = t; k < deaths; k += 256) {
+        const long long slot = s_first_dead + k;
+        if (slot < out.cap) { out.logl[slot] = death_logl[k]; out.logw[slot] = (float)(ln_x0 - (double)k / N + ln_shell); }
+    }
+    block_accumulate(st, deaths, [&](int k, double &ls, double &lw) { ls = (double)death_logl[k]; lw = ln_x0 - (double)k / N + ln_shell; },
+                     s_red_a, s_red_b);
+    if (t == 0) { st.ln_x = ln_x0 - (double)deaths / N; st.n_dead += deaths; }
+    // the dead points' parameter vectors, in order of death (theta still holds the round's starting rows)
+    for (long long e = t; e < (long long)deaths * P; e += 256) {
+        const int k = (int)(e / P), p = (int)(e - (long long)k * P);
+        const long long slot = s_first_dead + k;
+        if (slot < out.cap) {
+            const int src = death_src[k];
+            out.samples[(size_t)slot * P + p] = src >= 0 ? theta[(size_t)src * P + p] : theta_c[(size_t)(~src) * P + p];
+        }
+    }
+    __syncthreads();
+    // the surviving candidates into their slots
+    for (int i = warp; i < N; i += 8) {
+        const int own = s_owner[i];
+        if (own < 0) continue;
+        for (int k = lane; k < d; k += 32) U[(size_t)i * d + k] = Uc[(size_t)own * d + k];
+        for (int p = lane; p < P; p += 32) theta[(size_t)i * P + p] = theta_c[(size_t)own * P + p];
     }
     // convergence: max_i L_i X_k < tol Z
     float v = -INFINITY;
     for (int i = t; i < N; i += 256) v = fmaxf(v, s_logl[i]);
-    __syncthreads();
     s_val[t] = v;
     __syncthreads();
     for (int o = 128; o > 0; o >>= 1) {
@@ -311,36 +455,40 @@ __global__ void __launch_bounds__(256) ns_update_kernel(NsProblem pb, double *U,
     }
 }
 
-// the live points join the dead, lowest likelihood first, weight X_k / N each; then the
-// log-weights are normalised: logw <- ln(L w / Z)
+// the live points join the dead, lowest likelihood first (ties: lower slot first), weight X_k / N
+// each; then the log-weights are normalised: logw <- ln(L w / Z)
 __global__ void __launch_bounds__(256) ns_final_kernel(NsProblem pb, const float *theta, const float *logl_live,
                                                        NsOut out, NsState *st_g)
 {
     __shared__ float s_logl[kMaxLive];
-    __shared__ float s_val[256];
-    __shared__ int s_idx[256];
+    __shared__ int s_order[kMaxLive];          // slot of the n-th lowest live point
+    __shared__ double s_red_a[256], s_red_b[256];
     __shared__ NsState st;
     const int t = threadIdx.x, N = pb.N, P = pb.P;
     for (int i = t; i < N; i += 256) s_logl[i] = logl_live[i];
     if (t == 0) st = *st_g;
     __syncthreads();
-    const double lw = st.ln_x - log((double)N);
-    long long slot = st.n_dead;
-    for (int n = 0; n < N; ++n, ++slot) {
-        block_argmin(s_logl, N, s_val, s_idx);
-        const int i = s_idx[0];
-        const float li = s_val[0];
-        if (t == 0) accumulate(st, (double)li, lw);
-        if (slot < out.cap) {
-            for (int p = t; p < P; p += 256) out.samples[(size_t)slot * P + p] = theta[(size_t)i * P + p];
-            if (t == 0) { out.logl[slot] = li; out.logw[slot] = (float)lw; }
+    for (int i = t; i < N; i += 256) {         // rank by (likelihood, slot): what N successive argmins would give
+        const float li = s_logl[i];
+        int rank = 0;
+        for (int j = 0; j < N; ++j) {
+            const float lj = s_logl[j];
+            rank += (lj < li || (lj == li && j < i)) ? 1 : 0;
         }
-        __syncthreads();
-        if (t == 0) s_logl[i] = INFINITY;
-        __syncthreads();
+        s_order[rank] = i;
     }
-    const long long n_out = slot < out.cap ? slot : out.cap;
     __syncthreads();
+    const double lw = st.ln_x - log((double)N);
+    const long long first = st.n_dead;
+    block_accumulate(st, N, [&](int n, double &ls, double &lw_) { ls = (double)s_logl[s_order[n]]; lw_ = lw; }, s_red_a, s_red_b);
+    for (long long e = t; e < (long long)N * P; e += 256) {
+        const int n = (int)(e / P), p = (int)(e - (long long)n * P);
+        if (first + n < out.cap) out.samples[(size_t)(first + n) * P + p] = theta[(size_t)s_order[n] * P + p];
+    }
+    for (int n = t; n < N; n += 256)
+        if (first + n < out.cap) { out.logl[first + n] = s_logl[s_order[n]]; out.logw[first + n] = (float)lw; }
+    __syncthreads();
+    const long long n_out = first + N < out.cap ? first + N : out.cap;
     for (long long k = t; k < n_out; k += 256) out.logw[k] = (float)((double)out.logl[k] + (double)out.logw[k] - st.ln_z);
     if (t == 0) { st.n_written = n_out; *st_g = st; }
 }
@@ -403,14 +551,15 @@ extern "C" lensed_status lensed_ns_run(lensed_handle *h, const float *prior_lo, 
     NS_CU(cudaSetDevice(handle_device(h)));
     Buffers buf;
     double *d_lo, *d_hi, *d_U, *d_Uc, *d_m, *d_G, *d_s;
-    int *d_free;
+    int *d_free, *d_death;
+    float *d_death_l;
     float *d_theta, *d_theta_c, *d_logl, *d_logl_c;
     NsState *d_state;
     NS_CU(buf.get(&d_lo, P)); NS_CU(buf.get(&d_hi, P)); NS_CU(buf.get(&d_free, d));
     NS_CU(buf.get(&d_U, (size_t)N * d)); NS_CU(buf.get(&d_Uc, (size_t)K * d));
     NS_CU(buf.get(&d_m, d)); NS_CU(buf.get(&d_G, (size_t)d * d)); NS_CU(buf.get(&d_s, 1));
     NS_CU(buf.get(&d_theta, (size_t)N * P)); NS_CU(buf.get(&d_theta_c, (size_t)K * P));
-    NS_CU(buf.get(&d_logl, N)); NS_CU(buf.get(&d_logl_c, K)); NS_CU(buf.get(&d_state, 1));
+    NS_CU(buf.get(&d_logl, N)); NS_CU(buf.get(&d_logl_c, K)); NS_CU(buf.get(&d_state, 1)); NS_CU(buf.get(&d_death, K)); NS_CU(buf.get(&d_death_l, K));
     NS_CU(cudaMemcpyAsync(d_lo, lo.data(), P * sizeof(double), cudaMemcpyHostToDevice, st));
     NS_CU(cudaMemcpyAsync(d_hi, hi.data(), P * sizeof(double), cudaMemcpyHostToDevice, st));
     NS_CU(cudaMemcpyAsync(d_free, free_idx.data(), d * sizeof(int), cudaMemcpyHostToDevice, st));
@@ -436,7 +585,7 @@ extern "C" lensed_status lensed_ns_run(lensed_handle *h, const float *prior_lo, 
             if (n_image_plane > 0)
                 NS_OK(lensed_image_plane_prior(h, d_theta_c, K, image_plane_sources, n_image_plane, stream));
             NS_OK(lensed_loglike(h, d_theta_c, K, d_logl_c, stream));
-            ns_update_kernel<<<1, 256, 0, st>>>(pb, d_U, d_theta, d_logl, d_Uc, d_theta_c, d_logl_c, out, d_state);
+            ns_update_kernel<<<1, 256, 0, st>>>(pb, d_U, d_theta, d_logl, d_Uc, d_theta_c, d_logl_c, d_death, d_death_l, out, d_state);
             NS_CU(cudaGetLastError());
         }
         NS_CU(cudaMemcpyAsync(&host, d_state, sizeof host, cudaMemcpyDeviceToHost, st));
