@@ -42,6 +42,8 @@ struct lensed_handle {
     double scale = 0, zp = 0;
     Program prog{};
     int n_quad = 0, R = 1, nq_pad = 0;
+    int np_pp = 2, nq_pp = 0;       // the rule in passes for the pixel-pair tracers (trace_static.cuh)
+    std::vector<float4> h_quad_pp;
     std::vector<float4> h_quad;     // host copy of d_quad (lensed_set_error_rule rewrites .w)
     bool has_error_rule = false;
     int KH = 1, KW = 1, NC = 1;
@@ -56,7 +58,7 @@ struct lensed_handle {
 
     // device, immutable after create
     float *d_image = nullptr, *d_wmask = nullptr;
-    float4 *d_quad = nullptr;
+    float4 *d_quad = nullptr, *d_quad_pp = nullptr;
     uint32_t *d_pix_ll = nullptr, *d_pix_all = nullptr, *d_tiles_ll = nullptr, *d_tiles_all = nullptr;
     int npix_ll = 0, npix_all = 0, ntiles_ll = 0, ntiles_all = 0;
 
@@ -371,6 +373,7 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
             ta.derived = h->d_derived + (size_t)b0 * prog.D;
             ta.pix = render ? h->d_pix_all : h->d_pix_ll;
             ta.quad = h->d_quad;
+            ta.quad_pp = h->d_quad_pp; ta.nq_pp = h->nq_pp; ta.np_pp = h->np_pp;
             ta.fixmask = refine ? h->d_fixmask : nullptr;
             ta.L = h->d_L;
             ta.l_stride = (long long)HWp;
@@ -555,6 +558,15 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     std::vector<float4> hq(h->nq_pad, make_float4(0.f, 0.f, 0.f, 0.f));
     for (int k = 0; k < n_quad; ++k)
         hq[k] = make_float4(quad[3 * k], quad[3 * k + 1], (float)((double)quad[3 * k + 2] / wsum), 0.f);
+    // the same rule in passes of np_pp points, every pass a 16-byte-aligned stretch of 4 or 8 table
+    // entries (the rest zero-weight and never evaluated): layout of the pixel-pair tracers
+    h->np_pp = trace_pick_np(n_quad);
+    {
+        const int npp = h->np_pp <= 4 ? 4 : 8, n_pass = (n_quad + h->np_pp - 1) / h->np_pp;
+        h->nq_pp = n_pass * npp;
+        h->h_quad_pp.assign(h->nq_pp, make_float4(0.f, 0.f, 0.f, 0.f));
+        for (int k = 0; k < n_quad; ++k) h->h_quad_pp[(k / h->np_pp) * npp + k % h->np_pp] = hq[k];
+    }
     {
         // first and third moments of the rule: the foreground expansion (trace_static.cuh) drops
         // them, so it is used only when they vanish (every Cartesian-product rule of the paper does)
@@ -645,6 +657,7 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
         }
     }
     CREATE_FAIL(upload(h, &h->d_quad, hq.data(), hq.size()));
+    CREATE_FAIL(upload(h, &h->d_quad_pp, h->h_quad_pp.data(), h->h_quad_pp.size()));
     {
         const unsigned long long zero = 0;
         CREATE_FAIL(upload(h, &h->d_refined, &zero, 1));
@@ -673,6 +686,7 @@ lensed_status lensed_clone(const lensed_handle *src, lensed_handle **out)
     h->device = src->device; h->H = src->H; h->W = src->W; h->scale = src->scale; h->zp = src->zp;
     h->prog = src->prog;
     h->n_quad = src->n_quad; h->R = src->R; h->nq_pad = src->nq_pad; h->h_quad = src->h_quad;
+    h->np_pp = src->np_pp; h->nq_pp = src->nq_pp; h->h_quad_pp = src->h_quad_pp;
     h->has_error_rule = src->has_error_rule;
     h->KH = src->KH; h->KW = src->KW; h->NC = src->NC; h->n_sm = src->n_sm;
     h->tap_off = src->tap_off; h->tap_pairs = src->tap_pairs; h->d_gtaps = src->d_gtaps;
@@ -685,6 +699,7 @@ lensed_status lensed_clone(const lensed_handle *src, lensed_handle **out)
 #define CLONE_FAIL(expr) do { s = (expr); if (s != LENSED_OK) { g_last_error = h->err; lensed_destroy(h); return s; } } while (0)
     if (cudaSetDevice(h->device) != cudaSuccess) { lensed_destroy(h); return fail(nullptr, LENSED_ECUDA, "cudaSetDevice failed"); }
     CLONE_FAIL(upload(h, &h->d_quad, h->h_quad.data(), h->h_quad.size()));
+    CLONE_FAIL(upload(h, &h->d_quad_pp, h->h_quad_pp.data(), h->h_quad_pp.size()));
     const unsigned long long zero = 0;
     const unsigned zero32 = 0;
     CLONE_FAIL(upload(h, &h->d_refined, &zero, 1));
@@ -951,7 +966,7 @@ void lensed_destroy(lensed_handle *h)
     cudaDeviceSynchronize();
     for (EventPair &ep : h->used) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
     for (EventPair &ep : h->pool) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
-    cudaFree(h->d_quad); cudaFree(h->d_tiles_ll); cudaFree(h->d_tiles_all);
+    cudaFree(h->d_quad); cudaFree(h->d_quad_pp); cudaFree(h->d_tiles_ll); cudaFree(h->d_tiles_all);
     if (h->shared && h->shared->refs.fetch_sub(1) == 1) {       // the last handle of this problem
         // the pointers of the handle are the shared ones unless create failed half-way
         cudaFree(h->d_image); cudaFree(h->d_wmask); cudaFree(h->d_pix_ll); cudaFree(h->d_pix_all); cudaFree(h->d_gtaps);

@@ -109,6 +109,9 @@ struct TraceArgs {
     const uint32_t *pix;   // [npix] packed (row << 16) | column
     const float4 *quad;    // [nq_pad] (xi, eta, w, w - w'), zero-weight padding up to a multiple of R (even);
                            // w' = embedded rule of lensed_set_error_rule (0 before it is set)
+    const float4 *quad_pp; // the same rule laid out for the specialised tracers' pixel pairs: passes of np_pp
+                           // points, each padded with zero-weight entries to 4 (np_pp <= 4) or 8 entries
+    int nq_pp, np_pp;      // entries of quad_pp; rule points per pass (trace_pick_np)
     float *err;            // [.][H*W] quadrature error estimates instead of L (trace.cu ERR), or NULL
     uint32_t *fixmask;     // [nvec][blocks per vector][256] or NULL: per tracer thread, bit i = its i-th
                            // pixel (list index block base + 256 i + thread) wants the FP64 refinement (refine.cu)
@@ -182,7 +185,8 @@ cudaError_t launch_deflect(const Program &prog, const float *params, int B, cons
 cudaError_t launch_image_plane_prior(const Program &prog, const int *par_offs, int n_src, float *params, int B,
                                      cudaStream_t st);
 cudaError_t conv_setup();                 // one-time function attributes
-int trace_pick_R(int n_quad);             // rays per register block for an n_quad-point rule
+int trace_pick_R(int n_quad);             // rays per register block for an n_quad-point rule (ray pairs)
+int trace_pick_np(int n_quad);            // rule points per pass for the pixel-pair tracers
 size_t trace_smem_bytes(const Program &prog, int nq_pad);
 // shape: 0 narrow (128 threads, 64 x 64 tiles, 2 blocks per SM), 1 wide (256 threads, 64 x 128), 2 strip
 // (8 independent warps, 16 x 64 strips)

@@ -197,6 +197,21 @@ int trace_pick_R(int n_quad)
     return best;
 }
 
+// Rule points per pass of the pixel-pair tracers (trace_static.cuh), NP in {2, 3, 4, 5}: the
+// least padded rule length, the larger NP on ties (4 -> 4, 9 -> 3, 16 -> 4, 25 -> 5, 49 -> 5).
+int trace_pick_np(int n_quad)
+{
+#ifdef LENSED_TRACE_FORCE_NP           // tuning builds (build.py defines=...)
+    return LENSED_TRACE_FORCE_NP;
+#endif
+    int best = 2, best_pad = 1 << 30;
+    for (int np = 2; np <= 5; ++np) {
+        const int pad = (n_quad + np - 1) / np * np;
+        if (pad <= best_pad) { best = np; best_pad = pad; }
+    }
+    return best;
+}
+
 namespace {
 
 // every static signature; a NULL err only asks whether the signature matches

@@ -51,6 +51,61 @@ __device__ __forceinline__ void load_pairs(const float *row, f2 (&out)[NP])
     }
 }
 
+// NP consecutive scalars of one table row (16-byte aligned start)
+template <int NP>
+__device__ __forceinline__ void load_scalars(const float *row, float (&out)[NP])
+{
+    static_assert(NP <= 8, "at most eight points per pass");
+    const float4 t = *reinterpret_cast<const float4 *>(row);
+    const float v[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+    for (int i = 0; i < NP && i < 4; ++i) out[i] = v[i];
+    if constexpr (NP > 4) {
+        const float4 t2 = *reinterpret_cast<const float4 *>(row + 4);
+        const float v2[4] = {t2.x, t2.y, t2.z, t2.w};
+#pragma unroll
+        for (int i = 4; i < NP; ++i) out[i] = v2[i - 4];
+    }
+}
+
+// Two ways to fill a packed pair, chosen by the type of the frame origin:
+//   float origin  "ray pairs":   the pair = two consecutive rule points of ONE pixel
+//                 (interpreting tracer): table entries come as pairs, the origin is broadcast;
+//   f2 origin     "pixel pairs": the pair = the SAME rule point of TWO pixels (specialised
+//                 tracers): the table entry is broadcast, the origins come as a pair.  No rule is
+//                 padded to an even length, per-pixel arithmetic is packed too, and a table row is
+//                 read once for both pixels.
+template <int NP>
+__device__ __forceinline__ void enter(const float *row, float origin, f2 (&out)[NP])
+{
+    f2 p[NP];
+    load_pairs<NP>(row, p);
+#pragma unroll
+    for (int k = 0; k < NP; ++k) out[k] = add2(p[k], bc(origin));
+}
+template <int NP>
+__device__ __forceinline__ void enter(const float *row, f2 origin, f2 (&out)[NP])
+{
+    float t[NP];
+    load_scalars<NP>(row, t);
+#pragma unroll
+    for (int k = 0; k < NP; ++k) out[k] = add2(bc(t[k]), origin);
+}
+// rule weights of a pass, as the multiplicand of the pixel sum
+template <int NP>
+__device__ __forceinline__ void pass_weights(const float *row, float, f2 (&out)[NP]) { load_pairs<NP>(row, out); }
+template <int NP>
+__device__ __forceinline__ void pass_weights(const float *row, f2, f2 (&out)[NP])
+{
+    float t[NP];
+    load_scalars<NP>(row, t);
+#pragma unroll
+    for (int k = 0; k < NP; ++k) out[k] = bc(t[k]);
+}
+// running minimum of a squared radius: per pixel
+__device__ __forceinline__ void min_radius(float &rmin, f2 r2) { rmin = min3(rmin, lo2(r2), hi2(r2)); }
+__device__ __forceinline__ void min_radius(float2 &rmin, f2 r2) { rmin.x = fminf(rmin.x, lo2(r2)); rmin.y = fminf(rmin.y, hi2(r2)); }
+
 // ---- minimax tables (gen_poly.py beside this file prints them with their errors) ---------
 // atan(z)/z and (2/ln 2) atanh(z)/z in t = z^2 on [0, T]; highest degree first.  The tables
 // marked "in s" are monomials in s = (2/T) t - 1: FP32 Horner in t itself loses up to 1e-5
@@ -168,20 +223,35 @@ __device__ __forceinline__ void sie_origin(const float4 *d, float jf, float rf, 
     v0 = fmaf(c1.x, dy, -c1.y * dx);
 }
 
+// the same origins for two pixels at once (pixel pairs): jf, rf = (column, row) of both
+__device__ __forceinline__ void centre_offset(const float4 &c0, f2 jf, f2 rf, f2 &dx, f2 &dy)
+{
+    dx = add2(add2(jf, bc(-c0.x)), bc(-c0.y));
+    dy = add2(add2(rf, bc(-c0.z)), bc(-c0.w));
+}
+__device__ __forceinline__ void sie_origin(const float4 *d, f2 jf, f2 rf, f2 &u0, f2 &v0)
+{
+    f2 dx, dy;
+    centre_offset(d[0], jf, rf, dx, dy);
+    const float4 c1 = d[1];
+    u0 = fma2(bc(c1.x), dx, mul2(bc(c1.y), dy));
+    v0 = fma2(bc(c1.x), dy, mul2(bc(-c1.y), dx));
+}
+
 // RAW: leave (atan, atanh-in-lg2-units) themselves in (r.ax, r.ay) instead of accumulating the
 // deflection: the sources then subtract B (atan, atanh), B = M_source x [amplitudes, rotation]
 // (trace_static.cuh "direct frames").
-template <int NP, int MODE, bool RAW = false>
-__device__ __forceinline__ void lens_sie(const float4 *d, const float *tu, const float *tv, float u0, float v0,
+template <int NP, int MODE, bool RAW = false, class O = float>
+__device__ __forceinline__ void lens_sie(const float4 *d, const float *tu, const float *tv, O u0, O v0,
                                          Rays<NP> &r)
 {
     const float4 c1 = d[1], c2 = d[2];
     f2 pu[NP], pv[NP];
-    load_pairs<NP>(tu, pu);
-    load_pairs<NP>(tv, pv);
+    enter<NP>(tu, u0, pu);
+    enter<NP>(tv, v0, pv);
 #pragma unroll
     for (int k = 0; k < NP; ++k) {
-        const f2 u = add2(pu[k], bc(u0)), v = add2(pv[k], bc(v0));
+        const f2 u = pu[k], v = pv[k];
         const f2 psi2 = fma2(mul2(u, bc(c1.z)), u, mul2(v, v));
         const f2 ipsi = map2(psi2, [](float x) { return mufu_rsq(fmaxf(x, kTiny)); });
         const f2 s = mul2(ipsi, bc(c1.w));
@@ -205,17 +275,22 @@ __device__ __forceinline__ void circular_origin(const float4 *d, float jf, float
     centre_offset(d[0], jf, rf, u0, v0);
 }
 
-template <int NP, bool POINT>
-__device__ __forceinline__ void lens_circular(const float4 *d, const float *tu, const float *tv, float u0, float v0,
+__device__ __forceinline__ void circular_origin(const float4 *d, f2 jf, f2 rf, f2 &u0, f2 &v0)
+{
+    centre_offset(d[0], jf, rf, u0, v0);
+}
+
+template <int NP, bool POINT, class O = float>
+__device__ __forceinline__ void lens_circular(const float4 *d, const float *tu, const float *tv, O u0, O v0,
                                               Rays<NP> &r)
 {
     const float amp = d[1].x;
     f2 pu[NP], pv[NP];
-    load_pairs<NP>(tu, pu);
-    load_pairs<NP>(tv, pv);
+    enter<NP>(tu, u0, pu);
+    enter<NP>(tv, v0, pv);
 #pragma unroll
     for (int k = 0; k < NP; ++k) {
-        const f2 u = add2(pu[k], bc(u0)), v = add2(pv[k], bc(v0));
+        const f2 u = pu[k], v = pv[k];
         const f2 r2 = fma2(u, u, mul2(v, v));
         const f2 inv = map2(r2, [](float x) { return POINT ? mufu_rcp(fmaxf(x, kTiny)) : mufu_rsq(fmaxf(x, kTiny)); });
         const f2 s = mul2(inv, bc(amp));
@@ -236,15 +311,23 @@ __device__ __forceinline__ void shear_origin(const float4 *d, float jf, float rf
     v0 = fmaf(c0.y, x0, -c0.x * y0);
 }
 
-template <int NP, bool INIT>
-__device__ __forceinline__ void lens_shear(const float *tu, const float *tv, float u0, float v0, Rays<NP> &r)
+__device__ __forceinline__ void shear_origin(const float4 *d, f2 jf, f2 rf, float cxh, float cyh, f2 &u0, f2 &v0)
+{
+    const float4 c0 = d[0];
+    const f2 x0 = add2(jf, bc(-cxh)), y0 = add2(rf, bc(-cyh));
+    u0 = fma2(bc(c0.x), x0, mul2(bc(c0.y), y0));
+    v0 = fma2(bc(c0.y), x0, mul2(bc(-c0.x), y0));
+}
+
+template <int NP, bool INIT, class O = float>
+__device__ __forceinline__ void lens_shear(const float *tu, const float *tv, O u0, O v0, Rays<NP> &r)
 {
     f2 pu[NP], pv[NP];
-    load_pairs<NP>(tu, pu);
-    load_pairs<NP>(tv, pv);
+    enter<NP>(tu, u0, pu);
+    enter<NP>(tv, v0, pv);
 #pragma unroll
     for (int k = 0; k < NP; ++k) {
-        const f2 a = add2(pu[k], bc(u0)), b = add2(pv[k], bc(v0));
+        const f2 a = pu[k], b = pv[k];
         r.ax[k] = INIT ? a : add2(r.ax[k], a);
         r.ay[k] = INIT ? b : add2(r.ay[k], b);
     }
@@ -265,22 +348,31 @@ __device__ __forceinline__ void light_origin(const float4 *d, float jf, float rf
     v0 = fmaf(c1.z, dx, c1.w * dy);
 }
 
+__device__ __forceinline__ void light_origin(const float4 *d, f2 jf, f2 rf, f2 &u0, f2 &v0)
+{
+    f2 dx, dy;
+    centre_offset(d[0], jf, rf, dx, dy);
+    const float4 c1 = d[1];
+    u0 = fma2(bc(c1.x), dx, mul2(bc(c1.y), dy));
+    v0 = fma2(bc(c1.z), dx, mul2(bc(c1.w), dy));
+}
+
 // cm: the 2 x 2 matrix applied to (r.ax, r.ay) of a source -- the frame M itself (d[1]) when
 // they hold the deflection, B when they hold the SIE's raw functions.
 // rmin (source Sersic only): running minimum of (R/r_S)^2 over the rays of the pixel; the caller
 // compares it with the block's T2 (lensed_internal.h) to flag the pixel for the FP64 refinement.
-template <int NP, bool SRC, bool GAUSS, bool INIT>
-__device__ __forceinline__ void light_profile(const float4 *d, const float *tu, const float *tv, float u0, float v0,
-                                              Rays<NP> &r, const float4 *cm, float &rmin)
+template <int NP, bool SRC, bool GAUSS, bool INIT, class O = float, class RM = float>
+__device__ __forceinline__ void light_profile(const float4 *d, const float *tu, const float *tv, O u0, O v0,
+                                              Rays<NP> &r, const float4 *cm, RM &rmin)
 {
     const float4 c1 = cm ? cm[0] : d[1], c2 = d[2];
     const float nk = -c2.y;
     f2 pu[NP], pv[NP];
-    load_pairs<NP>(tu, pu);
-    load_pairs<NP>(tv, pv);
+    enter<NP>(tu, u0, pu);
+    enter<NP>(tv, v0, pv);
 #pragma unroll
     for (int k = 0; k < NP; ++k) {
-        f2 u = add2(pu[k], bc(u0)), v = add2(pv[k], bc(v0));
+        f2 u = pu[k], v = pv[k];
         if (SRC) {
             u = fma2(r.ay[k], bc(-c1.y), fma2(r.ax[k], bc(-c1.x), u));
             v = fma2(r.ay[k], bc(-c1.w), fma2(r.ax[k], bc(-c1.z), v));
@@ -291,7 +383,7 @@ __device__ __forceinline__ void light_profile(const float4 *d, const float *tu, 
             x = fma2(r2, bc(nk), bc(c2.x));
         } else {
 #ifndef LENSED_NO_FLAG                  // tuning builds: what the flagging costs
-            if (SRC) rmin = min3(rmin, lo2(r2), hi2(r2));
+            if (SRC) min_radius(rmin, r2);
 #endif
             const f2 lg = map2(r2, [](float a) { return mufu_lg2(a); });
             const f2 e = map2(mul2(lg, bc(c2.z)), [](float a) { return mufu_ex2(a); });

@@ -246,6 +246,209 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
     if (a.fixmask) a.fixmask[((size_t)vec * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = flags;
 }
 
+// ---- pixel pairs ------------------------------------------------------------------------------
+// The specialised tracers work on PAIRS OF PIXELS: a thread takes its list entries two at a time
+// (ip, ip + 256) and a packed register pair holds the same rule point of both (trace_math.cuh
+// "enter").  Against pairs of rule points of one pixel: (1) no rule is padded to an even number of
+// points -- 9-, 25- and 49-point rules lose 10 %, 12 % and 2 % of padding; (2) the per-pixel
+// arithmetic (frame origins, the foreground expansion, the final sums) is packed as well; (3) a
+// table row is read once for two pixels, as scalars that enter as broadcast operands.  NP = rule
+// points per pass, each pass a 16-byte-aligned stretch of NPP = 4 (NP <= 4) or 8 table entries
+// (api.cu lays the rule out that way for these kernels: TraceArgs::quad / nq_pad as the static
+// launcher sets them).
+#ifndef LENSED_PIXEL_PAIRS
+#define LENSED_PIXEL_PAIRS 1
+#endif
+
+__device__ __forceinline__ void keep(f2 &x) { asm volatile("" : "+l"(x.v)); }
+
+// fg_expansion for two pixels at once (same expressions, packed; MUFU per half)
+__device__ __forceinline__ f2 fg_expansion(const float4 *d, const FgMoments &m, f2 a, f2 b, f2 s0, bool full)
+{
+    const float4 c2 = d[2];                              // log2 I0, b_n log2 e, 1/(2n)
+    const float c = c2.z;
+    const f2 e = map2(mul2(map2(s0, [](float x) { return mufu_lg2(x); }), bc(c)), [](float x) { return mufu_ex2(x); });
+    const f2 F = map2(fma2(e, bc(-c2.y), bc(c2.x)), [](float x) { return mufu_ex2(x); });
+    const f2 is = map2(s0, [](float x) { return mufu_rcp(x); });
+    const f2 h1 = mul2(mul2(e, bc(-(c2.y * 0.69314718056f) * c)), is);            // dh/ds = -b_n c s^(c-1)
+    const f2 h2 = mul2(mul2(h1, bc(c - 1.0f)), is);
+    const f2 h11 = mul2(h1, h1);
+    const f2 aa = mul2(a, a), ab = mul2(a, b), bb = mul2(b, b);
+    const f2 EL2 = mul2(fma2(aa, bc(m.S11), fma2(ab, bc(2.0f * m.S12), mul2(bb, bc(m.S22)))), bc(4.0f));
+    if (!full) return fma2(F, fma2(h1, bc(m.S11 + m.S22), mul2(mul2(add2(h11, h2), bc(0.5f)), EL2)), F);
+    const f2 h3 = mul2(mul2(h2, bc(c - 2.0f)), is), h4 = mul2(mul2(h3, bc(c - 3.0f)), is);
+    const f2 F2 = add2(h11, h2);
+    const f2 F3 = add2(mul2(h1, fma2(h2, bc(3.0f), h11)), h3);
+    const f2 F4 = add2(fma2(h11, fma2(h2, bc(6.0f), h11), mul2(mul2(h2, h2), bc(3.0f))), fma2(mul2(h1, h3), bc(4.0f), h4));
+    const float EQ = m.S11 + m.S22, EQ2 = m.T0 + 2.0f * m.T2 + m.T4;
+    const f2 EL2Q = mul2(fma2(aa, bc(m.T0 + m.T2), fma2(ab, bc(2.0f * (m.T1 + m.T3)), mul2(bb, bc(m.T2 + m.T4)))), bc(4.0f));
+    const f2 q1 = fma2(aa, bc(m.T0), fma2(ab, bc(4.0f * m.T1), mul2(bb, bc(6.0f * m.T2))));
+    const f2 q2 = fma2(ab, bc(4.0f * m.T3), mul2(bb, bc(m.T4)));
+    const f2 EL4 = mul2(fma2(aa, q1, mul2(bb, q2)), bc(16.0f));
+    f2 corr = mul2(h1, bc(EQ));
+    corr = fma2(mul2(F2, bc(0.5f)), add2(EL2, bc(EQ2)), corr);
+    corr = fma2(mul2(F3, bc(0.5f)), EL2Q, corr);
+    corr = fma2(mul2(F4, bc(1.0f / 24.0f)), EL4, corr);
+    return fma2(F, corr, F);
+}
+
+template <int NP, class S, int MODE>
+__device__ __forceinline__ void trace_pixel_pairs(const Program &prog, const TraceArgs &a, const TraceBlock &tb, float *Lb, int vec)
+{
+    constexpr int NPP = NP <= 4 ? 4 : 8;
+    constexpr int NL = S::n_lens, NPOS = S::n_pos;
+    constexpr int L_SIE = S::n_shear, L_SIS = L_SIE + S::n_sie, L_PT = L_SIS + S::n_sis;
+    constexpr int G_SG = S::n_ss, G_FS = G_SG + S::n_sg, G_FG = G_FS + S::n_fs;
+    const int nq = a.nq_pad;
+    const float4 *sder = tb.sder;
+    const float *ltab = tb.stab + 2 * nq;
+    const float *gtab = tb.stab + (size_t)(2 * (1 + NL)) * nq;
+
+    const int base = blockIdx.x * a.pix_per_block;
+    const int end = min(base + a.pix_per_block, a.npix);
+    // this thread's flags: bit i = its i-th pixel (list index base + 256 i + thread) has a ray inside a
+    // source Sersic's cusp zone (refine.cu); one loop pass takes pixels 2n and 2n + 1
+    uint32_t flags = 0, bit = 1;
+#pragma unroll 1
+    for (int ip = base + threadIdx.x; ip < end; ip += 2 * kTraceThreads, bit <<= 2) {
+        const bool two = ip + kTraceThreads < end;           // the list is odd for this thread: second pixel = the first again
+        const uint32_t rcA = a.pix[ip], rcB = a.pix[two ? ip + kTraceThreads : ip];
+        const int rowA = (int)(rcA >> 16), colA = (int)(rcA & 0xffffu), rowB = (int)(rcB >> 16), colB = (int)(rcB & 0xffffu);
+        const f2 jf = mk2((float)colA, (float)colB), rf = mk2((float)rowA, (float)rowB);
+        float2 rmin[S::n_ss > 0 ? S::n_ss : 1];
+#pragma unroll
+        for (int i = 0; i < S::n_ss; ++i) rmin[i] = make_float2(3e38f, 3e38f);
+        float2 rdummy = make_float2(0.0f, 0.0f);
+
+        f2 lu[NL > 0 ? NL : 1], lv[NL > 0 ? NL : 1], gu[NPOS > 0 ? NPOS : 1], gv[NPOS > 0 ? NPOS : 1];
+        if (S::n_shear) shear_origin(sder + S::lens_off4(0), jf, rf, a.cxh, a.cyh, lu[0], lv[0]);
+#pragma unroll
+        for (int i = 0; i < S::n_sie; ++i) sie_origin(sder + S::lens_off4(L_SIE + i), jf, rf, lu[L_SIE + i], lv[L_SIE + i]);
+#pragma unroll
+        for (int i = 0; i < S::n_sis + S::n_point; ++i)
+            circular_origin(sder + S::lens_off4(L_SIS + i), jf, rf, lu[L_SIS + i], lv[L_SIS + i]);
+#pragma unroll
+        for (int i = 0; i < NPOS; ++i) light_origin(sder + S::light_off4(i), jf, rf, gu[i], gv[i]);
+        if (S::direct && S::n_shear) {
+#pragma unroll
+            for (int i = 0; i < S::n_src; ++i) {              // sources come first among the lights
+                const float4 M = sder[S::light_off4(i) + 1];
+                gu[i] = fma2(lu[0], bc(-M.x), fma2(lv[0], bc(-M.y), gu[i]));
+                gv[i] = fma2(lu[0], bc(-M.z), fma2(lv[0], bc(-M.w), gv[i]));
+            }
+        }
+        // per-pixel values: keep ptxas from recomputing them inside the ray loop to save registers
+#pragma unroll
+        for (int i = 0; i < NL; ++i) { keep(lu[i]); keep(lv[i]); }
+#pragma unroll
+        for (int i = 0; i < S::n_src; ++i) { keep(gu[i]); keep(gv[i]); }
+
+        // foreground Sersics: moment expansion where it holds for both pixels, else the per-ray sum
+        f2 fg = bc(0.0f);
+#pragma unroll
+        for (int i = 0; i < S::n_fs; ++i) {
+            const float4 *d = sder + S::light_off4(G_FS + i);
+            const f2 s0 = fma2(gu[G_FS + i], gu[G_FS + i], mul2(gv[G_FS + i], gv[G_FS + i]));
+            const float4 rng = d[3];
+            const float sA = lo2(s0), sB = hi2(s0);
+            if (sA >= rng.x && sA <= rng.y && sB >= rng.x && sB <= rng.y) {
+                const bool full = !(sA >= rng.z && sA <= rng.w && sB >= rng.z && sB <= rng.w);
+                fg = add2(fg, fg_expansion(d, tb.sfgx[i], gu[G_FS + i], gv[G_FS + i], s0, full));
+            } else {
+                f2 accf = bc(0.0f);
+#pragma unroll 1
+                for (int q0 = 0; q0 < nq; q0 += NPP) {
+                    Rays<NP> rf_;
+                    light_profile<NP, false, false, true>(d, gtab + (size_t)(2 * (G_FS + i)) * nq + q0,
+                                                          gtab + (size_t)(2 * (G_FS + i) + 1) * nq + q0, gu[G_FS + i],
+                                                          gv[G_FS + i], rf_, nullptr, rdummy);
+                    f2 w[NP];
+                    pass_weights<NP>(tb.sw + q0, s0, w);
+#pragma unroll
+                    for (int k = 0; k < NP; ++k) accf = fma2(w[k], rf_.I[k], accf);
+                }
+                fg = add2(fg, accf);
+            }
+        }
+
+        f2 acc = bc(0.0f);
+#pragma unroll 1
+        for (int q0 = 0; q0 < nq; q0 += NPP) {
+            Rays<NP> r;
+            if (S::direct) {
+                // (ax, ay) are set by the SIE below
+            } else if (S::n_shear) {
+                lens_shear<NP, true>(ltab + q0, ltab + nq + q0, lu[0], lv[0], r);
+            } else {
+#pragma unroll
+                for (int k = 0; k < NP; ++k) { r.ax[k] = bc(0.0f); r.ay[k] = bc(0.0f); }
+            }
+#pragma unroll
+            for (int i = 0; i < S::n_sie; ++i) {
+                const int m = L_SIE + i;
+                lens_sie<NP, MODE, S::direct>(sder + S::lens_off4(m), ltab + (size_t)(2 * m) * nq + q0,
+                                              ltab + (size_t)(2 * m + 1) * nq + q0, lu[m], lv[m], r);
+            }
+#pragma unroll
+            for (int i = 0; i < S::n_sis; ++i) {
+                const int m = L_SIS + i;
+                lens_circular<NP, false>(sder + S::lens_off4(m), tb.stab + q0, tb.stab + nq + q0, lu[m], lv[m], r);
+            }
+#pragma unroll
+            for (int i = 0; i < S::n_point; ++i) {
+                const int m = L_PT + i;
+                lens_circular<NP, true>(sder + S::lens_off4(m), tb.stab + q0, tb.stab + nq + q0, lu[m], lv[m], r);
+            }
+            if (NPOS - S::n_fs == 0) {
+#pragma unroll
+                for (int k = 0; k < NP; ++k) r.I[k] = bc(0.0f);
+            }
+#define LENSED_LIGHT(m, SRC, GAUSS, INIT)                                                                 \
+    do {                                                                                                  \
+        if constexpr ((SRC) && !(GAUSS))                                                                  \
+            light_profile<NP, SRC, GAUSS, INIT>(sder + S::light_off4(m), gtab + (size_t)(2 * (m)) * nq + q0,      \
+                                                gtab + (size_t)(2 * (m) + 1) * nq + q0, gu[m], gv[m], r,          \
+                                                S::direct ? tb.smat + (m) : nullptr, rmin[(m) < S::n_ss ? (m) : 0]); \
+        else                                                                                              \
+            light_profile<NP, SRC, GAUSS, INIT>(sder + S::light_off4(m), gtab + (size_t)(2 * (m)) * nq + q0,      \
+                                                gtab + (size_t)(2 * (m) + 1) * nq + q0, gu[m], gv[m], r,          \
+                                                (SRC) && S::direct ? tb.smat + (m) : nullptr, rdummy);    \
+    } while (0)
+            constexpr bool fg_first = S::n_fg > 0;
+#pragma unroll
+            for (int i = 0; i < S::n_fg; ++i) {
+                if (i == 0) LENSED_LIGHT(G_FG + i, false, true, true);
+                else LENSED_LIGHT(G_FG + i, false, true, false);
+            }
+#pragma unroll
+            for (int i = 0; i < S::n_ss; ++i) {
+                if (i == 0 && !fg_first) LENSED_LIGHT(i, true, false, true);
+                else LENSED_LIGHT(i, true, false, false);
+            }
+#pragma unroll
+            for (int i = 0; i < S::n_sg; ++i) {
+                if (i == 0 && !fg_first && S::n_ss == 0) LENSED_LIGHT(G_SG + i, true, true, true);
+                else LENSED_LIGHT(G_SG + i, true, true, false);
+            }
+#undef LENSED_LIGHT
+            f2 w[NP];
+            pass_weights<NP>(tb.sw + q0, acc, w);
+#pragma unroll
+            for (int k = 0; k < NP; ++k) acc = fma2(w[k], r.I[k], acc);
+        }
+        const f2 total = add2(add2(acc, fg), bc(tb.sky));
+        store_pixel(a, Lb, rowA, colA, lo2(total));
+        if (two) store_pixel(a, Lb, rowB, colB, hi2(total));
+#pragma unroll
+        for (int i = 0; i < S::n_ss; ++i) {
+            const float T2 = sder[S::light_off4(i) + 2].w;
+            if (rmin[i].x < T2) flags |= bit;
+            if (two && rmin[i].y < T2) flags |= bit << 1;
+        }
+    }
+    if (a.fixmask) a.fixmask[((size_t)vec * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = flags;
+}
+
 // MINB = resident blocks per SM the register budget is cut for (3 -> 80 registers, 2 -> 128):
 // chosen per signature where it was measured (profiles/r1f.md)
 template <int NP, class S, int MINB>
@@ -298,24 +501,44 @@ __global__ void __launch_bounds__(kTraceThreads, MINB * (256 / kTraceThreads)) t
         __syncthreads();
     }
     float *Lb = a.L + (size_t)vec * a.l_stride;
+#if LENSED_PIXEL_PAIRS
+#define LENSED_TRACE_BODY trace_pixel_pairs
+#else
+#define LENSED_TRACE_BODY trace_pixels
+#endif
     if constexpr (S::n_sie == 0) {
-        trace_pixels<NP, S, 0>(prog, a, tb, Lb, vec);
+        LENSED_TRACE_BODY<NP, S, 0>(prog, a, tb, Lb, vec);
     } else {
         switch ((int)tb.sder[0].y) {              // SieMode of the vector (prep.cu), block-uniform
-        case 0: trace_pixels<NP, S, 0>(prog, a, tb, Lb, vec); break;
-        case 1: trace_pixels<NP, S, 1>(prog, a, tb, Lb, vec); break;
-        case 2: trace_pixels<NP, S, 2>(prog, a, tb, Lb, vec); break;
-        case 3: trace_pixels<NP, S, 3>(prog, a, tb, Lb, vec); break;
-        case 4: trace_pixels<NP, S, 4>(prog, a, tb, Lb, vec); break;
-        default: trace_pixels<NP, S, 5>(prog, a, tb, Lb, vec); break;
+        case 0: LENSED_TRACE_BODY<NP, S, 0>(prog, a, tb, Lb, vec); break;
+        case 1: LENSED_TRACE_BODY<NP, S, 1>(prog, a, tb, Lb, vec); break;
+        case 2: LENSED_TRACE_BODY<NP, S, 2>(prog, a, tb, Lb, vec); break;
+        case 3: LENSED_TRACE_BODY<NP, S, 3>(prog, a, tb, Lb, vec); break;
+        case 4: LENSED_TRACE_BODY<NP, S, 4>(prog, a, tb, Lb, vec); break;
+        default: LENSED_TRACE_BODY<NP, S, 5>(prog, a, tb, Lb, vec); break;
         }
     }
+#undef LENSED_TRACE_BODY
 }
 
-// R = rays per register block (2 NP); only the R values trace_pick_R can return
+// Pixel pairs: NP = rule points per pass (TraceArgs::np_pp, from trace_pick_np), on the rule laid out
+// in passes (quad_pp, nq_pp).  Ray pairs (LENSED_PIXEL_PAIRS=0): R = 2 NP rays per register block.
 template <class S, int MINB>
-cudaError_t launch_trace_static(const Program &prog, const TraceArgs &a, int R, int nvec, cudaStream_t st)
+cudaError_t launch_trace_static(const Program &prog, const TraceArgs &a0, int R, int nvec, cudaStream_t st)
 {
+#if LENSED_PIXEL_PAIRS
+    TraceArgs a = a0;
+    a.quad = a0.quad_pp;
+    a.nq_pad = a0.nq_pp;
+    switch (a0.np_pp) {
+    case 2: return launch_trace_kernel(trace_static_kernel<2, S, MINB>, prog, a, nvec, st);
+    case 3: return launch_trace_kernel(trace_static_kernel<3, S, MINB>, prog, a, nvec, st);
+    case 4: return launch_trace_kernel(trace_static_kernel<4, S, MINB>, prog, a, nvec, st);
+    case 5: return launch_trace_kernel(trace_static_kernel<5, S, MINB>, prog, a, nvec, st);
+    default: return cudaErrorInvalidValue;
+    }
+#else
+    const TraceArgs &a = a0;
     switch (R) {
     case 2: return launch_trace_kernel(trace_static_kernel<1, S, MINB>, prog, a, nvec, st);
     case 4: return launch_trace_kernel(trace_static_kernel<2, S, MINB>, prog, a, nvec, st);
@@ -324,6 +547,7 @@ cudaError_t launch_trace_static(const Program &prog, const TraceArgs &a, int R, 
     case 10: return launch_trace_kernel(trace_static_kernel<5, S, MINB>, prog, a, nvec, st);
     default: return cudaErrorInvalidValue;
     }
+#endif
 }
 
 // Defines  bool NAME(counts, prog, args, R, nvec, stream, &err): false if the signature does
