@@ -278,7 +278,7 @@ lensed_status build_tiles(lensed_handle *h, int shape)
 }
 
 // Shape lensed_create picks, from the pixels each shape's tile list computes (tiles x tile area)
-// and what was measured on the configs (profiles/r2b.md, r2e.md).  With full tiles the wide shape
+// and what was measured on the configs (profiles/r2b.md).  With full tiles the wide shape
 // is the fastest (31 x 31 PSF, 4096 Euclid vectors: wide 32.5, narrow 35.0, strip 35.3 ms: the
 // strip shape's unsynchronised warps miss the constant cache on the taps more often than a
 // block's lock-step warps).  A masked or small image goes to the shape that computes at least

@@ -24,7 +24,7 @@
 // tensor copy (cp.async.bulk.tensor.3d over (x, y, vector), completion on an mbarrier), double
 // buffered: item i+1 loads while item i is convolved (single buffer when two do not fit: PSFs
 // beyond ~45 x 45).  Against 256 threads x cp.async 16 B with an integer divide per element
-// (LENSED_CONV_TMA=0) the tensor copy is worth 0.8 % at 31 x 31 and 5-9 % at 9 x 9 ... 21 x 21
+// (LENSED_CONV_TMA=0) the tensor copy is worth 0.7 % at 31 x 31 and 3-11 % at 9 x 9 ... 21 x 21
 // (profiles/r2b.md).
 //
 // Thread tile: 4 rows x 8 columns of outputs (two 4-column groups 64 columns apart, so that

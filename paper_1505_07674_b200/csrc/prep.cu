@@ -259,7 +259,7 @@ __global__ void __launch_bounds__(kMaxModels * kPrepVec) prep_kernel(Program pro
 // vectors outside the model domain last.  The specialised tracers hold one straight-line copy of
 // the ray loop per mode (trace_static.cuh); with the vectors of a launch in arbitrary order the
 // blocks resident at one time run all six copies and miss the instruction cache (HST config:
-// `no_instruction` 2.8 stall cycles per issue, profiles/r2c.md).  Stable counting sort, one block
+// `no_instruction` 2.8 stall cycles per issue, profiles/r2b.md).  Stable counting sort, one block
 // per chunk: the order is a function of the inputs.  It only changes which block works on which
 // vector -- every vector's result is what it was.
 constexpr int kOrderKeys = 7;                   // SIE modes 0..5, 6 = invalid
