@@ -50,8 +50,9 @@
 //       64 x FFMA2
 //
 // Zero padding exists only in the tap columns (KW -> multiple of 4) and in the first / last
-// tap row of each pair; the traced set is dilated by p+1 rows (api.cu) and the padded frame
-// is zero-initialised, so a zero tap never meets a non-finite stale value.
+// tap row of each pair; the traced set is dilated by p+1 rows (api.cu), the padded frame is
+// zero-initialised and the tracers clamp what they store to the finite range (store_pixel), so
+// a zero tap never meets a non-finite value.
 // Summation is blocked (per chunk, then across chunks): FP32 error growth ~ sqrt(4 KH) + sqrt(NC).
 //
 // Epilogue: loglike -> per-thread FP32 sum over its 32 pixels, then FP64: warp shuffle

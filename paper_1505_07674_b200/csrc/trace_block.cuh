@@ -77,8 +77,13 @@ __device__ __forceinline__ TraceBlock trace_prologue(const Program &prog, const 
 // L_i into the padded frame the convolution reads (conv.cu "Input"): pixel (row, col) at
 // (row + py, col + px); a border pixel also fills the pad cells that clamp to it
 // ("border pixels are repeated").
+// The value is clamped to the finite range (NaN -> -FLT_MAX): the convolution multiplies every
+// staged value by tap pairs whose partner may be a structural zero (conv.cu "Pairing"), and
+// 0 x inf would put a NaN into an output whose PSF window does not hold the pixel at all.  A pixel
+// that overflows FP32 still drives its own window to +-inf, i.e. logL to -inf.
 __device__ __forceinline__ void store_pixel(const TraceArgs &a, float *Lb, int row, int col, float v)
 {
+    v = fminf(fmaxf(v, -3.402823466e38f), 3.402823466e38f);
     Lb[(size_t)(row + a.py) * a.Wp + col + a.px] = v;
     if (row == 0 || col == 0 || row == a.H - 1 || col == a.W - 1) {
         const int r0 = row == 0 ? 0 : row + a.py, r1 = row == a.H - 1 ? a.H - 1 + 2 * a.py : row + a.py;

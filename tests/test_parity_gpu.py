@@ -230,6 +230,26 @@ def test_invalid_vectors_give_minus_infinity_and_nan_image(L):
     assert logl_errors(logl_g[~bad], logl_o[~bad]).max() <= LOGL_RTOL
 
 
+def test_a_vector_that_overflows_fp32_gives_minus_infinity_not_nan(L):
+    """A valid vector whose source flux overflows FP32 (magnitude -300): its pixels are +inf, and
+    the convolution must not turn them into NaN through a structurally zero tap (the tracers clamp
+    what they store, trace_block.cuh store_pixel): logL = -inf like any hopeless vector, the
+    other vectors of the batch are untouched."""
+    cfg = synth.shrunk(synth.get_config(1), 40, 36, 4)
+    prob = Problem(cfg)
+    params = cfg.batch(4)
+    params[2, 10] = -300.0       # source magnitude
+    h = prob.create()
+    try:
+        logl_g, model_g = _gpu_eval(L, h, params, cfg.H, cfg.W)
+    finally:
+        L.lensed_destroy(h)
+    assert np.isneginf(logl_g[2]) and not np.any(np.isnan(model_g[2]))
+    ok = np.array([True, True, False, True])
+    logl_o = prob.oracle_loglike(params[ok], want_model=False)
+    assert logl_errors(logl_g[ok], logl_o).max() <= LOGL_RTOL
+
+
 def test_fully_masked_image_and_zero_weights(L):
     cfg = synth.shrunk(synth.get_config(1), 30, 30, 3)
     prob = Problem(cfg)
