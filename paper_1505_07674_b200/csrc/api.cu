@@ -208,6 +208,35 @@ void tile_list(const std::vector<uint8_t> &cnt, int H, int W, int tw, int th, in
         }
 }
 
+// Strips of the strip shape (conv.cu): sw x sh pixels, packed (first row << 16) | first column in
+// PIXEL coordinates.  Every band of sh rows (from the first selected row on) is covered on its own:
+// strips start at the band's first selected column (rounded down to a multiple of 4) and skip
+// stretches without a selected pixel, so a round mask is hugged band by band (SLACS annulus: 23
+// strips against 25 on one grid).  *rows, *cols = extent the strips reach.
+void strip_list(const std::vector<uint8_t> &sel, int H, int W, int sw, int sh, std::vector<uint32_t> &out, int *rows, int *cols)
+{
+    out.clear();
+    *rows = *cols = 0;
+    int y0 = H;
+    for (int i = 0; i < H && y0 == H; ++i)
+        for (int j = 0; j < W; ++j)
+            if (sel[(size_t)i * W + j]) { y0 = i; break; }
+    for (int y = y0; y < H; y += sh) {
+        std::vector<uint8_t> col(W, 0);
+        for (int i = y; i < std::min(H, y + sh); ++i)
+            for (int j = 0; j < W; ++j) col[j] |= sel[(size_t)i * W + j];
+        int x = 0;
+        while (x < W) {
+            while (x < W && !col[x]) ++x;
+            if (x >= W) break;
+            x = x / 4 * 4;
+            out.push_back(((uint32_t)y << 16) | (uint32_t)x);
+            *rows = std::max(*rows, y + sh); *cols = std::max(*cols, x + sw);
+            x += sw;
+        }
+    }
+}
+
 lensed_status timed_begin(lensed_handle *h, int phase, cudaStream_t st)
 {
     h->launches[phase] += 1;
@@ -260,12 +289,23 @@ lensed_status build_tiles(lensed_handle *h, int shape)
             if (h->counted[(size_t)i * W + j]) { x0 = std::min(x0, j); y0 = std::min(y0, i); }
     h->ox_ll = x0 < W ? x0 / 4 * 4 : 0;
     h->oy_ll = y0 < H ? y0 : 0;
-    int ny_ll, nx_ll, ny_all, nx_all;
-    tile_list(h->counted, H, W, h->tile_w, h->tile_h, h->ox_ll, h->oy_ll, tiles_ll, &ny_ll, &nx_ll);
-    tile_list(all, H, W, h->tile_w, h->tile_h, 0, 0, tiles_all, &ny_all, &nx_all);
-    // padded frame: the image, and every tile of either grid with its PSF halo
-    const int rows = std::max(std::max(ny_all * h->tile_h, h->oy_ll + ny_ll * h->tile_h), H);
-    const int cols = std::max(std::max(nx_all * h->tile_w, h->ox_ll + nx_ll * h->tile_w), W);
+    int rows, cols;
+    if (shape == 2) {
+        // strips carry their own pixel coordinates (strip_list): no grid origin
+        int r1, c1, r2, c2;
+        h->ox_ll = h->oy_ll = 0;
+        strip_list(h->counted, H, W, h->tile_w, h->tile_h, tiles_ll, &r1, &c1);
+        strip_list(all, H, W, h->tile_w, h->tile_h, tiles_all, &r2, &c2);
+        rows = std::max(std::max(r1, r2), H);
+        cols = std::max(std::max(c1, c2), W);
+    } else {
+        int ny_ll, nx_ll, ny_all, nx_all;
+        tile_list(h->counted, H, W, h->tile_w, h->tile_h, h->ox_ll, h->oy_ll, tiles_ll, &ny_ll, &nx_ll);
+        tile_list(all, H, W, h->tile_w, h->tile_h, 0, 0, tiles_all, &ny_all, &nx_all);
+        // padded frame: the image, and every tile of either grid with its PSF halo
+        rows = std::max(std::max(ny_all * h->tile_h, h->oy_ll + ny_ll * h->tile_h), H);
+        cols = std::max(std::max(nx_all * h->tile_w, h->ox_ll + nx_ll * h->tile_w), W);
+    }
     conv_padded_shape(rows, cols, h->KH, h->NC, &h->Hp, &h->Wp);
     h->ntiles_ll = (int)tiles_ll.size(); h->ntiles_all = (int)tiles_all.size();
     CU(h, cudaSetDevice(h->device));
@@ -297,7 +337,8 @@ int default_shape(const lensed_handle *h)
             for (int j = 0; j < h->W; ++j)
                 if (h->counted[(size_t)i * h->W + j]) { x0 = std::min(x0, j); y0 = std::min(y0, i); }
         std::vector<uint32_t> tiles;
-        tile_list(h->counted, h->H, h->W, tw, th, x0 < h->W ? x0 / 4 * 4 : 0, y0 < h->H ? y0 : 0, tiles, &ny, &nx);
+        if (shape == 2) strip_list(h->counted, h->H, h->W, tw, th, tiles, &ny, &nx);
+        else tile_list(h->counted, h->H, h->W, tw, th, x0 < h->W ? x0 / 4 * 4 : 0, y0 < h->H ? y0 : 0, tiles, &ny, &nx);
         px[shape] = conv_shape_fits(h->KH, h->NC, shape) ? (long long)tiles.size() * tw * th : (1LL << 60);
     }
     const int block = px[0] * 100 <= px[1] * 85 ? 0 : 1;

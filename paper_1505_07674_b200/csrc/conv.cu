@@ -413,8 +413,9 @@ __global__ void __launch_bounds__(NTX * kNTY, NTX == 16 ? 1 : 2) conv_kernel(con
 // lose at their barriers -- the tile prologue (wait for the copy), the epilogue (chi-square
 // reduction) and the ramps of the chunk loops, during which a block's warps all leave the FMA pipe
 // together -- a warp here loses alone, while the other warp of its scheduler keeps the pipe busy.
-// Masked images skip work per strip instead of per tile (SLACS annulus: 62 % of the computed
-// pixels are counted instead of 49 %).  The per-thread arithmetic (thread tile 4 x 8, tap pairs,
+// Masked images skip work per strip instead of per tile, and the strips of every 16-row band
+// start at the band's own first counted column (api.cu strip_list; a.tiles holds PIXEL
+// coordinates for this shape): SLACS annulus, 68 % of the computed pixels are counted instead of 49 %.  The per-thread arithmetic (thread tile 4 x 8, tap pairs,
 // rotating rows, blocked summation) is the code of the block shapes, so the results agree with
 // theirs bit for bit per pixel; the chi-square partials are per strip.
 // Data d and weights w of the strip are read from global memory in the epilogue (L2 hits: the
@@ -452,8 +453,7 @@ __global__ void __launch_bounds__(32) conv_strip_kernel(const __grid_constant__ 
             const int t = item / a.nb, b = item - t * a.nb;
             const uint32_t tile = a.tiles[t];
             mbar_expect_tx(&s_bar[s], (unsigned)((IH - kSlackRows) * IW * sizeof(float)));
-            tma_load_3d(s_stage + (size_t)s * stage_floats, &tmap, &s_bar[s], a.ox + (int)(tile & 0xffffu) * kSW,
-                        a.oy + (int)(tile >> 16) * kSH, b);
+            tma_load_3d(s_stage + (size_t)s * stage_floats, &tmap, &s_bar[s], (int)(tile & 0xffffu), (int)(tile >> 16), b);
         }
     };
 
@@ -469,7 +469,7 @@ __global__ void __launch_bounds__(32) conv_strip_kernel(const __grid_constant__ 
         const int s = a.n_stages == 2 ? ((item - lo) & 1) : 0;
         const int t = item / a.nb, b = item - t * a.nb;
         const uint32_t tile = a.tiles[t];
-        const int oy = a.oy + (int)(tile >> 16) * kSH + ty * kTR, ox = a.ox + (int)(tile & 0xffffu) * kSW + tx * 4;
+        const int oy = (int)(tile >> 16) + ty * kTR, ox = (int)(tile & 0xffffu) + tx * 4;      // strips carry pixel coordinates
         const bool more = item + 1 < hi;
         if (a.n_stages == 2 && more) issue(item + 1, s ^ 1);      // its last readers passed the __syncwarp below
 

@@ -140,7 +140,8 @@ struct ConvArgs {
     const float *Lp;       // [nb][Hp*Wp] chunk-local padded unconvolved images (TraceArgs::L)
     const float *image;    // [H*W] d
     const float *wmask;    // [H*W] w_i, 0 where masked
-    const uint32_t *tiles; // [n_tiles] packed (tile row << 16) | tile column (active tiles)
+    const uint32_t *tiles; // [n_tiles] packed (tile row << 16) | tile column of the active tiles; for the strip shape
+                           // (first pixel row << 16) | first pixel column of each strip (api.cu strip_list)
     double *partial;       // [nb][n_tiles] chunk-local chi-square partials   (loglike)
     float *model;          // [nb][H*W] chunk-local output                    (render)
     const float *derived;  // [nb][D] chunk-local (valid flag)                (render)

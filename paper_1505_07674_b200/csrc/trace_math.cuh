@@ -253,7 +253,16 @@ __device__ __forceinline__ void lens_sie(const float4 *d, const float *tu, const
     for (int k = 0; k < NP; ++k) {
         const f2 u = pu[k], v = pv[k];
         const f2 psi2 = fma2(mul2(u, bc(c1.z)), u, mul2(v, v));
+#ifdef LENSED_RSQ_NEWTON            // tuning build: the SIE's rsqrt off the XU pipe (integer seed + packed Newton steps)
+        f2 ipsi = map2(psi2, [](float x) { return __uint_as_float(0x5f375a86u - (__float_as_uint(fmaxf(x, kTiny)) >> 1)); });
+        {
+            const f2 hx = mul2(map2(psi2, [](float x) { return fmaxf(x, kTiny); }), bc(0.5f));
+#pragma unroll
+            for (int it = 0; it < LENSED_RSQ_NEWTON; ++it) ipsi = mul2(ipsi, fma2(mul2(hx, ipsi), mul2(ipsi, bc(-1.0f)), bc(1.5f)));
+        }
+#else
         const f2 ipsi = map2(psi2, [](float x) { return mufu_rsq(fmaxf(x, kTiny)); });
+#endif
         const f2 s = mul2(ipsi, bc(c1.w));
         const f2 at = sie_atan2x<MODE>(mul2(u, s));
         const f2 lv = sie_atanh2x<MODE>(v, s, c1.w);
