@@ -223,6 +223,33 @@ class Bench:
         L.lensed_set_profiling(h, False)
         return ms, phase_ms, phase_n, t0, t1
 
+    def back_to_back(self, n=30):
+        """ms per step of n calls in a row with profiling off and no L2 flush -- how a sampler calls it --
+        issued one by one, and replayed from a CUDA graph of one step"""
+        L, torch = self.L, self.torch
+        a, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        L.lensed_loglike(self.h, self.p_dev, self.logl)
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(n):
+            L.lensed_loglike(self.h, self.p_dev, self.logl)
+        e.record()
+        torch.cuda.synchronize()
+        plain = a.elapsed_time(e) / n
+        s, g = torch.cuda.Stream(), torch.cuda.CUDAGraph()
+        with torch.cuda.stream(s):
+            L.lensed_loglike(self.h, self.p_dev, self.logl, stream=s)
+            s.synchronize()
+            with torch.cuda.graph(g, stream=s):
+                L.lensed_loglike(self.h, self.p_dev, self.logl, stream=torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(n):
+            g.replay()
+        e.record()
+        torch.cuda.synchronize()
+        return plain, a.elapsed_time(e) / n
+
     def flop_model(self, steps, phase_n):
         """algorithmic flops of ONE launch of the tracer / the convolution, averaged over its launches"""
         cfg = self.cfg
@@ -248,7 +275,9 @@ class Bench:
         per_launch = self.flop_model(steps, phase_n)
         k = self.kernels(steps, phase_ms, phase_n)
         whole = (per_launch["trace"] * phase_n["trace"] + per_launch["conv"] * phase_n["conv"]) / (sum(ms) * 1e-3) / 1e12
-        return {"config": self.index, "workload": workload_name(cfg, self.B), "logl_per_s": value,
+        b2b, graph = self.back_to_back()
+        return {"config": self.index, "ms_per_step_back_to_back": b2b, "ms_per_step_cuda_graph": graph,
+                "logl_per_s_back_to_back": self.B / (b2b * 1e-3), "workload": workload_name(cfg, self.B), "logl_per_s": value,
                 "rays_per_s": value * self.n_traced * len(cfg.quad), "ms_per_step": sum(ms) / steps, "steps": steps,
                 "tracer": self.tracer_kind, "conv_shape": self.conv_shape,
                 "trace_ms": k["trace"]["ms_per_step"], "trace_frac": k["trace"]["frac"],

@@ -100,8 +100,9 @@ def _check(status, handle=None):
 
 
 def _stream(stream):
+    """None = torch's current stream; else a torch.cuda.Stream or a raw cudaStream_t value"""
     if stream is not None:
-        return ctypes.c_void_p(int(stream))
+        return ctypes.c_void_p(int(getattr(stream, "cuda_stream", stream)))
     import torch
     return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
 

@@ -250,6 +250,44 @@ def test_a_vector_that_overflows_fp32_gives_minus_infinity_not_nan(L):
     assert logl_errors(logl_g[ok], logl_o).max() <= LOGL_RTOL
 
 
+def test_a_step_captured_into_a_cuda_graph_replays_bit_for_bit(L):
+    """After one call at a batch size (scratch at its high-water mark, no allocation left in the
+    path) lensed_loglike is a fixed sequence of kernel launches and memsets on the caller's stream:
+    it can be captured into a CUDA graph -- what a sampler does with its inner loop -- and the
+    replay writes the same bits; new parameter values in the same buffer are picked up."""
+    import torch
+    cfg = synth.shrunk(synth.get_config(2), 64, 56, 4)
+    prob = Problem(cfg)
+    params = cfg.batch(40)
+    h = prob.create()
+    try:
+        p = torch.from_numpy(params[:20]).cuda()
+        direct = torch.empty(20, dtype=torch.float32, device="cuda")
+        out = torch.empty_like(direct)
+        L.lensed_loglike(h, p, direct)
+        torch.cuda.synchronize()
+        s = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(s):
+            L.lensed_loglike(h, p, out, stream=s)
+            s.synchronize()
+            with torch.cuda.graph(g, stream=s):
+                L.lensed_loglike(h, p, out, stream=torch.cuda.current_stream())
+        out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, direct)
+        p.copy_(torch.from_numpy(params[20:]))               # the sampler's next batch, same buffers
+        g.replay()
+        torch.cuda.synchronize()
+        L.lensed_loglike(h, p, direct)
+        torch.cuda.synchronize()
+        assert torch.equal(out, direct)
+        assert logl_errors(out.cpu().numpy(), prob.oracle_loglike(params[20:], want_model=False)).max() <= LOGL_RTOL
+    finally:
+        L.lensed_destroy(h)
+
+
 def test_fully_masked_image_and_zero_weights(L):
     cfg = synth.shrunk(synth.get_config(1), 30, 30, 3)
     prob = Problem(cfg)
