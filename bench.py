@@ -6,8 +6,11 @@ fused ray-trace + surface brightness + quadrature -> PSF convolution + chi-squar
 (all rows of SURVEY.md section 8(a)).  Workload at N = 1: BASELINE.json's largest config,
 the Euclid-scale sweep (512x512 @ 0.1"/px, SIE + shear + Sersic source + Sersic lens light
 + sky, 31x31 Moffat PSF, 16-point sub4 rule) at its largest batch, B = 16384 -- the config
-north_star quotes the roofline target on.  `--config 0..4 --batch B` time the other configs
-(parity-test cases, not bench lines).
+north_star quotes the roofline target on.  The same line carries, as extras, a short row for each
+of the other configs (`per_config`: 0-3 and 5 = the paper's mock scenario; flushed, back-to-back
+and CUDA-graph step times, tracer / convolution fraction of the FP32 roofline, the oracle beside
+it), the Euclid batch sweep (`sweep`) and the likelihood rate inside the device-resident nested
+sampler (`nested_sampling`).  `--config N --batch B` time one config alone.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
 
@@ -462,7 +465,11 @@ def main():
         per_config = []
         for c, steps in ((0, 20), (1, 20), (2, 10), (3, 5), (5, 10)):
             b = Bench(lensed, torch, c, synth.get_config(c).B, local, rank, args)
-            per_config.append(b.summary(steps, 3, flush))
+            row = b.summary(steps, 3, flush)
+            if not args.no_cpu_baseline:                     # the oracle beside every row, ~3 s each
+                v, cores, n, dt = time_oracle(b.cfg, b.image, b.weight, b.params, 3.0)
+                row["cpu_oracle"] = {"logl_per_s": v, "cores": cores, "sample": "%d vectors, %.1f s" % (n, dt)}
+            per_config.append(row)
             b.close()
         nested = nested_row(lensed, torch, local)
 
