@@ -259,6 +259,9 @@ __device__ __forceinline__ void trace_pixels(const Program &prog, const TraceArg
 #ifndef LENSED_PIXEL_PAIRS
 #define LENSED_PIXEL_PAIRS 1
 #endif
+#ifndef LENSED_PIPELINE
+#define LENSED_PIPELINE 0          // tuning builds: deflection of the next pass beside the brightness of this one
+#endif
 
 __device__ __forceinline__ void keep(f2 &x) { asm volatile("" : "+l"(x.v)); }
 
@@ -372,9 +375,8 @@ __device__ __forceinline__ void trace_pixel_pairs(const Program &prog, const Tra
         }
 
         f2 acc = bc(0.0f);
-#pragma unroll 1
-        for (int q0 = 0; q0 < nq; q0 += NPP) {
-            Rays<NP> r;
+        // the two stages of a pass: deflection (FP32-pipe heavy) and brightness + rule sum (MUFU heavy)
+        auto lenses = [&](int q0, Rays<NP> &r) {
             if (S::direct) {
                 // (ax, ay) are set by the SIE below
             } else if (S::n_shear) {
@@ -399,6 +401,8 @@ __device__ __forceinline__ void trace_pixel_pairs(const Program &prog, const Tra
                 const int m = L_PT + i;
                 lens_circular<NP, true>(sder + S::lens_off4(m), tb.stab + q0, tb.stab + nq + q0, lu[m], lv[m], r);
             }
+        };
+        auto lights = [&](int q0, Rays<NP> &r) {
             if (NPOS - S::n_fs == 0) {
 #pragma unroll
                 for (int k = 0; k < NP; ++k) r.I[k] = bc(0.0f);
@@ -435,6 +439,33 @@ __device__ __forceinline__ void trace_pixel_pairs(const Program &prog, const Tra
             pass_weights<NP>(tb.sw + q0, acc, w);
 #pragma unroll
             for (int k = 0; k < NP; ++k) acc = fma2(w[k], r.I[k], acc);
+        };
+#if LENSED_PIPELINE
+        if constexpr (S::direct) {
+            // software pipeline: the SIE of pass p + 1 sits in the same loop body as the light profiles
+            // of pass p, so every warp issues a steady mix for both pipes instead of alternating
+            // between an FP32-heavy and a MUFU-heavy phase
+            Rays<NP> r, n;
+            lenses(0, n);
+#pragma unroll 1
+            for (int q0 = 0; q0 + NPP < nq; q0 += NPP) {
+#pragma unroll
+                for (int k = 0; k < NP; ++k) { r.ax[k] = n.ax[k]; r.ay[k] = n.ay[k]; }
+                lenses(q0 + NPP, n);
+                lights(q0, r);
+            }
+#pragma unroll
+            for (int k = 0; k < NP; ++k) { r.ax[k] = n.ax[k]; r.ay[k] = n.ay[k]; }
+            lights(nq - NPP, r);
+        } else
+#endif
+        {
+#pragma unroll 1
+            for (int q0 = 0; q0 < nq; q0 += NPP) {
+                Rays<NP> r;
+                lenses(q0, r);
+                lights(q0, r);
+            }
         }
         const f2 total = add2(add2(acc, fg), bc(tb.sky));
         store_pixel(a, Lb, rowA, colA, lo2(total));
