@@ -212,8 +212,11 @@ __device__ __forceinline__ void conv_chunk(f2 (&acc)[2][8], const float4 *in_r, 
         for (int e = 0; e < 8; ++e) acc[p][e] = add2(acc[p][e], part[p][e]);
 }
 
+// __maxnreg__(176) instead of __launch_bounds__: with the looser budget of (256, 1) ptxas rotates one
+// staged row through 16 MOVs per loop body (317 instructions); capped at 176 it allocates the four
+// rows without moves (301; 157 registers used, no spills) -- profiles/r2b.md.
 template <bool RENDER, int NTX, bool GT>
-__global__ void __launch_bounds__(NTX * kNTY, NTX == 16 ? 1 : 2) conv_kernel(const __grid_constant__ ConvArgs a,
+__global__ void __maxnreg__(176) conv_kernel(const __grid_constant__ ConvArgs a,
                                                                              const __grid_constant__ CUtensorMap tmap)
 {
     constexpr int kThreads = Shape<NTX>::kThreads, kGroup = Shape<NTX>::kGroup, kTW = Shape<NTX>::kTW;
