@@ -191,7 +191,7 @@ class Bench:
             lensed.lensed_set_static_tracer(self.h, 0)
         if args is not None and args.conv_shape != "auto":
             lensed.lensed_set_conv_shape(self.h, lensed.CONV_SHAPES.index(args.conv_shape))
-        self.tracer_kind = "static" if lensed.lensed_get_static_tracer(self.h) == 1 else "interpreter"
+        self.tracer_kind = ("interpreter", "static", "jit")[lensed.lensed_get_static_tracer(self.h)]
         self.conv_shape = lensed.CONV_SHAPES[lensed.lensed_get_conv_shape(self.h)]
         self.n_traced = cfg.n_traced()                       # m_d, the required set
         assert self.n_traced <= lensed.lensed_num_traced(self.h)

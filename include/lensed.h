@@ -250,17 +250,21 @@ int lensed_get_conv_shape(const lensed_handle *h);
 int lensed_uses_global_taps(const lensed_handle *h);
 void lensed_debug_force_global_taps(int on);
 
-/* Tracer selection.  The ray tracer exists as one kernel that interprets any model list
- * and as kernels specialised at compile time for eight model lists (same arithmetic,
- * straight-line code; a list matches by its per-kind counts, sky components aside:
- * SIS + Gaussian source; SIE + shear + 1 or 2 Sersic sources + Sersic lens light; 2 SIE +
- * point mass + shear + 2 Sersic + 1 Gaussian source + Sersic lens light; SIE + Sersic
- * source with / without Sersic lens light; SIE + shear + Sersic source; SIS + Sersic
- * source).  lensed_create picks the specialised
- * kernel when the list has one.  lensed_set_static_tracer(h, 0) forces the interpreting
- * kernel (tests compare the two); (h, 1) re-enables the specialised one and returns
- * LENSED_EUNSUPPORTED if the list has none.  lensed_get_static_tracer: 1 / 0 = which one
- * the next call runs, -1 for NULL.                                                      */
+/* Tracer selection.  The ray tracer exists as one kernel that interprets any model list and as
+ * kernels SPECIALISED for one list each (same arithmetic, straight-line code; a list matches by
+ * its per-kind counts, sky components aside).  Nine signatures are built in (SIS + Gaussian
+ * source; SIE + shear + 1 or 2 Sersic sources + Sersic lens light; 2 SIE + point mass + shear + 2
+ * Sersic + 1 Gaussian source + Sersic lens light; SIE + Sersic source with / without Sersic lens
+ * light; SIE + shear + Sersic source; SIS + Sersic source; 2 SIE + 2 Sersic sources + 3 Sersic
+ * foregrounds).  For any other list lensed_create compiles the specialised kernel at run time
+ * (NVRTC, a few seconds once per process; the paper compiles its kernel at run time as well,
+ * PAPER.md:149) -- lists with at most one shear, three SIEs, six lenses and eight positioned light
+ * components; beyond that, without libnvrtc, or with LENSED_JIT=0 in the environment, the
+ * interpreting kernel runs.
+ * lensed_set_static_tracer(h, 0) forces the interpreting kernel (tests compare the two); (h, 1)
+ * re-enables the specialised one and returns LENSED_EUNSUPPORTED if the list has none.
+ * lensed_get_static_tracer: which one the next call runs: 1 = built-in specialised, 2 = specialised
+ * at run time, 0 = interpreting; -1 for NULL.                                              */
 lensed_status lensed_set_static_tracer(lensed_handle *h, int on);
 int lensed_get_static_tracer(const lensed_handle *h);
 

@@ -3,6 +3,7 @@
 // Host logic only; every step of the path runs in prep.cu / trace.cu / conv.cu.
 #include "../../include/lensed.h"
 #include "lensed_internal.h"
+#include "jit.h"
 
 #include <math.h>
 #include <stdarg.h>
@@ -80,7 +81,8 @@ struct lensed_handle {
     float *d_stage_in = nullptr; size_t cap_stage_in = 0;
     float *d_stage_out = nullptr; size_t cap_stage_out = 0;
     long long chunk_bytes = 1ll << 30;
-    bool static_tracer = false;     // the model list has a compile-time-specialised tracer and may use it
+    bool static_tracer = false;     // the model list has a specialised tracer (built in, or compiled at create: jit) and may use it
+    const JitTracer *jit = nullptr; // the run-time compiled one (jit.cu), when the list has no built-in signature
 
     // instrumentation
     bool profiling = false;
@@ -423,7 +425,7 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
             ta.pix_per_block = ppb;
             ta.cxh = 0.5f * (h->W - 1); ta.cyh = 0.5f * (h->H - 1);
             if ((s = timed_begin(h, PH_TRACE, st)) != LENSED_OK) return s;
-            CU(h, launch_trace(prog, ta, h->R, nb, h->static_tracer, st));
+            CU(h, launch_trace(prog, ta, h->R, nb, h->static_tracer, h->jit, st));
             if ((s = timed_end(h, st)) != LENSED_OK) return s;
             if (refine) {
                 // FP64 re-trace of the pixels the tracer flagged (refine.cu), before the convolution
@@ -709,6 +711,18 @@ lensed_status lensed_create(int H, int W, double pixel_scale, const float *image
     CREATE_FAIL(upload(h, &h->d_pix_ll, pix_ll.data(), pix_ll.size()));
     CREATE_FAIL(upload(h, &h->d_pix_all, pix_all.data(), pix_all.size()));
     CREATE_FAIL(build_tiles(h, default_shape(h)));
+    if (!h->static_tracer) {
+        // no built-in signature for this list: specialise the tracer for it now (jit.cu); on any
+        // failure the interpreting tracer runs, as it does with LENSED_JIT=0
+        int counts[K_COUNT] = {0};
+        for (int m = 0; m < pg.n_models; ++m) counts[pg.kind[m]] += 1;
+        if (jit_wanted(counts)) {
+            std::string why;
+            h->jit = jit_get(counts, h->np_pp, h->device, &why);
+            h->static_tracer = h->jit != nullptr;
+            if (!h->jit) h->err = "run-time specialisation of the tracer not available (" + why + "): interpreting tracer";
+        }
+    }
 #undef CREATE_FAIL
     *out = h;
     return LENSED_OK;
@@ -734,7 +748,7 @@ lensed_status lensed_clone(const lensed_handle *src, lensed_handle **out)
     h->counted = src->counted;
     h->d_image = src->d_image; h->d_wmask = src->d_wmask; h->d_pix_ll = src->d_pix_ll; h->d_pix_all = src->d_pix_all;
     h->npix_ll = src->npix_ll; h->npix_all = src->npix_all;
-    h->chunk_bytes = src->chunk_bytes; h->static_tracer = src->static_tracer; h->refine_gain = src->refine_gain;
+    h->chunk_bytes = src->chunk_bytes; h->static_tracer = src->static_tracer; h->jit = src->jit; h->refine_gain = src->refine_gain;
     h->fgx_tau = src->fgx_tau; h->rule_symmetric = src->rule_symmetric; h->rule_radius = src->rule_radius;
     lensed_status s = LENSED_OK;
 #define CLONE_FAIL(expr) do { s = (expr); if (s != LENSED_OK) { g_last_error = h->err; lensed_destroy(h); return s; } } while (0)
@@ -822,7 +836,7 @@ lensed_status lensed_render_error(lensed_handle *h, const float *params_dev, int
         ta.pix_per_block = ta.npix >= (1 << 11) ? 2048 : 256;
         ta.cxh = 0.5f * (h->W - 1); ta.cyh = 0.5f * (h->H - 1);
         if ((s = timed_begin(h, PH_TRACE, st)) != LENSED_OK) return s;
-        CU(h, launch_trace(prog, ta, h->R, nb, false, st));
+        CU(h, launch_trace(prog, ta, h->R, nb, false, nullptr, st));
         if ((s = timed_end(h, st)) != LENSED_OK) return s;
     }
     return LENSED_OK;
@@ -976,13 +990,17 @@ int lensed_uses_global_taps(const lensed_handle *h) { return h ? (h->d_gtaps ? 1
 lensed_status lensed_set_static_tracer(lensed_handle *h, int on)
 {
     if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
-    if (on && !trace_has_static(h->prog))
+    if (on && !trace_has_static(h->prog) && !h->jit)
         return fail(h, LENSED_EUNSUPPORTED, "no specialised tracer for this model list");
     h->static_tracer = on != 0;
     return LENSED_OK;
 }
 
-int lensed_get_static_tracer(const lensed_handle *h) { return h ? (h->static_tracer ? 1 : 0) : -1; }
+int lensed_get_static_tracer(const lensed_handle *h)
+{
+    if (!h) return -1;
+    return !h->static_tracer ? 0 : trace_has_static(h->prog) ? 1 : 2;
+}
 
 lensed_status lensed_fma_peak(int device, int iters, double *tflops)
 {

@@ -6,8 +6,14 @@
 // for every lens here (SIS, SIE, point mass: alpha(lambda x; lambda b) = lambda alpha(x; b);
 // shear is linear in x).
 #pragma once
+#ifdef __CUDACC_RTC__              // compiled at run time by NVRTC (jit.cu): no host headers, kernels only
+typedef unsigned char uint8_t;
+typedef unsigned short uint16_t;
+typedef unsigned int uint32_t;
+#else
 #include <cuda_runtime.h>
 #include <stdint.h>
+#endif
 
 struct lensed_handle;
 
@@ -166,12 +172,16 @@ struct FinalArgs {
     int B, n_tiles, D;
 };
 
+#ifndef __CUDACC_RTC__
 // launchers (each returns the cudaGetLastError of its launch)
 cudaError_t launch_prep(const Program &prog, const PrepArgs &a, cudaStream_t st);
 // order[c * Bc + i] = index within chunk c of its i-th vector by (SIE mode, index); invalid vectors last
 cudaError_t launch_order(const float *derived, int D, int B, int Bc, int *order, cudaStream_t st);
 // allow_static: use the compile-time-specialised kernel when the list has one (trace.cu)
-cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nvec, bool allow_static, cudaStream_t st);
+struct JitTracer;
+// jit: the run-time compiled tracer of a list without a built-in signature (jit.cu) or NULL
+cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nvec, bool allow_static, const JitTracer *jit,
+                         cudaStream_t st);
 inline int trace_blocks_per_vector(const TraceArgs &a) { return (a.npix + a.pix_per_block - 1) / a.pix_per_block; }
 cudaError_t launch_refine(const Program &prog, const RefineArgs &a, int n_sm, cudaStream_t st);
 bool trace_has_static(const Program &prog);
@@ -199,5 +209,6 @@ cudaError_t run_fma_peak(int iters, double *tflops);
 // for the clients of the handle outside api.cu (nested.cu): error text on the handle, its device
 int handle_fail(::lensed_handle *h, int status, const char *fmt, ...);
 int handle_device(const ::lensed_handle *h);
+#endif  // !__CUDACC_RTC__
 
 }  // namespace lensed

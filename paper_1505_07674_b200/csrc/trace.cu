@@ -28,6 +28,8 @@
 // trace_kernel below, which interprets any list (a block-uniform switch per model).
 // launch_trace picks the static one when the list's signature matches.
 #include "trace_block.cuh"
+#include "jit.h"
+#include <stdlib.h>
 
 namespace lensed {
 
@@ -229,8 +231,17 @@ void count_kinds(const Program &prog, int (&counts)[K_COUNT])
 
 }  // namespace
 
+// LENSED_NO_BUILTIN=1 (tuning / tests): ignore the built-in signatures, so that a config's list goes
+// through the run-time specialisation (jit.cu) and the two can be compared
+static bool builtin_enabled()
+{
+    const char *env = getenv("LENSED_NO_BUILTIN");
+    return !(env && env[0] == '1');
+}
+
 bool trace_has_static(const Program &prog)
 {
+    if (!builtin_enabled()) return false;
     int counts[K_COUNT];
     count_kinds(prog, counts);
     for (StaticTracer f : kStaticTracers)
@@ -238,14 +249,17 @@ bool trace_has_static(const Program &prog)
     return false;
 }
 
-cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nvec, bool allow_static, cudaStream_t st)
+cudaError_t launch_trace(const Program &prog, const TraceArgs &a, int R, int nvec, bool allow_static, const JitTracer *jit,
+                         cudaStream_t st)
 {
     if (allow_static && a.err == nullptr) {
         int counts[K_COUNT];
         count_kinds(prog, counts);
         cudaError_t err = cudaSuccess;
-        for (StaticTracer f : kStaticTracers)
-            if (f(counts, prog, a, R, nvec, st, &err)) return err;
+        if (builtin_enabled())
+            for (StaticTracer f : kStaticTracers)
+                if (f(counts, prog, a, R, nvec, st, &err)) return err;
+        if (jit) return jit_launch(jit, prog, a, nvec, st);
     }
     const bool err = a.err != nullptr;
     switch (R) {

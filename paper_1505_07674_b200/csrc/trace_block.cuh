@@ -93,6 +93,7 @@ __device__ __forceinline__ void store_pixel(const TraceArgs &a, float *Lb, int r
     }
 }
 
+#ifndef __CUDACC_RTC__
 template <class Kernel>
 cudaError_t launch_trace_kernel(Kernel kernel, const Program &prog, const TraceArgs &a, int nvec, cudaStream_t st)
 {
@@ -105,5 +106,7 @@ cudaError_t launch_trace_kernel(Kernel kernel, const Program &prog, const TraceA
     kernel<<<grid, kTraceThreads, smem, st>>>(prog, a);
     return cudaGetLastError();
 }
+
+#endif  // !__CUDACC_RTC__
 
 }  // namespace lensed

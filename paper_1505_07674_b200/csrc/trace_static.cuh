@@ -44,11 +44,13 @@ struct TraceSig {
                                                    : 3 * NSG + (m < NSS + NSG + NFS ? 4 * (m - NSS - NSG)
                                                                                     : 4 * NFS + 3 * (m - NSS - NSG - NFS))));
     }
+#ifndef __CUDACC_RTC__
     static bool matches(const int (&c)[K_COUNT])
     {
         return c[K_SHEAR] == NSHEAR && c[K_SIE] == NSIE && c[K_SIS] == NSIS && c[K_POINT] == NPOINT &&
                c[K_SRC_SERSIC] == NSS && c[K_SRC_GAUSS] == NSG && c[K_FG_SERSIC] == NFS && c[K_FG_GAUSS] == NFG;
     }
+#endif
 };
 
 // ---- foreground expansion ------------------------------------------------------------------
@@ -552,6 +554,7 @@ __global__ void __launch_bounds__(kTraceThreads, MINB * (256 / kTraceThreads)) t
 #undef LENSED_TRACE_BODY
 }
 
+#ifndef __CUDACC_RTC__
 // Pixel pairs: NP = rule points per pass (TraceArgs::np_pp, from trace_pick_np), on the rule laid out
 // in passes (quad_pp, nq_pp).  Ray pairs (LENSED_PIXEL_PAIRS=0): R = 2 NP rays per register block.
 template <class S, int MINB>
@@ -593,5 +596,7 @@ cudaError_t launch_trace_static(const Program &prog, const TraceArgs &a0, int R,
         if (err) *err = launch_trace_static<S, MINB>(prog, a, R, nvec, st);                             \
         return true;                                                                                    \
     }
+
+#endif  // !__CUDACC_RTC__
 
 }  // namespace lensed

@@ -522,6 +522,54 @@ def test_shape_picked_at_create_and_shared_memory_limits(L):
         L.lensed_destroy(h)
 
 
+def test_a_list_without_a_built_in_signature_gets_its_tracer_compiled_at_create(L):
+    """SIE + shear + two Gaussian sources + Gaussian lens light + sky has none of the built-in
+    signatures: lensed_create specialises the tracer for it with NVRTC (csrc/jit.cu; the paper
+    compiles its kernel at run time too).  Same results as the oracle and as the
+    interpreting tracer within the tolerances; LENSED_JIT=0 keeps the interpreter."""
+    import os
+    models = ("sie", "shear", "src_gauss", "src_gauss", "fg_gauss", "sky")
+    truth = [0.02, -0.03, 0.5, 0.7, 35.0, 0.03, -0.02,
+             0.05, 0.08, 0.06, synth.mag_of_flux(30.0), 0.8, 20.0,
+             -0.1, 0.02, 0.04, synth.mag_of_flux(10.0), 0.6, 100.0,
+             0.0, 0.01, 0.3, synth.mag_of_flux(400.0), 0.7, 60.0,
+             0.01]
+    cfg = _mini(models, truth, H=45, W=52, psf=synth.gaussian_psf(7, 2.0), quad=synth.gauss_legendre_rule(3))
+    prob = Problem(cfg)
+    rng = np.random.default_rng(5)
+    params = np.vstack([cfg.truth] * 6).astype(np.float32)
+    params[1:] *= (1.0 + 0.05 * rng.standard_normal(params[1:].shape)).astype(np.float32)
+    params[:, 3] = np.clip(params[:, 3], 0.3, 1.0)
+    params[:, [11, 17, 23]] = np.clip(params[:, [11, 17, 23]], 0.2, 1.0)
+    logl_o, model_o = prob.oracle_loglike(params, want_model=True)
+    h = prob.create()
+    try:
+        kind = L.lensed_get_static_tracer(h)
+        assert kind == 2, L.lensed_last_error(h)
+        logl_j, model_j = _gpu_eval(L, h, params, cfg.H, cfg.W)
+        L.lensed_set_static_tracer(h, 0)
+        assert L.lensed_get_static_tracer(h) == 0
+        logl_i, model_i = _gpu_eval(L, h, params, cfg.H, cfg.W)
+        L.lensed_set_static_tracer(h, 1)
+        assert L.lensed_get_static_tracer(h) == 2
+    finally:
+        L.lensed_destroy(h)
+    for logl, model in ((logl_j, model_j), (logl_i, model_i)):
+        assert logl_errors(logl, logl_o).max() <= LOGL_RTOL
+        assert pixel_errors(model, model_o).max() <= PIXEL_RTOL
+    os.environ["LENSED_JIT"] = "0"
+    try:
+        h = prob.create()
+        try:
+            assert L.lensed_get_static_tracer(h) == 0
+            with pytest.raises(L.LensedError):
+                L.lensed_set_static_tracer(h, 1)
+        finally:
+            L.lensed_destroy(h)
+    finally:
+        del os.environ["LENSED_JIT"]
+
+
 def test_largest_rule_and_longest_model_list(L):
     """LENSED_MAX_QUAD-class rule (15 x 15 = 225 points, the size of the paper's g7k15) and a list
     of LENSED_MAX_MODELS = 32 objects (interpreting tracer, every kind present)."""
