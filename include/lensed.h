@@ -267,6 +267,10 @@ void lensed_debug_force_global_taps(int on);
  * at run time, 0 = interpreting; -1 for NULL.                                              */
 lensed_status lensed_set_static_tracer(lensed_handle *h, int on);
 int lensed_get_static_tracer(const lensed_handle *h);
+/* Test hook: only the compilation step of that run-time specialisation, for a model list (host
+ * array of lensed_kind) and an n_quad-point rule; needs NVRTC but no device.  Returns the size of
+ * the cubin in bytes, or -1 with the reason (the compiler's log) in log[log_len] (may be NULL).  */
+int lensed_debug_jit_compile(const int *models, int n_models, int n_quad, char *log, int log_len);
 
 /*
  * lensed_estimate_weights -- create-time variance estimation from the data (PAPER.md:190-212

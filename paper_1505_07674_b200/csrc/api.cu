@@ -996,6 +996,23 @@ lensed_status lensed_set_static_tracer(lensed_handle *h, int on)
     return LENSED_OK;
 }
 
+int lensed_debug_jit_compile(const int *models, int n_models, int n_quad, char *log, int log_len)
+{
+    int counts[K_COUNT] = {0};
+    if (!models || n_models < 1 || n_quad < 1) return -1;
+    for (int m = 0; m < n_models; ++m) {
+        if (models[m] < 0 || models[m] >= K_COUNT) return -1;
+        counts[models[m]] += 1;
+    }
+    int n_pos = 0;
+    for (int k = 0; k < K_SKY; ++k) n_pos += counts[k];
+    std::vector<char> cubin;
+    std::string name;
+    const std::string msg = jit_compile(counts, trace_pick_np(n_quad), n_pos <= 5 ? 3 : 2, &cubin, &name);
+    if (log && log_len > 0) snprintf(log, (size_t)log_len, "%s", msg.c_str());
+    return msg.empty() ? (int)cubin.size() : -1;
+}
+
 int lensed_get_static_tracer(const lensed_handle *h)
 {
     if (!h) return -1;

@@ -121,41 +121,23 @@ bool jit_wanted(const int (&c)[K_COUNT])
     return c[K_SHEAR] <= 1 && c[K_SIE] <= 3 && n_lens <= 6 && n_pos >= 0 && n_pos <= 8 && n_lens + n_pos >= 1;
 }
 
-// The tracer for these per-kind counts with np rule points per pass on the current device: from the
-// cache, else compiled now.  NULL (and a line in *why) when NVRTC or the driver entry points are
-// missing or the compilation fails.
-const JitTracer *jit_get(const int (&c)[K_COUNT], int np, int device, std::string *why)
+// NVRTC: the explicit instantiation of trace_static_kernel for these counts -> cubin and the
+// kernel's lowered name; returns an empty string, or what went wrong.  Needs no device.
+std::string jit_compile(const int (&c)[K_COUNT], int np, int minb, std::vector<char> *cubin, std::string *name)
 {
-    const int n_models = c[K_SHEAR] + c[K_SIE] + c[K_SIS] + c[K_POINT] + c[K_SRC_SERSIC] + c[K_SRC_GAUSS] + c[K_FG_SERSIC] + c[K_FG_GAUSS];
-    const int minb = n_models <= 5 ? 3 : 2;      // resident blocks per SM: 80 or 128 registers (as the built-in signatures)
-    char key[160], expr[256];
-    snprintf(key, sizeof key, "%d:%d,%d,%d,%d,%d,%d,%d,%d:%d:%d", device, c[K_SHEAR], c[K_SIE], c[K_SIS], c[K_POINT],
-             c[K_SRC_SERSIC], c[K_SRC_GAUSS], c[K_FG_SERSIC], c[K_FG_GAUSS], np, minb);
-    std::lock_guard<std::mutex> lock(g_mutex);
-    auto it = g_cache.find(key);
-    if (it != g_cache.end()) return it->second;
-    auto fail = [&](const std::string &msg) -> const JitTracer * {
-        if (why) *why = msg;
-        g_cache[key] = nullptr;                  // do not try again in this process
-        return nullptr;
-    };
     const Nvrtc &rt = nvrtc();
-    if (!rt.ok) return fail("NVRTC (libnvrtc.so.12) not found");
-    const Driver &drv = driver();
-    if (!drv.ok) return fail("driver entry points not available");
-
+    if (!rt.ok) return "NVRTC (libnvrtc.so.12) not found";
+    char expr[256];
     snprintf(expr, sizeof expr, "lensed::trace_static_kernel<%d, lensed::TraceSig<%d, %d, %d, %d, %d, %d, %d, %d>, %d>", np,
              c[K_SHEAR], c[K_SIE], c[K_SIS], c[K_POINT], c[K_SRC_SERSIC], c[K_SRC_GAUSS], c[K_FG_SERSIC], c[K_FG_GAUSS], minb);
     const std::string src = std::string("#include \"trace_static.cuh\"\ntemplate __global__ void ") + expr +
                             "(lensed::Program, lensed::TraceArgs);\n";
     void *prog = nullptr;
     if (rt.CreateProgram(&prog, src.c_str(), "lensed_jit.cu", kJitHeaderCount, kJitHeaderTexts, kJitHeaderNames) != 0)
-        return fail("nvrtcCreateProgram failed");
+        return "nvrtcCreateProgram failed";
     const char *opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", "-lineinfo"};
     std::string msg;
-    std::vector<char> cubin;
     const char *lowered = nullptr;
-    std::string name;
     if (rt.AddNameExpression(prog, expr) != 0) msg = "nvrtcAddNameExpression failed";
     else if (rt.CompileProgram(prog, 3, opts) != 0) {
         size_t n = 0;
@@ -167,13 +149,40 @@ const JitTracer *jit_get(const int (&c)[K_COUNT], int np, int device, std::strin
         size_t n = 0;
         if (rt.GetCUBINSize(prog, &n) != 0 || n == 0) msg = "no cubin";
         else {
-            cubin.resize(n);
-            if (rt.GetCUBIN(prog, cubin.data()) != 0) msg = "nvrtcGetCUBIN failed";
+            cubin->resize(n);
+            if (rt.GetCUBIN(prog, cubin->data()) != 0) msg = "nvrtcGetCUBIN failed";
             else if (rt.GetLoweredName(prog, expr, &lowered) != 0 || !lowered) msg = "nvrtcGetLoweredName failed";
-            else name = lowered;
+            else *name = lowered;
         }
     }
     rt.DestroyProgram(&prog);
+    return msg;
+}
+
+// The tracer for these per-kind counts with np rule points per pass on the current device: from the
+// cache, else compiled now.  NULL (and a line in *why) when NVRTC or the driver entry points are
+// missing or the compilation fails.
+const JitTracer *jit_get(const int (&c)[K_COUNT], int np, int device, std::string *why)
+{
+    const int n_models = c[K_SHEAR] + c[K_SIE] + c[K_SIS] + c[K_POINT] + c[K_SRC_SERSIC] + c[K_SRC_GAUSS] + c[K_FG_SERSIC] + c[K_FG_GAUSS];
+    const int minb = n_models <= 5 ? 3 : 2;      // resident blocks per SM: 80 or 128 registers (as the built-in signatures)
+    char key[160];
+    snprintf(key, sizeof key, "%d:%d,%d,%d,%d,%d,%d,%d,%d:%d:%d", device, c[K_SHEAR], c[K_SIE], c[K_SIS], c[K_POINT],
+             c[K_SRC_SERSIC], c[K_SRC_GAUSS], c[K_FG_SERSIC], c[K_FG_GAUSS], np, minb);
+    std::lock_guard<std::mutex> lock(g_mutex);
+    auto it = g_cache.find(key);
+    if (it != g_cache.end()) return it->second;
+    auto fail = [&](const std::string &msg) -> const JitTracer * {
+        if (why) *why = msg;
+        g_cache[key] = nullptr;                  // do not try again in this process
+        return nullptr;
+    };
+    const Driver &drv = driver();
+    if (!drv.ok) return fail("driver entry points not available");
+
+    std::vector<char> cubin;
+    std::string name;
+    const std::string msg = jit_compile(c, np, minb, &cubin, &name);
     if (!msg.empty()) return fail(msg);
 
     if (cudaSetDevice(device) != cudaSuccess || cudaFree(nullptr) != cudaSuccess) return fail("no current context");

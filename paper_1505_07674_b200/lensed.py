@@ -52,6 +52,7 @@ SYMBOLS = {
     "lensed_debug_force_global_taps": (None, [_i]),
     "lensed_set_static_tracer": (_i, [_p, _i]),
     "lensed_get_static_tracer": (_i, [_p]),
+    "lensed_debug_jit_compile": (_i, [_p, _i, _i, ctypes.c_char_p, _i]),
     "lensed_ns_run": (_i, [_p, _p, _p, _p, _i, _p, _p, _p, _p, _p, _ll, _p]),
     "lensed_ns_philox": (None, [_p, _p, _p]),
     "lensed_fma_peak": (_i, [_i, _i, _p]),
@@ -288,6 +289,14 @@ def lensed_set_static_tracer(h, on):
 
 def lensed_get_static_tracer(h):
     return lib().lensed_get_static_tracer(h)
+
+
+def lensed_debug_jit_compile(models, n_quad):
+    """-> (cubin bytes or -1, log): the NVRTC step of the run-time specialisation alone (no device needed)"""
+    m = _np(models, np.int32).reshape(-1)
+    log = ctypes.create_string_buffer(2048)
+    n = lib().lensed_debug_jit_compile(_hp(m), len(m), int(n_quad), log, len(log))
+    return n, log.value.decode(errors="replace")
 
 
 class NsOptions(ctypes.Structure):

@@ -132,3 +132,21 @@ def test_estimate_weights_rejects_bad_arguments(kwargs):
     with pytest.raises(lensed.LensedError) as e:
         lensed.lensed_estimate_weights(**args)
     assert e.value.status == lensed.EINVAL
+
+
+def test_the_embedded_tracer_sources_compile_for_a_new_signature_without_a_device():
+    """The run-time specialisation (csrc/jit.cu) hands NVRTC the tracer headers that build.py
+    embeds in the library: its compilation step needs no GPU, so the CPU suite checks that those
+    sources still build on their own (guards for host-only code, no missing header) for a list
+    with no built-in signature."""
+    import ctypes.util
+    from paper_1505_07674_b200 import lensed, synth
+    try:
+        ctypes.CDLL("libnvrtc.so.12")
+    except OSError:
+        pytest.skip("no libnvrtc on this machine")
+    models = synth.kind_ids(("sie", "point", "src_gauss", "src_sersic", "fg_gauss", "sky"))
+    n, log = lensed.lensed_debug_jit_compile(models, 9)
+    assert n > 50_000, log
+    n, log = lensed.lensed_debug_jit_compile([99], 9)
+    assert n == -1
