@@ -570,6 +570,58 @@ def test_a_list_without_a_built_in_signature_gets_its_tracer_compiled_at_create(
         del os.environ["LENSED_JIT"]
 
 
+_PARS = {"sis": lambda r: [r.uniform(-.1, .1), r.uniform(-.1, .1), r.uniform(.2, .5)],
+         "sie": lambda r: [r.uniform(-.1, .1), r.uniform(-.1, .1), r.uniform(.3, .6), r.uniform(.25, 1.), r.uniform(0, 180)],
+         "point": lambda r: [r.uniform(-.3, .3), r.uniform(-.3, .3), r.uniform(.02, .08)],
+         "shear": lambda r: [r.uniform(-.05, .05), r.uniform(-.05, .05)],
+         "src_sersic": lambda r: [r.uniform(-.1, .1), r.uniform(-.1, .1), r.uniform(.05, .2), synth.mag_of_flux(r.uniform(10, 40)),
+                                  r.uniform(.5, 4.), r.uniform(.4, 1.), r.uniform(0, 180)],
+         "fg_sersic": lambda r: [r.uniform(-.1, .1), r.uniform(-.1, .1), r.uniform(.2, .5), synth.mag_of_flux(r.uniform(200, 800)),
+                                 r.uniform(1., 4.), r.uniform(.5, 1.), r.uniform(0, 180)],
+         "src_gauss": lambda r: [r.uniform(-.1, .1), r.uniform(-.1, .1), r.uniform(.04, .1), synth.mag_of_flux(r.uniform(10, 40)),
+                                 r.uniform(.4, 1.), r.uniform(0, 180)],
+         "fg_gauss": lambda r: [r.uniform(-.1, .1), r.uniform(-.1, .1), r.uniform(.2, .4), synth.mag_of_flux(r.uniform(100, 300)),
+                                r.uniform(.5, 1.), r.uniform(0, 180)],
+         "sky": lambda r: [r.uniform(0, .02)]}
+
+
+@pytest.mark.parametrize("seed,models,n_rule", [
+    (1, ("fg_sersic", "fg_gauss", "sky"), 2),                                  # no lens, no source: foreground only
+    (2, ("sis", "point", "src_sersic", "src_gauss"), 3),                       # circular lenses only, two kinds of source
+    (3, ("sie", "sis", "shear", "src_sersic", "fg_gauss", "sky"), 2),          # one SIE but not "direct" (a SIS beside it)
+    (4, ("sie", "sie", "sie", "src_gauss", "sky"), 3),                         # three SIEs, their modes mixed
+    (5, ("point", "shear", "src_gauss", "src_gauss", "src_gauss", "fg_sersic", "fg_sersic"), 5),
+    (6, ("sie", "src_sersic", "src_sersic", "src_sersic", "fg_sersic", "fg_gauss", "fg_gauss", "sky", "sky"), 4),
+    (7, ("shear", "src_gauss"), 7),                                            # 49-point rule: 5 points per pass, one dummy
+])
+def test_run_time_specialised_tracers_of_assorted_lists_against_the_oracle(L, seed, models, n_rule):
+    """The specialised tracer is one template over the per-kind counts; the built-in signatures
+    exercise nine points of that space.  Here NVRTC instantiates it for lists that take its other
+    paths (no lens / no source / several SIEs / SIE + SIS without direct frames / foreground
+    Gaussians first / 4-, 9-, 16-, 25- and 49-point rules) and each is compared with the oracle and
+    with the interpreting tracer on drawn vectors, masked image, odd number of traced pixels."""
+    rng = np.random.default_rng(100 + seed)
+    draw = lambda: np.concatenate([_PARS[m](rng) for m in models])
+    truth = draw()
+    H, W = 33, 29
+    mask = synth.annulus_mask(H, W, 2.0, 13.5)
+    cfg = _mini(models, list(truth), H=H, W=W, psf=synth.gaussian_psf(5, 1.8), mask=mask, quad=synth.gauss_legendre_rule(n_rule))
+    prob = Problem(cfg)
+    params = np.vstack([truth] + [draw() for _ in range(5)]).astype(np.float32)
+    logl_o, model_o = prob.oracle_loglike(params, want_model=True)
+    h = prob.create()
+    try:
+        assert L.lensed_get_static_tracer(h) == 2, L.lensed_last_error(h)
+        got = [_gpu_eval(L, h, params, H, W)]
+        L.lensed_set_static_tracer(h, 0)
+        got.append(_gpu_eval(L, h, params, H, W))
+    finally:
+        L.lensed_destroy(h)
+    for logl, model in got:
+        assert logl_errors(logl, logl_o).max() <= LOGL_RTOL
+        assert pixel_errors(model, model_o).max() <= PIXEL_RTOL
+
+
 def test_largest_rule_and_longest_model_list(L):
     """LENSED_MAX_QUAD-class rule (15 x 15 = 225 points, the size of the paper's g7k15) and a list
     of LENSED_MAX_MODELS = 32 objects (interpreting tracer, every kind present)."""
