@@ -56,7 +56,9 @@ __device__ double sersic_bn(double n)
         const double lden = a * t - b - (lgam_a1 - log(a));
         const double dt = (lp + kLn2) * exp(lp - lden);
         t -= dt;
-        if (fabs(dt) < 1e-15 * fmax(1.0, fabs(t))) break;
+        // quadratic convergence: a step below 1e-9 leaves an error below 1e-17, so the check that
+        // would only confirm it (one more evaluation of the series) is not made
+        if (fabs(dt) < 1e-9 * fmax(1.0, fabs(t))) break;
     }
     return exp(t);
 }
