@@ -347,16 +347,24 @@ int default_shape(const lensed_handle *h)
     return px[2] * 100 <= px[block] * 85 ? 2 : block;
 }
 
-// Pixels of the traced list one tracer block walks: it amortises its prologue (constants +
-// frame tables) over them.  Measured per config (ms per step at 512 / 1024 / 2048 / 4096 / 8192
-// pixels): HST 0.296 / 0.273 / 0.264 / 0.269 / 0.288, SLACS 4.55 / 4.34 / 4.23 / 4.15 / 4.13,
-// Euclid - / 34.6 / 34.0 / 33.6 / 33.5 per 4096 vectors.  At most 8192 (TraceArgs::fixmask).
+// Pixels of the traced list one tracer block walks: it amortises its prologue (constants, frame
+// tables, rule moments, four barriers) over them, so few large blocks of EQUAL size -- the list is
+// split into ceil(npix / kPpbMax) blocks and the block size rounded up to whole passes of 256
+// threads.  Round 2, pixel-pair tracers, ms per step at fixed 1024 / 2048 / 4096 / 5120 / 8192:
+// HST (10 000 pixels) 0.241 / 0.221 / 0.224 / 0.213 / 0.245 (5120 = two equal blocks), mock (14 400)
+// 4.72 / 4.53 / 4.43 / 4.40 / 4.43, SLACS (21 160) 3.75 / - / 3.48 / 3.47 / 3.44.  At most 8192
+// (32 flag bits per thread, TraceArgs::fixmask).
+#ifndef LENSED_PPB_MAX
+#define LENSED_PPB_MAX 8192
+#endif
 int pix_per_block(int npix)
 {
 #ifdef LENSED_PIX_PER_BLOCK             // tuning builds (build.py defines=...)
     return LENSED_PIX_PER_BLOCK;
 #else
-    return npix >= (1 << 16) ? 8192 : npix >= (1 << 14) ? 4096 : npix >= (1 << 11) ? 2048 : 256;
+    if (npix <= 256) return 256;
+    const int n_blocks = (npix + LENSED_PPB_MAX - 1) / LENSED_PPB_MAX;
+    return ((npix + n_blocks - 1) / n_blocks + 255) / 256 * 256;
 #endif
 }
 
