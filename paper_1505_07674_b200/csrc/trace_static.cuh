@@ -494,42 +494,49 @@ __global__ void __launch_bounds__(kTraceThreads, MINB * (256 / kTraceThreads)) t
         if (a.fixmask) a.fixmask[((size_t)vec * gridDim.x + blockIdx.x) * kTraceThreads + threadIdx.x] = 0;
         return;
     }
-    if constexpr (S::direct) {
-        // source tables lose M Gamma (rule offset); B per source (TraceSig "direct frames")
+    if constexpr (S::direct || S::n_fs > 0) {
         const int nq = a.nq_pad;
-        float *stab = const_cast<float *>(tb.stab);
-        float *gtab = stab + (size_t)(2 * (1 + S::n_lens)) * nq;
-        if (S::n_shear) {
-            for (int i = threadIdx.x; i < S::n_src * nq; i += kTraceThreads) {
-                const int m = i / nq, k = i - m * nq;
-                const float4 M = tb.sder[S::light_off4(m) + 1];
-                const float su = stab[2 * nq + k], sv = stab[3 * nq + k];     // shear = lens 0
-                gtab[(size_t)(2 * m) * nq + k] -= fmaf(M.x, su, M.y * sv);
-                gtab[(size_t)(2 * m + 1) * nq + k] -= fmaf(M.z, su, M.w * sv);
+        if constexpr (S::n_fs > 0) {
+            // rule moments in the frame of every foreground Sersic ("foreground expansion"), from the
+            // table the per-ray path reads (padding entries have zero weight): one warp per component,
+            // the rule points across its lanes, a fixed shuffle tree
+            const int lane = threadIdx.x & 31;
+            for (int i = threadIdx.x >> 5; i < S::n_fs; i += kTraceThreads / 32) {
+                const int m = S::n_ss + S::n_sg + i;
+                const float *tu = tb.stab + (size_t)(2 * (1 + S::n_lens + m)) * nq, *tv = tu + nq;
+                float v[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+                for (int k = lane; k < nq; k += 32) {
+                    const float w = tb.sw[k], d1 = tu[k], d2 = tv[k], w11 = w * d1 * d1, w12 = w * d1 * d2, w22 = w * d2 * d2;
+                    v[0] += w11; v[1] += w12; v[2] += w22;
+                    v[3] += w11 * d1 * d1; v[4] += w11 * d1 * d2; v[5] += w11 * d2 * d2; v[6] += w12 * d2 * d2; v[7] += w22 * d2 * d2;
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) v[e] += __shfl_xor_sync(0xffffffffu, v[e], o);
+                if (lane == 0) tb.sfgx[i] = FgMoments{v[0], v[1], v[2], v[3], v[4], v[5], v[6], v[7]};
             }
         }
-        if (threadIdx.x < S::n_src) {
-            const float4 M = tb.sder[S::light_off4(threadIdx.x) + 1];
-            const float4 c2 = tb.sder[S::lens_off4(S::n_shear) + 2];  // (cs A, sn A, cs A l, -sn A l)
-            tb.smat[threadIdx.x] = make_float4(fmaf(M.x, c2.x, M.y * c2.y), fmaf(M.x, c2.w, M.y * c2.z),
-                                               fmaf(M.z, c2.x, M.w * c2.y), fmaf(M.z, c2.w, M.w * c2.z));
-        }
-        __syncthreads();
-    }
-    if constexpr (S::n_fs > 0) {
-        // rule moments in the frame of every foreground Sersic ("foreground expansion"), from the
-        // table the per-ray path reads (padding entries have zero weight)
-        if (threadIdx.x < S::n_fs) {
-            const int nq = a.nq_pad;
-            const int m = S::n_ss + S::n_sg + threadIdx.x;
-            const float *tu = tb.stab + (size_t)(2 * (1 + S::n_lens + m)) * nq, *tv = tu + nq;
-            FgMoments mo{0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-            for (int k = 0; k < nq; ++k) {
-                const float w = tb.sw[k], d1 = tu[k], d2 = tv[k], w11 = w * d1 * d1, w12 = w * d1 * d2, w22 = w * d2 * d2;
-                mo.S11 += w11; mo.S12 += w12; mo.S22 += w22;
-                mo.T0 += w11 * d1 * d1; mo.T1 += w11 * d1 * d2; mo.T2 += w11 * d2 * d2; mo.T3 += w12 * d2 * d2; mo.T4 += w22 * d2 * d2;
+        if constexpr (S::direct) {
+            // source tables lose M Gamma (rule offset); B per source (TraceSig "direct frames").  The
+            // moments above read foreground tables only, so both share one barrier.
+            float *stab = const_cast<float *>(tb.stab);
+            float *gtab = stab + (size_t)(2 * (1 + S::n_lens)) * nq;
+            if (S::n_shear) {
+                for (int i = threadIdx.x; i < S::n_src * nq; i += kTraceThreads) {
+                    const int m = i / nq, k = i - m * nq;
+                    const float4 M = tb.sder[S::light_off4(m) + 1];
+                    const float su = stab[2 * nq + k], sv = stab[3 * nq + k];     // shear = lens 0
+                    gtab[(size_t)(2 * m) * nq + k] -= fmaf(M.x, su, M.y * sv);
+                    gtab[(size_t)(2 * m + 1) * nq + k] -= fmaf(M.z, su, M.w * sv);
+                }
             }
-            tb.sfgx[threadIdx.x] = mo;
+            if (threadIdx.x < S::n_src) {
+                const float4 M = tb.sder[S::light_off4(threadIdx.x) + 1];
+                const float4 c2 = tb.sder[S::lens_off4(S::n_shear) + 2];          // (cs A, sn A, cs A l, -sn A l)
+                tb.smat[threadIdx.x] = make_float4(fmaf(M.x, c2.x, M.y * c2.y), fmaf(M.x, c2.w, M.y * c2.z),
+                                                   fmaf(M.z, c2.x, M.w * c2.y), fmaf(M.z, c2.w, M.w * c2.z));
+            }
         }
         __syncthreads();
     }
