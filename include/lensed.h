@@ -232,8 +232,9 @@ long long lensed_frame_bytes(const lensed_handle *h);
  *               (PSFs up to about 37 rows)
  *   1 "wide"    256 threads on 64 x 128 output tiles, one block per SM: any PSF
  *   0 "narrow"  128 threads on 64 x 64 tiles, two blocks per SM: small or masked images
- * lensed_create picks one (wide for full images; narrow or strip where a mask or a small image
- * makes their tile list compute at least 15 % fewer pixels); lensed_set_conv_shape(h, shape) forces one (it
+ * lensed_create picks one (strip for PSFs up to 21 x 21, where its stages are double buffered, and
+ * where a mask makes its strip list compute at least 15 % fewer pixels; else wide, or narrow on
+ * the same 15 % rule); lensed_set_conv_shape(h, shape) forces one (it
  * rebuilds the tile lists and the frame layout and synchronises the device; EINVAL for another
  * value, LENSED_EUNSUPPORTED if the PSF is too large for that shape's shared memory).
  * lensed_get_conv_shape: 2 / 1 / 0, -1 for NULL.  Rendered pixels do not depend on the shape at

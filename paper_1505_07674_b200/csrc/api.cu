@@ -320,12 +320,11 @@ lensed_status build_tiles(lensed_handle *h, int shape)
 }
 
 // Shape lensed_create picks, from the pixels each shape's tile list computes (tiles x tile area)
-// and what was measured on the configs (profiles/r2b.md).  With full tiles the wide shape
-// is the fastest (31 x 31 PSF, 4096 Euclid vectors: wide 32.5, narrow 35.0, strip 35.3 ms: the
-// strip shape's unsynchronised warps miss the constant cache on the taps more often than a
-// block's lock-step warps).  A masked or small image goes to the shape that computes at least
-// 15 % fewer pixels: narrow's 64-column tiles, or the 16 x 64 strips (SLACS annulus: 25 strips =
-// 25.6 k pixels against 8 narrow tiles = 32.8 k; 1.72 against 2.10 ms per 4096 vectors).
+// and what was measured on the configs (profiles/r2b.md).  Large PSFs on full tiles: wide (31 x 31
+// PSF, 4096 Euclid vectors: wide 32.4, narrow 34.7, strip 34.6 ms -- the strip shape has one stage
+// per warp there and its unsynchronised warps miss the constant cache on the taps more often than
+// a block's lock-step warps).  Masked images: the shape that computes at least 15 % fewer pixels
+// (SLACS annulus: 23 strips = 23.6 k pixels against 8 narrow tiles = 32.8 k; 1.49 against 2.10 ms).
 int default_shape(const lensed_handle *h)
 {
 #ifdef LENSED_CONV_FORCE_SHAPE
@@ -344,7 +343,11 @@ int default_shape(const lensed_handle *h)
         px[shape] = conv_shape_fits(h->KH, h->NC, shape) ? (long long)tiles.size() * tw * th : (1LL << 60);
     }
     const int block = px[0] * 100 <= px[1] * 85 ? 0 : 1;
-    return px[2] * 100 <= px[block] * 85 ? 2 : block;
+    if (!conv_shape_fits(h->KH, h->NC, 2)) return block;
+    // strips: where their stages are double buffered (PSFs up to 21 x 21) they are as fast as the wide
+    // tiles on full images and faster on small ones (HST 0.069 against 0.076 ms); with one stage per
+    // warp (larger PSFs) only where they compute at least 15 % fewer pixels
+    return conv_num_stages(h->KH, h->NC, false, 2) == 2 || px[2] * 100 <= px[block] * 85 ? 2 : block;
 }
 
 // Pixels of the traced list one tracer block walks: it amortises its prologue (constants, frame

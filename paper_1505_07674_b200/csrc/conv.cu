@@ -407,12 +407,13 @@ __global__ void __maxnreg__(176) conv_kernel(const __grid_constant__ ConvArgs a,
 // Eight ONE-WARP blocks per SM and no block-level step at all: a work item is (16 x 64 output
 // strip, parameter vector), items are ordered strip-major and split evenly over all warps of the
 // grid, and a warp owns its input stage(s) in shared memory, its mbarrier(s) and its TMA copies
-// (lane 0 issues; box = (16 + KH - 1) rows x (64 + 4 NC) floats).  One warp per block: all loop
-// indices derive from blockIdx, and the kernel is declared __launch_bounds__(32) WITHOUT a
-// minimum block count -- with (32, 8) ptxas keeps the tap pairs in vector registers (LDC + MOV
-// instead of LDCU + UR operands: 327 instead of 305 instructions per loop body, 25 % slower);
-// eight blocks per SM are resident because 8 x (registers, shared memory) fit.
-// What the block shapes above
+// (lane 0 issues; box = (16 + KH - 1) rows x (64 + 4 NC) floats).  One warp per block; eight blocks
+// per SM are resident because 8 x (registers, shared memory) fit.  The register cap is part of the
+// code generation (cuobjdump, profiles/r2b.md): capped at 224 ptxas keeps the tap pairs on the
+// uniform datapath (LDCU + UR operands, 305 instructions per loop body); with 255, or with a
+// minimum block count in __launch_bounds__, it moves them to vector registers (LDC + 24-28 MOV,
+// 327 instructions, 14 % slower).
+// // What the block shapes above
 // lose at their barriers -- the tile prologue (wait for the copy), the epilogue (chi-square
 // reduction) and the ramps of the chunk loops, during which a block's warps all leave the FMA pipe
 // together -- a warp here loses alone, while the other warp of its scheduler keeps the pipe busy.
@@ -421,13 +422,13 @@ __global__ void __maxnreg__(176) conv_kernel(const __grid_constant__ ConvArgs a,
 // coordinates for this shape): SLACS annulus, 68 % of the computed pixels are counted instead of 49 %.  The per-thread arithmetic (thread tile 4 x 8, tap pairs,
 // rotating rows, blocked summation) is the code of the block shapes, so the results agree with
 // theirs bit for bit per pixel; the chi-square partials are per strip.
-// Data d and weights w of the strip are read from global memory in the epilogue (L2 hits: the
-// same strip is reused for many vectors); stages are double buffered when 16 of them fit.
+// Data d and weights w of a strip are loaded once per strip and stay in registers for all its
+// vectors (64 of the 255 a one-warp block may use); stages are double buffered when 16 of them fit.
 constexpr int kSH = 16, kSW = 64;      // strip: the 4 x 8 lanes of a warp on 4 x 8 thread tiles
 constexpr int kStripWarps = 8;
 
 template <bool RENDER, bool GT>
-__global__ void __launch_bounds__(32) conv_strip_kernel(const __grid_constant__ ConvArgs a,
+__global__ void __maxnreg__(224) conv_strip_kernel(const __grid_constant__ ConvArgs a,
                                                                          const __grid_constant__ CUtensorMap tmap)
 {
     constexpr int NTX = 8, kGroup = 32;
@@ -463,6 +464,7 @@ __global__ void __launch_bounds__(32) conv_strip_kernel(const __grid_constant__ 
     issue(lo, 0);
     int cur_t = -1;
     bool warp_any = true;
+    float wreg[kTR][8], dreg[kTR][8];          // weights and data of the current strip (loglike)
     const int NC4 = 4 * a.NC;
     const int n4 = (a.KH + 1) >> 2;
     const bool tail2 = ((a.KH + 1) & 2) != 0;
@@ -477,8 +479,8 @@ __global__ void __launch_bounds__(32) conv_strip_kernel(const __grid_constant__ 
         if (a.n_stages == 2 && more) issue(item + 1, s ^ 1);      // its last readers passed the __syncwarp below
 
         if (!RENDER && t != cur_t) {
-            // warps whose strip is fully masked never get here (api.cu lists strips with a counted
-            // pixel); the test stays for the strips of a render-sized list used by loglike
+            // data and weights of the strip stay in REGISTERS for all its vectors (a one-warp block
+            // may use 255 of them): loaded once per strip, no epilogue latency.  w = 0 outside the image.
             cur_t = t;
             bool any = false;
 #pragma unroll
@@ -486,8 +488,10 @@ __global__ void __launch_bounds__(32) conv_strip_kernel(const __grid_constant__ 
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
                     const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
-                    const float wv = (y < a.H && x < a.W) ? __ldg(a.wmask + (size_t)y * a.W + x) : 0.0f;
-                    any = any | (wv != 0.0f);
+                    const bool in = y < a.H && x < a.W;
+                    wreg[o][e] = in ? __ldg(a.wmask + (size_t)y * a.W + x) : 0.0f;
+                    dreg[o][e] = in ? __ldg(a.image + (size_t)y * a.W + x) : 0.0f;
+                    any = any | (wreg[o][e] != 0.0f);
                 }
             warp_any = __any_sync(0xffffffffu, any);
         }
@@ -535,22 +539,13 @@ __global__ void __launch_bounds__(32) conv_strip_kernel(const __grid_constant__ 
             float part = 0.0f;
             if (warp_any) {
 #pragma unroll
-                for (int o = 0; o < kTR; ++o) {
-                    float wv[8], dv[8];
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
-                        const bool in = y < a.H && x < a.W;
-                        wv[e] = in ? __ldg(a.wmask + (size_t)y * a.W + x) : 0.0f;
-                        dv[e] = in ? __ldg(a.image + (size_t)y * a.W + x) : 0.0f;
-                    }
+                for (int o = 0; o < kTR; ++o)
 #pragma unroll
                     for (int e = 0; e < 8; ++e)
-                        if (wv[e] != 0.0f) {               // masked pixels may see untraced L: never touch them
-                            const float diff = dv[e] - out[o][e];
-                            part = fmaf(wv[e] * diff, diff, part);
+                        if (wreg[o][e] != 0.0f) {          // masked pixels may see untraced L: never touch them
+                            const float diff = dreg[o][e] - out[o][e];
+                            part = fmaf(wreg[o][e] * diff, diff, part);
                         }
-                }
             }
             double sum = (double)part;
 #pragma unroll

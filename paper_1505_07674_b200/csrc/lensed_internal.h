@@ -204,6 +204,7 @@ size_t trace_smem_bytes(const Program &prog, int nq_pad);
 void conv_tile_shape(int shape, int *tile_w, int *tile_h);
 size_t conv_smem_bytes(int KH, int NC, bool render, int shape);
 bool conv_shape_fits(int KH, int NC, int shape);
+int conv_num_stages(int KH, int NC, bool render, int shape);   // input-tile buffers per block (2 = double buffered)
 cudaError_t run_fma_peak(int iters, double *tflops);
 
 // for the clients of the handle outside api.cu (nested.cu): error text on the handle, its device
