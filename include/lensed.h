@@ -323,7 +323,11 @@ lensed_status lensed_render_error(lensed_handle *h, const float *params_dev, int
  *                       through lensed_image_plane_prior before its likelihood
  *   opt                 n_live in [free parameters + 1, 4096]; batch >= 1; tol: stop when
  *                       max live L * X < tol * Z; enlarge >= 1: linear enlargement of the ellipsoid
- *                       that bounds the live points; seed of the counter-based generator
+ *                       that bounds the live points; seed of the counter-based generator;
+ *                       tied_to [P] HOST or NULL: parameter p with tied_to[p] = q >= 0 is not drawn but takes
+ *                       the value drawn for parameter q ("the centre of the mass distribution
+ *                       [forced] to coincide with the centre of the surface brightness distribution"); it
+ *                       needs lo[p] == hi[p], q untied and q != p (EINVAL otherwise); -1 = not tied
  *   res                 HOST, receives ln Z, its error sqrt(H/n_live), the information H, counts
  *   samples_dev [capacity][P], logl_dev [capacity], logw_dev [capacity]: device f32 or NULL with
  *                       capacity 0: the dead points in order of death, then the live points; logw =
@@ -336,6 +340,7 @@ typedef struct {
     int n_live, batch, max_rounds;
     double tol, enlarge;
     unsigned long long seed;
+    const int *tied_to;       /* HOST [P] or NULL: see above */
 } lensed_ns_options;
 typedef struct {
     double ln_z, ln_z_err, information;

@@ -51,6 +51,7 @@ struct NsState {
 struct NsProblem {
     const double *lo, *hi;           // [P] device
     const int *free_idx;             // [d] device: parameter index of each free dimension
+    const int *tied_to;              // [P] device: parameter p takes the drawn value of parameter tied_to[p] (-1: its own)
     int P, d, N, K;
     double enlarge, ln_tol;
     unsigned long long seed;
@@ -88,7 +89,8 @@ __device__ inline void normals4(unsigned long long seed, uint32_t stream, uint32
     z[0] = r0 * c0; z[1] = r0 * s0; z[2] = r1 * c1; z[3] = r1 * s1;
 }
 
-// theta = lo + u (hi - lo) on the free dimensions, lo on the fixed ones, rounded to float
+// theta = lo + u (hi - lo) on the free dimensions, lo on the fixed ones, rounded to float; tied
+// parameters then copy the parameter they follow (mass centre = light centre)
 __device__ inline void write_theta(const NsProblem &pb, const double *u, float *theta)
 {
     for (int p = 0; p < pb.P; ++p) theta[p] = (float)pb.lo[p];
@@ -96,6 +98,8 @@ __device__ inline void write_theta(const NsProblem &pb, const double *u, float *
         const int p = pb.free_idx[k];
         theta[p] = (float)(pb.lo[p] + u[k] * (pb.hi[p] - pb.lo[p]));
     }
+    for (int p = 0; p < pb.P; ++p)
+        if (pb.tied_to[p] >= 0) theta[p] = theta[pb.tied_to[p]];
 }
 
 __global__ void ns_init_kernel(NsProblem pb, double *U, float *theta, NsState *st)
@@ -526,6 +530,16 @@ extern "C" lensed_status lensed_ns_run(lensed_handle *h, const float *prior_lo, 
             return (lensed_status)handle_fail(h, LENSED_EINVAL, "lensed_ns_run: prior of parameter %d is [%g, %g]", p, lo[p], hi[p]);
         if (hi[p] > lo[p]) free_idx.push_back(p);
     }
+    std::vector<int> tied(P, -1);
+    if (opt->tied_to) {
+        for (int p = 0; p < P; ++p) {
+            const int q = opt->tied_to[p];
+            if (q < 0) continue;
+            if (q >= P || q == p || opt->tied_to[q] >= 0 || hi[p] > lo[p])
+                return (lensed_status)handle_fail(h, LENSED_EINVAL, "lensed_ns_run: tied_to[%d] = %d (needs another, untied parameter, and lo == hi for the tied one)", p, q);
+            tied[p] = q;
+        }
+    }
     const int d = (int)free_idx.size();
     if (d < 1) return (lensed_status)handle_fail(h, LENSED_EINVAL, "lensed_ns_run: no free parameter (every prior has lo == hi)");
     if (d > kMaxFree) return (lensed_status)handle_fail(h, LENSED_EUNSUPPORTED, "lensed_ns_run: %d free parameters > %d", d, kMaxFree);
@@ -551,11 +565,11 @@ extern "C" lensed_status lensed_ns_run(lensed_handle *h, const float *prior_lo, 
     NS_CU(cudaSetDevice(handle_device(h)));
     Buffers buf;
     double *d_lo, *d_hi, *d_U, *d_Uc, *d_m, *d_G, *d_s;
-    int *d_free, *d_death;
+    int *d_free, *d_death, *d_tied;
     float *d_death_l;
     float *d_theta, *d_theta_c, *d_logl, *d_logl_c;
     NsState *d_state;
-    NS_CU(buf.get(&d_lo, P)); NS_CU(buf.get(&d_hi, P)); NS_CU(buf.get(&d_free, d));
+    NS_CU(buf.get(&d_lo, P)); NS_CU(buf.get(&d_hi, P)); NS_CU(buf.get(&d_free, d)); NS_CU(buf.get(&d_tied, P));
     NS_CU(buf.get(&d_U, (size_t)N * d)); NS_CU(buf.get(&d_Uc, (size_t)K * d));
     NS_CU(buf.get(&d_m, d)); NS_CU(buf.get(&d_G, (size_t)d * d)); NS_CU(buf.get(&d_s, 1));
     NS_CU(buf.get(&d_theta, (size_t)N * P)); NS_CU(buf.get(&d_theta_c, (size_t)K * P));
@@ -563,9 +577,10 @@ extern "C" lensed_status lensed_ns_run(lensed_handle *h, const float *prior_lo, 
     NS_CU(cudaMemcpyAsync(d_lo, lo.data(), P * sizeof(double), cudaMemcpyHostToDevice, st));
     NS_CU(cudaMemcpyAsync(d_hi, hi.data(), P * sizeof(double), cudaMemcpyHostToDevice, st));
     NS_CU(cudaMemcpyAsync(d_free, free_idx.data(), d * sizeof(int), cudaMemcpyHostToDevice, st));
+    NS_CU(cudaMemcpyAsync(d_tied, tied.data(), P * sizeof(int), cudaMemcpyHostToDevice, st));
     NS_CU(cudaStreamSynchronize(st));                       // the host vectors above go out of scope otherwise
 
-    const NsProblem pb{d_lo, d_hi, d_free, P, d, N, K, opt->enlarge, log(opt->tol), opt->seed};
+    const NsProblem pb{d_lo, d_hi, d_free, d_tied, P, d, N, K, opt->enlarge, log(opt->tol), opt->seed};
     const NsOut out{samples_dev, logl_dev, logw_dev, capacity};
 
     // step 0: the live points from the prior

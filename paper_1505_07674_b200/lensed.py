@@ -301,7 +301,7 @@ def lensed_debug_jit_compile(models, n_quad):
 
 class NsOptions(ctypes.Structure):
     _fields_ = [("n_live", _i), ("batch", _i), ("max_rounds", _i), ("tol", _d), ("enlarge", _d),
-                ("seed", ctypes.c_ulonglong)]
+                ("seed", ctypes.c_ulonglong), ("tied_to", _p)]
 
 
 class NsResult(ctypes.Structure):
@@ -310,7 +310,7 @@ class NsResult(ctypes.Structure):
 
 
 def lensed_ns_run(h, prior_lo, prior_hi, n_live=400, batch=256, tol=1e-3, enlarge=1.2, seed=1, max_rounds=100000,
-                  image_plane_sources=None, samples_dev=None, logl_dev=None, logw_dev=None, stream=None):
+                  image_plane_sources=None, tied_to=None, samples_dev=None, logl_dev=None, logw_dev=None, stream=None):
     """-> dict of the lensed_ns_result fields.  prior_lo / prior_hi: host arrays [P]; the three
     output tensors (float32 CUDA, [cap][P], [cap], [cap]) are optional."""
     lo, hi = _np(prior_lo, np.float32), _np(prior_hi, np.float32)
@@ -324,7 +324,10 @@ def lensed_ns_run(h, prior_lo, prior_hi, n_live=400, batch=256, tol=1e-3, enlarg
         _check_out(samples_dev, cap, cap * P)
         _check_out(logl_dev, cap, cap)
         _check_out(logw_dev, cap, cap)
-    opt = NsOptions(int(n_live), int(batch), int(max_rounds), float(tol), float(enlarge), int(seed))
+    tied = None if tied_to is None else _np(tied_to, np.int32).reshape(-1)
+    if tied is not None and tied.shape != (P,):
+        raise LensedError(EINVAL, "tied_to must be [%d]" % P)
+    opt = NsOptions(int(n_live), int(batch), int(max_rounds), float(tol), float(enlarge), int(seed), _hp(tied))
     res = NsResult()
     ptr = lambda t: None if t is None else ctypes.c_void_p(t.data_ptr())
     _check(lib().lensed_ns_run(h, _hp(lo), _hp(hi), _hp(ip), 0 if ip is None else len(ip), ctypes.byref(opt),

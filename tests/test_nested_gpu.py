@@ -177,6 +177,42 @@ def test_shrunk_hst_case_with_an_image_plane_prior(L):
     assert abs(mg[7] - t[7]) < 5 * sr[7] + 0.01 and abs(mg[8] - t[8]) < 5 * sr[8] + 0.01
 
 
+def test_tied_parameters_follow_the_parameter_they_are_tied_to(L):
+    """the mass centre forced onto the centre of the light.  tied_to makes a parameter
+    take the drawn value of another; the oracle driver does the same through its transform hook.
+    tiny config: the source position (x, y) tied to the lens position, which is free."""
+    cfg = synth.get_config(0)
+    prob = Problem(cfg)
+    lo, hi = _tiny_priors(cfg)
+    lo[3:5] = hi[3:5] = 0.0                      # source (x, y): not drawn
+    tied = -np.ones(len(lo), dtype=np.int32)
+    tied[3], tied[4] = 0, 1
+
+    def transform(theta):
+        out = theta.copy()
+        out[:, 3], out[:, 4] = out[:, 0], out[:, 1]
+        return out
+
+    kw = dict(n_live=48, batch=64, tol=1e-12, enlarge=1.3, seed=3, max_rounds=4)
+    ref = ns.run(lambda t: prob.oracle_loglike(t.astype(np.float32), want_model=False), lo, hi, transform=transform, **kw)
+    got = _gpu_run(L, prob, lo, hi, 4096, tied_to=tied, **kw)
+    nd = ref["n_dead"]
+    assert got["n_dead"] == nd and nd > 0
+    assert np.array_equal(got["samples"][:nd], ref["samples"][:nd].astype(np.float32))
+    assert np.array_equal(got["samples"][:, 3], got["samples"][:, 0]) and np.array_equal(got["samples"][:, 4], got["samples"][:, 1])
+    h = prob.create()
+    try:
+        bad = tied.copy(); bad[0] = 3            # a chain: 3 -> 0 -> 3
+        with pytest.raises(L.LensedError) as e:
+            L.lensed_ns_run(h, lo, hi, tied_to=bad, **kw)
+        assert e.value.status == L.EINVAL
+        lo2, hi2 = lo.copy(), hi.copy(); hi2[3] = 0.1     # a tied parameter with a free prior
+        with pytest.raises(L.LensedError):
+            L.lensed_ns_run(h, lo2, hi2, tied_to=tied, **kw)
+    finally:
+        L.lensed_destroy(h)
+
+
 def test_bad_arguments_are_rejected(L):
     cfg = synth.get_config(0)
     lo, hi = _tiny_priors(cfg)
