@@ -339,7 +339,7 @@ def main():
     ap.add_argument("--no-extras", action="store_true",
                     help="skip the per-config rows (configs 0-3, 5) and the nested-sampling row")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--conv-shape", default="auto", choices=("auto", "wide", "narrow", "strip"),
+    ap.add_argument("--conv-shape", default="auto", choices=("auto", "wide", "narrow", "strip", "half"),
                     help="convolution shape (include/lensed.h); auto = what lensed_create picks")
     ap.add_argument("--interpreter", action="store_true",
                     help="run the interpreting tracer instead of the compile-time specialised one")

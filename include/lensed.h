@@ -225,19 +225,21 @@ lensed_status lensed_set_fg_expansion(lensed_handle *h, double tau);
 lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes);
 long long lensed_frame_bytes(const lensed_handle *h);
 
-/* Convolution shape.  The convolution exists in three shapes (same per-pixel arithmetic):
+/* Convolution shape.  The convolution exists in four shapes (same per-pixel arithmetic):
+ *   3 "half"    as "strip", on 16 x 32 strips with each half-warp on its own parameter vector:
+ *               hugs a mask closer still and moves two vectors per tensor copy: the strip shape
+ *               lensed_create picks
  *   2 "strip"   one block of 8 INDEPENDENT warps per SM, each on its own 16 x 64 output strip with
  *               its own shared-memory stage: nothing is lost at block barriers, masked images skip
  *               whole strips; needs 8 stages of (16 + psf_h - 1) x (64 + 4 ceil(psf_w / 4)) floats
  *               (PSFs up to about 37 rows)
  *   1 "wide"    256 threads on 64 x 128 output tiles, one block per SM: any PSF
  *   0 "narrow"  128 threads on 64 x 64 tiles, two blocks per SM: small or masked images
- * lensed_create picks one (strip for PSFs up to 21 x 21, where its stages are double buffered, and
- * where a mask makes its strip list compute at least 15 % fewer pixels; else wide, or narrow on
- * the same 15 % rule); lensed_set_conv_shape(h, shape) forces one (it
+ * lensed_create picks one (strips for PSFs up to 23 x 23, and where a mask makes the strip list
+ * compute at least 15 % fewer pixels; else wide, or narrow on the same 15 % rule); lensed_set_conv_shape(h, shape) forces one (it
  * rebuilds the tile lists and the frame layout and synchronises the device; EINVAL for another
  * value, LENSED_EUNSUPPORTED if the PSF is too large for that shape's shared memory).
- * lensed_get_conv_shape: 2 / 1 / 0, -1 for NULL.  Rendered pixels do not depend on the shape at
+ * lensed_get_conv_shape: 3 / 2 / 1 / 0, -1 for NULL.  Rendered pixels do not depend on the shape at
  * all; logL only through the order in which the per-tile chi-square partials are summed.
  *
  * PSF taps.  The taps of a handle normally sit in a 60 KB pool of constant memory shared by

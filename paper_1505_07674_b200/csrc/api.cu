@@ -54,7 +54,7 @@ struct lensed_handle {
     int n_sm = 1;
     int tap_off = -1, tap_pairs = 0; // this handle's range of the constant tap pool
     unsigned long long *d_gtaps = nullptr;   // the taps in global memory instead, when the pool was full
-    int shape = 1;                  // convolution shape: 0 narrow, 1 wide, 2 strip (conv.cu)
+    int shape = 1;                  // convolution shape: 0 narrow, 1 wide, 2 strip, 3 half-width strip (conv.cu)
     std::vector<uint8_t> counted;   // host copy of the counted-pixel map (lensed_set_conv_shape rebuilds the tiles)
 
     // device, immutable after create
@@ -292,7 +292,7 @@ lensed_status build_tiles(lensed_handle *h, int shape)
     h->ox_ll = x0 < W ? x0 / 4 * 4 : 0;
     h->oy_ll = y0 < H ? y0 : 0;
     int rows, cols;
-    if (shape == 2) {
+    if (shape >= 2) {
         // strips carry their own pixel coordinates (strip_list): no grid origin
         int r1, c1, r2, c2;
         h->ox_ll = h->oy_ll = 0;
@@ -330,24 +330,27 @@ int default_shape(const lensed_handle *h)
 #ifdef LENSED_CONV_FORCE_SHAPE
     return LENSED_CONV_FORCE_SHAPE;
 #endif
-    long long px[3];
-    for (int shape = 0; shape < 3; ++shape) {
+    long long px[4];
+    for (int shape = 0; shape < 4; ++shape) {
         int tw, th, ny, nx, x0 = h->W, y0 = h->H;
         conv_tile_shape(shape, &tw, &th);
         for (int i = 0; i < h->H; ++i)
             for (int j = 0; j < h->W; ++j)
                 if (h->counted[(size_t)i * h->W + j]) { x0 = std::min(x0, j); y0 = std::min(y0, i); }
         std::vector<uint32_t> tiles;
-        if (shape == 2) strip_list(h->counted, h->H, h->W, tw, th, tiles, &ny, &nx);
+        if (shape >= 2) strip_list(h->counted, h->H, h->W, tw, th, tiles, &ny, &nx);
         else tile_list(h->counted, h->H, h->W, tw, th, x0 < h->W ? x0 / 4 * 4 : 0, y0 < h->H ? y0 : 0, tiles, &ny, &nx);
         px[shape] = conv_shape_fits(h->KH, h->NC, shape) ? (long long)tiles.size() * tw * th : (1LL << 60);
     }
     const int block = px[0] * 100 <= px[1] * 85 ? 0 : 1;
-    if (!conv_shape_fits(h->KH, h->NC, 2)) return block;
-    // strips: where their stages are double buffered (PSFs up to 21 x 21) they are as fast as the wide
-    // tiles on full images and faster on small ones (HST 0.069 against 0.076 ms); with one stage per
-    // warp (larger PSFs) only where they compute at least 15 % fewer pixels
-    return conv_num_stages(h->KH, h->NC, false, 2) == 2 || px[2] * 100 <= px[block] * 85 ? 2 : block;
+    const int strip = conv_shape_fits(h->KH, h->NC, 3) ? 3 : 2;      // half-width strips wherever their two-vector stage fits
+    if (!conv_shape_fits(h->KH, h->NC, strip)) return block;
+    // strips: with PSFs up to 23 x 23 (where full strips are double buffered) they are as fast as the
+    // wide tiles on full images and faster on small ones (HST 0.067 against 0.076 ms); with larger PSFs
+    // only where they compute at least 15 % fewer pixels.  Half-width strips beat full ones on every
+    // config (two vectors per tensor copy; SLACS annulus 39 x 512 = 20.0 k pixels against 23 x 1024 =
+    // 23.6 k: 1.27 against 1.49 ms; Euclid 33.9 against 34.6; profiles/r2b.md).
+    return conv_num_stages(h->KH, h->NC, false, 2) == 2 || px[strip] * 100 <= px[block] * 85 ? strip : block;
 }
 
 // Pixels of the traced list one tracer block walks: it amortises its prologue (constants, frame
@@ -985,10 +988,10 @@ lensed_status lensed_set_chunk_bytes(lensed_handle *h, long long bytes)
 lensed_status lensed_set_conv_shape(lensed_handle *h, int shape)
 {
     if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
-    if (shape < 0 || shape > 2) return fail(h, LENSED_EINVAL, "shape = %d is not 0 (narrow), 1 (wide) or 2 (strip)", shape);
+    if (shape < 0 || shape > 3) return fail(h, LENSED_EINVAL, "shape = %d is not 0 (narrow), 1 (wide), 2 (strip) or 3 (half-width strip)", shape);
     if (!conv_shape_fits(h->KH, h->NC, shape))
         return fail(h, LENSED_EUNSUPPORTED, "a %d x %d PSF does not fit the %s shape's shared memory", h->KH, h->KW,
-                    shape == 0 ? "narrow" : "strip");
+                    shape == 0 ? "narrow" : shape == 2 ? "strip" : "half-width strip");
     return build_tiles(h, shape);
 }
 

@@ -426,19 +426,29 @@ __global__ void __maxnreg__(176) conv_kernel(const __grid_constant__ ConvArgs a,
 // vectors (64 of the 255 a one-warp block may use); stages are double buffered when 16 of them fit.
 constexpr int kSH = 16, kSW = 64;      // strip: the 4 x 8 lanes of a warp on 4 x 8 thread tiles
 constexpr int kStripWarps = 8;
+// staged row pitch in float4: strip width + 4 NC; half-width strips pad it to an odd number of float4
+// (4 mod 8 floats): see conv_strip_kernel HALF
+__host__ __device__ constexpr int strip_pitch4(int NC, bool half) { return half ? (8 + NC) | 1 : kSW / 4 + NC; }
 
-template <bool RENDER, bool GT>
+// HALF: strips of 16 x 32 pixels, each half-warp on its own parameter vector (same strip, vectors
+// 2 pb and 2 pb + 1; ONE tensor copy with a box two vectors deep fetches both tiles).  For masked
+// images: the narrower strips hug the mask better (SLACS annulus: 80 % of the computed pixels are
+// counted against 68 % with 64-wide strips).  Thread tile, taps and loops are the same; the staged
+// row pitch is kept at 4 (mod 8) floats so that the 4 + 4 lanes of a quarter-warp, two tile rows
+// apart in pitch, fall on different halves of the banks.
+template <bool RENDER, bool GT, bool HALF>
 __global__ void __maxnreg__(224) conv_strip_kernel(const __grid_constant__ ConvArgs a,
-                                                                         const __grid_constant__ CUtensorMap tmap)
+                                                   const __grid_constant__ CUtensorMap tmap)
 {
-    constexpr int NTX = 8, kGroup = 32;
+    constexpr int NTX = HALF ? 4 : 8, kGroup = 4 * NTX, kW = 2 * kGroup;
     const unsigned long long *gt = a.gtaps;
     extern __shared__ __align__(128) float4 smem4[];
     __shared__ __align__(8) unsigned long long s_bar[2];
     const int lane = threadIdx.x;
-    const int IW4 = kSW / 4 + a.NC, IW = 4 * IW4;
+    const int IW4 = strip_pitch4(a.NC, HALF), IW = 4 * IW4;
     const int IH = kSH + a.KH - 1 + kSlackRows;
-    const int stage_floats = (IH * IW + 31) / 32 * 32;
+    const int slab4 = (IH - kSlackRows) * IW4;                       // one vector's tile, float4 units
+    const int stage_floats = ((HALF ? 2 : 1) * 4 * slab4 + kSlackRows * IW + 31) / 32 * 32;
     float *s_stage = reinterpret_cast<float *>(smem4);
     if (lane == 0) {
         mbar_init(&s_bar[0], 1);
@@ -447,17 +457,20 @@ __global__ void __maxnreg__(224) conv_strip_kernel(const __grid_constant__ ConvA
     }
     __syncwarp();
 
-    const long long n_items = (long long)a.n_tiles * a.nb;
+    const int n_sub = HALF ? (a.nb + 1) >> 1 : a.nb;                 // items per strip: vectors, or pairs of vectors
+    const long long n_items = (long long)a.n_tiles * n_sub;
     const int lo = (int)(n_items * blockIdx.x / gridDim.x), hi = (int)(n_items * (blockIdx.x + 1) / gridDim.x);
     if (lo >= hi) return;
-    const int tx = lane & 7, ty = lane >> 3;
+    const int half = HALF ? lane >> 4 : 0;
+    const int tx = lane & (NTX - 1), ty = (lane >> (HALF ? 2 : 3)) & 3;
 
     auto issue = [&](int item, int s) {
         if (lane == 0) {
-            const int t = item / a.nb, b = item - t * a.nb;
+            const int t = item / n_sub, pb = item - t * n_sub;
             const uint32_t tile = a.tiles[t];
-            mbar_expect_tx(&s_bar[s], (unsigned)((IH - kSlackRows) * IW * sizeof(float)));
-            tma_load_3d(s_stage + (size_t)s * stage_floats, &tmap, &s_bar[s], (int)(tile & 0xffffu), (int)(tile >> 16), b);
+            mbar_expect_tx(&s_bar[s], (unsigned)((HALF ? 2 : 1) * 4 * slab4 * sizeof(float)));
+            tma_load_3d(s_stage + (size_t)s * stage_floats, &tmap, &s_bar[s], (int)(tile & 0xffffu), (int)(tile >> 16),
+                        HALF ? 2 * pb : pb);
         }
     };
 
@@ -472,7 +485,9 @@ __global__ void __maxnreg__(224) conv_strip_kernel(const __grid_constant__ ConvA
 #pragma unroll 1
     for (int item = lo; item < hi; ++item) {
         const int s = a.n_stages == 2 ? ((item - lo) & 1) : 0;
-        const int t = item / a.nb, b = item - t * a.nb;
+        const int t = item / n_sub, pb = item - t * n_sub;
+        const int b = HALF ? 2 * pb + half : pb;                      // this (half-)warp's parameter vector
+        const bool has_b = b < a.nb;                                  // odd batch: the last pair's second half idles
         const uint32_t tile = a.tiles[t];
         const int oy = (int)(tile >> 16) + ty * kTR, ox = (int)(tile & 0xffffu) + tx * 4;      // strips carry pixel coordinates
         const bool more = item + 1 < hi;
@@ -505,7 +520,7 @@ __global__ void __maxnreg__(224) conv_strip_kernel(const __grid_constant__ ConvA
             for (int e = 0; e < 8; ++e) acc[p][e] = bc(0.0f);
         if (warp_any) {
             const float4 *in_base = reinterpret_cast<const float4 *>(s_stage + (size_t)s * stage_floats) +
-                                    (size_t)(ty * kTR) * IW4 + tx;
+                                    (size_t)half * slab4 + (size_t)(ty * kTR) * IW4 + tx;
             const int last_taps = a.KW - 4 * (a.NC - 1);
             const int n_full = last_taps == 4 ? a.NC : a.NC - 1;
 #pragma unroll 1
@@ -526,15 +541,17 @@ __global__ void __maxnreg__(224) conv_strip_kernel(const __grid_constant__ ConvA
             for (int e = 0; e < 8; ++e) un2(acc[p][e], out[2 * p][e], out[2 * p + 1][e]);
 
         if (RENDER) {
-            const bool valid = a.derived[(size_t)b * a.D] != 0.0f;
-            float *mb = a.model + (size_t)b * a.H * a.W;
+            if (has_b) {
+                const bool valid = a.derived[(size_t)b * a.D] != 0.0f;
+                float *mb = a.model + (size_t)b * a.H * a.W;
 #pragma unroll
-            for (int o = 0; o < kTR; ++o)
+                for (int o = 0; o < kTR; ++o)
 #pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
-                    if (y < a.H && x < a.W) mb[(size_t)y * a.W + x] = valid ? out[o][e] : nanf("");
-                }
+                    for (int e = 0; e < 8; ++e) {
+                        const int y = oy + o, x = ox + (e & 3) + (e >> 2) * kGroup;
+                        if (y < a.H && x < a.W) mb[(size_t)y * a.W + x] = valid ? out[o][e] : nanf("");
+                    }
+            }
         } else {
             float part = 0.0f;
             if (warp_any) {
@@ -547,10 +564,10 @@ __global__ void __maxnreg__(224) conv_strip_kernel(const __grid_constant__ ConvA
                             part = fmaf(wreg[o][e] * diff, diff, part);
                         }
             }
-            double sum = (double)part;
+            double sum = (double)part;                      // over the lanes of this vector: the warp, or its half
 #pragma unroll
-            for (int off = 16; off > 0; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
-            if (lane == 0) a.partial[(size_t)b * a.n_tiles + t] = sum;
+            for (int off = HALF ? 8 : 16; off > 0; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
+            if ((lane & (HALF ? 15 : 31)) == 0 && has_b) a.partial[(size_t)b * a.n_tiles + t] = sum;
         }
         __syncwarp();              // every lane is done with stage s
         if (a.n_stages == 1 && more) issue(item + 1, 0);
@@ -570,32 +587,38 @@ __global__ void final_kernel(FinalArgs a)
 
 }  // namespace
 
-// shape: 0 = narrow, 1 = wide, 2 = strip (ConvArgs::shape)
+// shape: 0 = narrow, 1 = wide, 2 = strip, 3 = half-width strip (ConvArgs::shape)
 void conv_tile_shape(int shape, int *tile_w, int *tile_h)
 {
-    *tile_w = shape == 1 ? Shape<16>::kTW : shape == 0 ? Shape<8>::kTW : kSW;
-    *tile_h = shape == 2 ? kSH : kTH;
+    *tile_w = shape == 1 ? Shape<16>::kTW : shape == 0 ? Shape<8>::kTW : shape == 2 ? kSW : kSW / 2;
+    *tile_h = shape >= 2 ? kSH : kTH;
 }
 
 // rows x cols = the image rounded up to cover every tile of the grids in use (api.cu)
 void conv_padded_shape(int rows, int cols, int KH, int NC, int *Hp, int *Wp)
 {
     *Hp = rows + KH - 1;
-    *Wp = (cols + 3) / 4 * 4 + 4 * NC;
+    *Wp = (cols + 3) / 4 * 4 + 4 * NC + 4;               // + 4: the padded pitch of the half-width strips' boxes
 }
 
 namespace {
 // dynamic shared memory a block may take: 227 KB per SM minus the static arrays, per resident block
-size_t smem_limit(int shape) { return shape == 0 ? 112 * 1024 : shape == 2 ? 28 * 1024 : 226 * 1024; }   // strip: 8 blocks per SM
+size_t smem_limit(int shape) { return shape == 0 ? 112 * 1024 : shape >= 2 ? 28 * 1024 : 226 * 1024; }   // strips: 8 blocks per SM
 size_t stage_bytes(int KH, int NC, int shape)
 {
-    int tw, th;
-    conv_tile_shape(shape, &tw, &th);
-    const size_t floats = (size_t)(th + KH - 1 + kSlackRows) * (tw + 4 * NC);
+    size_t floats;
+    if (shape >= 2) {
+        const size_t IW = 4 * (size_t)strip_pitch4(NC, shape == 3);
+        floats = (shape == 3 ? 2 : 1) * (size_t)(kSH + KH - 1) * IW + kSlackRows * IW;
+    } else {
+        int tw, th;
+        conv_tile_shape(shape, &tw, &th);
+        floats = (size_t)(th + KH - 1 + kSlackRows) * (tw + 4 * NC);
+    }
     return (floats + 31) / 32 * 32 * sizeof(float);
 }
-// d and w of a tile staged in shared memory (block shapes, loglike); the strip shape reads them from global memory
-size_t dw_bytes(bool render, int shape) { return render || shape == 2 ? 0 : (size_t)2 * kTH * (shape == 1 ? 128 : 64) * sizeof(float); }
+// d and w of a tile staged in shared memory (block shapes, loglike); the strip shapes keep them in registers
+size_t dw_bytes(bool render, int shape) { return render || shape >= 2 ? 0 : (size_t)2 * kTH * (shape == 1 ? 128 : 64) * sizeof(float); }
 }  // namespace
 
 int conv_num_stages(int KH, int NC, bool render, int shape)
@@ -621,10 +644,10 @@ cudaError_t set_attr()
     return cudaFuncSetAttribute(conv_kernel<RENDER, NTX, GT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)smem_limit(NTX == 16 ? 1 : 0));
 }
-template <bool RENDER, bool GT>
+template <bool RENDER, bool GT, bool HALF>
 cudaError_t set_attr_strip()
 {
-    return cudaFuncSetAttribute(conv_strip_kernel<RENDER, GT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024);
+    return cudaFuncSetAttribute(conv_strip_kernel<RENDER, GT, HALF>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024);
 }
 template <bool RENDER, int NTX, bool GT>
 void launch(const ConvArgs &a, const CUtensorMap &tmap, int grid, size_t smem, cudaStream_t st)
@@ -634,7 +657,8 @@ void launch(const ConvArgs &a, const CUtensorMap &tmap, int grid, size_t smem, c
 template <bool RENDER, bool GT>
 void launch_strip(const ConvArgs &a, const CUtensorMap &tmap, int grid, size_t smem, cudaStream_t st)
 {
-    conv_strip_kernel<RENDER, GT><<<grid, 32, smem, st>>>(a, tmap);
+    if (a.shape == 3) conv_strip_kernel<RENDER, GT, true><<<grid, 32, smem, st>>>(a, tmap);
+    else conv_strip_kernel<RENDER, GT, false><<<grid, 32, smem, st>>>(a, tmap);
 }
 }  // namespace
 
@@ -645,7 +669,7 @@ cudaError_t conv_setup()
     LENSED_SET(false, 16, false) LENSED_SET(true, 16, false) LENSED_SET(false, 8, false) LENSED_SET(true, 8, false)
     LENSED_SET(false, 16, true) LENSED_SET(true, 16, true) LENSED_SET(false, 8, true) LENSED_SET(true, 8, true)
 #undef LENSED_SET
-#define LENSED_SET(R, G) if ((e = set_attr_strip<R, G>()) != cudaSuccess) return e;
+#define LENSED_SET(R, G) if ((e = set_attr_strip<R, G, false>()) != cudaSuccess || (e = set_attr_strip<R, G, true>()) != cudaSuccess) return e;
     LENSED_SET(false, false) LENSED_SET(true, false) LENSED_SET(false, true) LENSED_SET(true, true)
 #undef LENSED_SET
     return cudaSuccess;
@@ -675,7 +699,8 @@ cudaError_t conv_make_tensor_map(void *out, const float *L, int Wp, int Hp, long
     const cuuint64_t strides[2] = {(cuuint64_t)Wp * sizeof(float), (cuuint64_t)Wp * Hp * sizeof(float)};
     int tw, th;
     conv_tile_shape(shape, &tw, &th);
-    const cuuint32_t box[3] = {(cuuint32_t)(tw + 4 * NC), (cuuint32_t)(th + KH - 1), 1};
+    const cuuint32_t box[3] = {(cuuint32_t)(shape >= 2 ? 4 * strip_pitch4(NC, shape == 3) : tw + 4 * NC), (cuuint32_t)(th + KH - 1),
+                               (cuuint32_t)(shape == 3 ? 2 : 1)};
     const cuuint32_t estr[3] = {1, 1, 1};
     const CUresult r = encode((CUtensorMap *)out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)L, dims, strides, box, estr,
                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
@@ -691,7 +716,8 @@ cudaError_t launch_conv(ConvArgs a, const void *tensor_map, bool render, int n_s
     a.n_stages = conv_num_stages(a.KH, a.NC, render, a.shape);
     size_t smem = conv_smem_bytes(a.KH, a.NC, render, a.shape);
     const long long n_items = (long long)a.n_tiles * a.nb;
-    if (a.shape == 2) {
+    if (a.shape >= 2) {
+        const long long n_strip_items = (long long)a.n_tiles * (a.shape == 3 ? (a.nb + 1) / 2 : a.nb);
         // k one-warp blocks per SM: the request is padded so that exactly k fit (228 KB per SM, 1 KB
         // reserved per block) -- otherwise the block scheduler packs up to 12 on some SMs and leaves
         // others empty
@@ -700,7 +726,7 @@ cudaError_t launch_conv(ConvArgs a, const void *tensor_map, bool render, int n_s
         k = std::max(1, std::min(k, (int)((228 * 1024) / (smem + 1024 + 64))));
         smem = std::max(smem, (size_t)((228 * 1024) / k - 1024 - 64) / 128 * 128);
         const long long n_warps = (long long)n_sm * k;
-        const int grid = (int)(n_items < n_warps ? n_items : n_warps);
+        const int grid = (int)(n_strip_items < n_warps ? n_strip_items : n_warps);
         if (grid < 1) return cudaSuccess;
         if (render) { if (gt) launch_strip<true, true>(a, tmap, grid, smem, st); else launch_strip<true, false>(a, tmap, grid, smem, st); }
         else        { if (gt) launch_strip<false, true>(a, tmap, grid, smem, st); else launch_strip<false, false>(a, tmap, grid, smem, st); }

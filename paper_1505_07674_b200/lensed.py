@@ -264,7 +264,7 @@ def lensed_frame_bytes(h):
     return lib().lensed_frame_bytes(h)
 
 
-CONV_SHAPES = ("narrow", "wide", "strip")     # lensed_set_conv_shape / lensed_get_conv_shape: 0, 1, 2
+CONV_SHAPES = ("narrow", "wide", "strip", "half")     # lensed_set_conv_shape / lensed_get_conv_shape: 0, 1, 2, 3
 
 
 def lensed_set_conv_shape(h, shape):

@@ -485,25 +485,26 @@ def test_all_convolution_shapes_and_both_tap_paths(L, index, H, W, B, global_tap
     try:
         assert L.lensed_uses_global_taps(h) == int(global_taps)
         models = []
-        for shape in (2, 1, 0):
+        for shape in (3, 2, 1, 0):
             L.lensed_set_conv_shape(h, shape)
             assert L.lensed_get_conv_shape(h) == shape
             logl, model = _gpu_eval(L, h, params, cfg.H, cfg.W)
             assert logl_errors(logl, logl_o).max() <= LOGL_RTOL
             assert pixel_errors(model, model_o).max() <= PIXEL_RTOL
             models.append(model)
-        assert np.array_equal(models[0], models[1]) and np.array_equal(models[0], models[2])
+        assert all(np.array_equal(models[0], m) for m in models[1:])
         with pytest.raises(L.LensedError) as e:
-            L.lensed_set_conv_shape(h, 3)
+            L.lensed_set_conv_shape(h, 4)
         assert e.value.status == L.EINVAL
     finally:
         L.lensed_destroy(h)
 
 
 def test_shape_picked_at_create_and_shared_memory_limits(L):
-    """lensed_create: wide for a full image, strip for the SLACS annulus (its strips compute 22 %
-    fewer pixels than the narrow tiles); a 63 x 63 PSF does not fit the strip shape's eight stages."""
-    for index, want in ((4, 1), (2, 2)):
+    """lensed_create: wide for a full image with a large PSF, half-width strips for the SLACS annulus
+    (39 of them compute 20.0 k pixels, 23 full strips 23.6 k, 8 narrow tiles 32.8 k); a 63 x 63 PSF
+    does not fit the strip shapes' eight stages."""
+    for index, want in ((4, 1), (2, 3)):
         h = Problem(synth.get_config(index), image=np.zeros((synth.get_config(index).H, synth.get_config(index).W), np.float32),
                     weight=np.ones((synth.get_config(index).H, synth.get_config(index).W), np.float32)).create()
         try:
@@ -515,9 +516,10 @@ def test_shape_picked_at_create_and_shared_memory_limits(L):
     h = Problem(cfg, image=np.zeros((40, 36), np.float32), weight=np.ones((40, 36), np.float32)).create()
     try:
         assert L.lensed_get_conv_shape(h) in (0, 1)
-        with pytest.raises(L.LensedError) as e:
-            L.lensed_set_conv_shape(h, 2)
-        assert e.value.status == L.EUNSUPPORTED
+        for shape in (2, 3):
+            with pytest.raises(L.LensedError) as e:
+                L.lensed_set_conv_shape(h, shape)
+            assert e.value.status == L.EUNSUPPORTED
     finally:
         L.lensed_destroy(h)
 
