@@ -365,7 +365,9 @@ void lensed_ns_philox(const unsigned *counter, const unsigned *key, unsigned *ou
 lensed_status lensed_fma_peak(int device, int iters, double *tflops);
 
 /* Text of the last error on this handle (valid until the next call on the handle); for
- * a failed lensed_create or lensed_fma_peak pass NULL to read the thread-local text.    */
+ * a failed lensed_create or lensed_fma_peak pass NULL to read the thread-local text.  After a
+ * successful lensed_create it is empty, or says why the list's tracer could not be specialised at
+ * run time (the interpreting tracer is then in use; see "Tracer selection").               */
 const char *lensed_last_error(const lensed_handle *h);
 
 /* Frees the handle and its device memory (synchronises the device).  NULL is a no-op.   */

@@ -721,8 +721,8 @@ cudaError_t launch_conv(ConvArgs a, const void *tensor_map, bool render, int n_s
         // k one-warp blocks per SM: the request is padded so that exactly k fit (228 KB per SM, 1 KB
         // reserved per block) -- otherwise the block scheduler packs up to 12 on some SMs and leaves
         // others empty
-        int k = kStripWarps;
-        if (const char *e = getenv("LENSED_STRIP_WARPS")) k = atoi(e);       // tuning
+        static const int k_env = [] { const char *e = getenv("LENSED_STRIP_WARPS"); return e ? atoi(e) : 0; }();   // tuning
+        int k = k_env > 0 ? k_env : kStripWarps;
         k = std::max(1, std::min(k, (int)((228 * 1024) / (smem + 1024 + 64))));
         smem = std::max(smem, (size_t)((228 * 1024) / k - 1024 - 64) / 128 * 128);
         const long long n_warps = (long long)n_sm * k;
