@@ -524,6 +524,16 @@ def test_shape_picked_at_create_and_shared_memory_limits(L):
         L.lensed_destroy(h)
 
 
+def _require_jit(L, h):
+    """the handle's tracer must be the run-time specialised one; skip where that is switched off or
+    the box has no NVRTC (the library then runs the interpreter, which the other tests cover)"""
+    import os
+    kind, why = L.lensed_get_static_tracer(h), L.lensed_last_error(h) or ""
+    if kind != 2 and (os.environ.get("LENSED_JIT", "")[:1] == "0" or "not found" in why):
+        pytest.skip("run-time specialisation unavailable: " + (why or "LENSED_JIT=0"))
+    assert kind == 2, why
+
+
 def test_a_list_without_a_built_in_signature_gets_its_tracer_compiled_at_create(L):
     """SIE + shear + two Gaussian sources + Gaussian lens light + sky has none of the built-in
     signatures: lensed_create specialises the tracer for it with NVRTC (csrc/jit.cu; the paper
@@ -546,8 +556,7 @@ def test_a_list_without_a_built_in_signature_gets_its_tracer_compiled_at_create(
     logl_o, model_o = prob.oracle_loglike(params, want_model=True)
     h = prob.create()
     try:
-        kind = L.lensed_get_static_tracer(h)
-        assert kind == 2, L.lensed_last_error(h)
+        _require_jit(L, h)
         logl_j, model_j = _gpu_eval(L, h, params, cfg.H, cfg.W)
         L.lensed_set_static_tracer(h, 0)
         assert L.lensed_get_static_tracer(h) == 0
@@ -613,7 +622,7 @@ def test_run_time_specialised_tracers_of_assorted_lists_against_the_oracle(L, se
     logl_o, model_o = prob.oracle_loglike(params, want_model=True)
     h = prob.create()
     try:
-        assert L.lensed_get_static_tracer(h) == 2, L.lensed_last_error(h)
+        _require_jit(L, h)
         got = [_gpu_eval(L, h, params, H, W)]
         L.lensed_set_static_tracer(h, 0)
         got.append(_gpu_eval(L, h, params, H, W))
