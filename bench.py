@@ -469,13 +469,16 @@ def main():
     if args.config == DEFAULT_CONFIG and not args.no_extras and world == 1 and not args.batch:
         per_config = []
         for c, steps in ((0, 20), (1, 20), (2, 10), (3, 5), (5, 10)):
-            b = Bench(lensed, torch, c, synth.get_config(c).B, local, rank, args)
-            row = b.summary(steps, 3, flush)
-            if not args.no_cpu_baseline:                     # the oracle beside every row, ~3 s each
-                v, cores, n, dt = time_oracle(b.cfg, b.image, b.weight, b.params, 3.0)
-                row["cpu_oracle"] = {"logl_per_s": v, "cores": cores, "sample": "%d vectors, %.1f s" % (n, dt)}
+            try:
+                b = Bench(lensed, torch, c, synth.get_config(c).B, local, rank, args)
+                row = b.summary(steps, 3, flush)
+                if not args.no_cpu_baseline:                 # the oracle beside every row, ~3 s each
+                    v, cores, n, dt = time_oracle(b.cfg, b.image, b.weight, b.params, 3.0)
+                    row["cpu_oracle"] = {"logl_per_s": v, "cores": cores, "sample": "%d vectors, %.1f s" % (n, dt)}
+                b.close()
+            except Exception as ex:                          # noqa: BLE001 -- an extra: the bench line stands without it
+                row = {"config": c, "error": str(ex)[:200]}
             per_config.append(row)
-            b.close()
         try:
             nested = nested_row(lensed, torch, local)
         except Exception as ex:                              # noqa: BLE001 -- an extra, see above
