@@ -364,6 +364,13 @@ void lensed_ns_philox(const unsigned *counter, const unsigned *key, unsigned *ou
  * the achieved TFLOP/s (2 flops per FFMA) in *tflops.  Synchronous.                     */
 lensed_status lensed_fma_peak(int device, int iters, double *tflops);
 
+/* lensed_issue_probe -- a second micro-benchmark behind the kernel design (DESIGN.md section 5,
+ * profiles/r2b.md): FP32-pipe time of a loop body of 64 packed FFMA2 with n_extra in {0, 8, 16, 32,
+ * 64} instructions of another kind among them (kind 0 none, 1 LOP3 on the ALU pipe, 2 MUFU.EX2,
+ * 3 scalar FFMA, 4 IMAD), `warps` in {1, 2, 4} warps per scheduler on every SM.  *cycles_per_body:
+ * SM cycles per body and warp (128 = the pipe's full rate).  Synchronous.  EINVAL / ECUDA.      */
+lensed_status lensed_issue_probe(int device, int kind, int n_extra, int warps, double *cycles_per_body);
+
 /* Text of the last error on this handle (valid until the next call on the handle); for
  * a failed lensed_create or lensed_fma_peak pass NULL to read the thread-local text.  After a
  * successful lensed_create it is empty, or says why the list's tracer could not be specialised at

@@ -1033,6 +1033,17 @@ int lensed_get_static_tracer(const lensed_handle *h)
     return !h->static_tracer ? 0 : trace_has_static(h->prog) ? 1 : 2;
 }
 
+lensed_status lensed_issue_probe(int device, int kind, int n_extra, int warps, double *cycles_per_body)
+{
+    if (!cycles_per_body) return fail(nullptr, LENSED_EINVAL, "lensed_issue_probe: null argument");
+    if (cudaSetDevice(device) != cudaSuccess)
+        return fail(nullptr, LENSED_ECUDA, "lensed_issue_probe: no CUDA device %d", device);
+    const cudaError_t e = run_issue_probe(kind, n_extra, warps, cycles_per_body);
+    if (e == cudaErrorInvalidValue) return fail(nullptr, LENSED_EINVAL, "lensed_issue_probe: kind 0..4, n_extra in {0, 8, 16, 32, 64}, warps in {1, 2, 4}");
+    if (e != cudaSuccess) return fail(nullptr, LENSED_ECUDA, "lensed_issue_probe: %s", cudaGetErrorString(e));
+    return LENSED_OK;
+}
+
 lensed_status lensed_fma_peak(int device, int iters, double *tflops)
 {
     if (!tflops || iters < 1) return fail(nullptr, LENSED_EINVAL, "lensed_fma_peak: bad argument");

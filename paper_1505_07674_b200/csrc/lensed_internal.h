@@ -206,6 +206,7 @@ size_t conv_smem_bytes(int KH, int NC, bool render, int shape);
 bool conv_shape_fits(int KH, int NC, int shape);
 int conv_num_stages(int KH, int NC, bool render, int shape);   // input-tile buffers per block (2 = double buffered)
 cudaError_t run_fma_peak(int iters, double *tflops);
+cudaError_t run_issue_probe(int kind, int n_extra, int warps, double *cycles_per_body);
 
 // for the clients of the handle outside api.cu (nested.cu): error text on the handle, its device
 int handle_fail(::lensed_handle *h, int status, const char *fmt, ...);

@@ -56,6 +56,7 @@ SYMBOLS = {
     "lensed_ns_run": (_i, [_p, _p, _p, _p, _i, _p, _p, _p, _p, _p, _ll, _p]),
     "lensed_ns_philox": (None, [_p, _p, _p]),
     "lensed_fma_peak": (_i, [_i, _i, _p]),
+    "lensed_issue_probe": (_i, [_i, _i, _i, _i, _p]),
     "lensed_last_error": (_c, [_p]),
     "lensed_destroy": (None, [_p]),
 }
@@ -348,6 +349,13 @@ def lensed_fma_peak(device=0, iters=4096):
     t = ctypes.c_double()
     _check(lib().lensed_fma_peak(int(device), int(iters), ctypes.byref(t)))
     return t.value
+
+
+def lensed_issue_probe(device=0, kind=0, n_extra=0, warps=2):
+    """-> SM cycles per body of 64 FFMA2 + n_extra instructions of `kind` (include/lensed.h)"""
+    out = ctypes.c_double()
+    _check(lib().lensed_issue_probe(int(device), int(kind), int(n_extra), int(warps), ctypes.byref(out)))
+    return out.value
 
 
 def lensed_last_error(h=None):
