@@ -682,8 +682,9 @@ def test_every_one_of_192_draws_of_the_prior_meets_the_tolerances(L, index, H, W
     bounds.  In plain FP32 about one draw in a hundred misses 1e-5 on logL (a source cusp on a
     pixel: DESIGN.md section 6); the FP64 refinement of the flagged pixels (refine.cu) closes
     that tail, and switching it off brings it back (test_refinement_switch below)."""
+    import os
     cfg = synth.shrunk(synth.get_config(index), H, W, 4)
-    params = cfg.batch(192)
+    params = cfg.batch(int(os.environ.get("LENSED_ENVELOPE_DRAWS", "192")))     # more draws: DESIGN.md section 6
     prob = Problem(cfg)
     h = prob.create()
     try:
