@@ -118,6 +118,9 @@ bool jit_wanted(const int (&c)[K_COUNT])
     if (env && env[0] == '0') return false;
     const int n_lens = c[K_SHEAR] + c[K_SIE] + c[K_SIS] + c[K_POINT];
     const int n_pos = c[K_SRC_SERSIC] + c[K_SRC_GAUSS] + c[K_FG_SERSIC] + c[K_FG_GAUSS];
+#ifdef LENSED_JIT_NO_LIMITS             // tuning builds: how far does the specialised template carry?
+    return c[K_SHEAR] <= 1 && n_lens + n_pos >= 1;
+#endif
     return c[K_SHEAR] <= 1 && c[K_SIE] <= 3 && n_lens <= 6 && n_pos >= 0 && n_pos <= 8 && n_lens + n_pos >= 1;
 }
 

@@ -633,6 +633,19 @@ def test_run_time_specialised_tracers_of_assorted_lists_against_the_oracle(L, se
         assert pixel_errors(model, model_o).max() <= PIXEL_RTOL
 
 
+def test_issue_probe_measures_the_fp32_pipe_at_its_full_rate(L):
+    """lensed_issue_probe (csrc/peak.cu), the micro-benchmark behind profiles/r2b.md: 64 packed FFMA2
+    per body take 128 cycles (2 each), extra ALU-pipe instructions cost less than a cycle each,
+    integer multiply-adds about two; bad arguments are EINVAL."""
+    base = L.lensed_issue_probe(0, 0, 0, 2)
+    assert 126.0 <= base <= 136.0
+    assert base <= L.lensed_issue_probe(0, 1, 16, 2) <= base + 16.0
+    assert L.lensed_issue_probe(0, 4, 32, 2) >= base + 40.0
+    with pytest.raises(L.LensedError) as e:
+        L.lensed_issue_probe(0, 1, 5, 2)
+    assert e.value.status == L.EINVAL
+
+
 def test_largest_rule_and_longest_model_list(L):
     """LENSED_MAX_QUAD-class rule (15 x 15 = 225 points, the size of the paper's g7k15) and a list
     of LENSED_MAX_MODELS = 32 objects (interpreting tracer, every kind present)."""
