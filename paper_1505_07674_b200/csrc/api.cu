@@ -419,7 +419,10 @@ lensed_status run(lensed_handle *h, const float *params_dev, int B, float *out_d
     if (sorted && (s = grow(h, &h->d_order, &h->cap_order, (size_t)B, st)) != LENSED_OK) return s;
     if ((s = timed_begin(h, PH_PREP, st)) != LENSED_OK) return s;
     CU(h, launch_prep(prog, pa, st));
-    if (sorted) CU(h, launch_order(h->d_derived, prog.D, B, Bc, h->d_order, st));
+    if (sorted) {
+        CU(h, launch_order(h->d_derived, prog.D, B, Bc, h->d_order, st));
+        h->launches[PH_PREP] += 1;                           // two kernels in this phase: prep, order
+    }
     if ((s = timed_end(h, st)) != LENSED_OK) return s;
 
     for (int b0 = 0; b0 < B; b0 += Bc) {
