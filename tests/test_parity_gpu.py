@@ -327,7 +327,7 @@ def test_host_buffer_calls_match_device_calls_and_chunking_does_not_change_resul
     assert np.array_equal(logl_dev, logl_host) and np.array_equal(logl_dev, out_pinned.numpy())
     assert np.array_equal(model_dev, model_host)
     assert np.array_equal(logl_dev, logl_chunked) and np.array_equal(model_dev, model_chunked)
-    assert n == {"prep": 1, "trace": 14, "refine": 28, "conv": 14, "final": 1}
+    assert n == {"prep": 2, "trace": 14, "refine": 28, "conv": 14, "final": 1}       # prep = prep_kernel + order_kernel
     assert all(v > 0 for v in ms.values())
 
 
