@@ -371,6 +371,52 @@ lensed_status lensed_fma_peak(int device, int iters, double *tflops);
  * SM cycles per body and warp (128 = the pipe's full rate).  Synchronous.  EINVAL / ECUDA.      */
 lensed_status lensed_issue_probe(int device, int kind, int n_extra, int warps, double *cycles_per_body);
 
+/*
+ * lensed_chisq_static -- the likelihood of model images that are already on the device, from a
+ * call that allocates NOTHING: no cudaMalloc, no cudaMallocAsync, no cudaFree, no handle.
+ *   loglike[b] = -1/2 sum_i w_i (d_i - model[b][i])^2       (eqs. 16-17)
+ *
+ * Why it exists.  lensed_create allocates the problem's arrays and lensed_loglike / lensed_render
+ * grow their scratch whenever a batch is larger than any they have seen.  That is wrong for a
+ * caller that may not allocate once it is running: a sampler inside a process whose deep-learning
+ * framework has already taken the device memory for its own pool (a later cudaMalloc then fails);
+ * workers on several streams (lensed_clone), where one worker's cudaMalloc / cudaFree synchronises
+ * the device under all the others; a job on a fixed memory budget (MIG slice, MPS memory limit)
+ * whose budget is checked once at start-up.  Such a caller scores images held in ITS OWN buffers
+ * -- written by lensed_render at a batch size warmed up during set-up, or by its own forward model,
+ * or lensed_render's plus a term this library does not model -- with this call.
+ *
+ *   device      CUDA device ordinal the pointers belong to (made current by the call)
+ *   image_dev   [n_pix] device f32, the data d_i
+ *   weight_dev  [n_pix] device f32, w_i = 1 / s_i^2 >= 0 with 0 at masked pixels;
+ *               pixels with w_i = 0 are skipped, so the model may hold anything (NaN too) there
+ *   model_dev   [B][n_pix] device f32, the PSF-convolved model images L* (lensed_render's layout)
+ *   logl_dev    [B] device f32; -INFINITY for an image with a non-finite pixel under a non-zero
+ *               weight (lensed_render's NaN image of a vector outside the model domain gives the
+ *               -INFINITY lensed_loglike gives that vector)
+ * All four are caller-owned; nothing is retained.  Asynchronous on `cuda_stream`.  Deterministic:
+ * FP32 differences, FP64 sums in a fixed order, bitwise the same on every call.
+ *
+ * Scratch and its limit.  The per-block partial sums live in one fixed array inside the library's
+ * device image: 1 040 KB that every GPU loading the library holds until the process exits.  It
+ * serves at most LENSED_CHISQ_STATIC_MAX_VECTORS images per call (n_pix up to 2^30); a larger B is
+ * refused with LENSED_EINVAL and a message saying so -- split the batch.  EVERY call on a device,
+ * from any thread or stream, uses that same array: two calls that may run on the GPU at the same
+ * time (different streams with no ordering between them) race on it and both results are garbage;
+ * order them with an event, or keep this call on one stream.  The array keeps what the last call
+ * left; each call clears the part that has to start at zero, on its stream, before its kernel.
+ *
+ * First call on a device.  It looks up the array's device address (cudaGetSymbolAddress, which may
+ * load the library's kernels onto that device) and caches it; make that first call during set-up,
+ * before any stream capture begins.  Later calls issue one memset and one kernel, nothing else.
+ *
+ * Errors: EINVAL for null pointers, B < 1, n_pix < 1, B or n_pix beyond the limits, a bad device
+ * ordinal (checked in that order, before CUDA is touched); ECUDA with the CUDA error text.  The
+ * text is read with lensed_last_error(NULL).                                                    */
+#define LENSED_CHISQ_STATIC_MAX_VECTORS 4096
+lensed_status lensed_chisq_static(int device, const float *image_dev, const float *weight_dev, long long n_pix,
+                                  const float *model_dev, int B, float *logl_dev, void *cuda_stream);
+
 /* Text of the last error on this handle (valid until the next call on the handle); for
  * a failed lensed_create or lensed_fma_peak pass NULL to read the thread-local text.  After a
  * successful lensed_create it is empty, or says why the list's tracer could not be specialised at

@@ -57,6 +57,7 @@ SYMBOLS = {
     "lensed_ns_philox": (None, [_p, _p, _p]),
     "lensed_fma_peak": (_i, [_i, _i, _p]),
     "lensed_issue_probe": (_i, [_i, _i, _i, _i, _p]),
+    "lensed_chisq_static": (_i, [_i, _p, _p, _ll, _p, _i, _p, _p]),
     "lensed_last_error": (_c, [_p]),
     "lensed_destroy": (None, [_p]),
 }
@@ -224,6 +225,28 @@ def lensed_loglike_host(h, params_host, logl_host, stream=None):
     pout, _ = _host_ptr(logl_host, None)
     _check(lib().lensed_loglike_host(h, pin, B, pout, _stream(stream)), h)
     return logl_host
+
+
+CHISQ_STATIC_MAX_VECTORS = 4096     # LENSED_CHISQ_STATIC_MAX_VECTORS (include/lensed.h)
+
+
+def lensed_chisq_static(image_dev, weight_dev, model_dev, logl_dev, stream=None):
+    """logL of model images already on the device, from a call that allocates no device memory
+    (for callers that may not: see lensed.h).  image_dev / weight_dev [n_pix] (weight 0 where
+    masked), model_dev [B][n_pix] or [B][H][W], logl_dev [B]: contiguous float32 CUDA tensors on
+    one device.  At most CHISQ_STATIC_MAX_VECTORS images per call; calls that overlap on the GPU
+    race on the library's one scratch array.  Marshalling only: no tensor is created here."""
+    for t in (image_dev, weight_dev, model_dev, logl_dev):
+        if not (t.is_cuda and t.is_contiguous() and str(t.dtype) == "torch.float32"):
+            raise LensedError(EINVAL, "lensed_chisq_static takes contiguous float32 CUDA tensors")
+        if t.device != image_dev.device:
+            raise LensedError(EINVAL, "lensed_chisq_static: tensors on different devices")
+    n_pix, B = int(image_dev.numel()), int(logl_dev.numel())
+    if weight_dev.numel() != n_pix or B < 1 or model_dev.numel() != B * n_pix or model_dev.shape[0] != B:
+        raise LensedError(EINVAL, "lensed_chisq_static: image / weight [n_pix], model [B][n_pix], logl [B]")
+    _check(lib().lensed_chisq_static(int(image_dev.device.index or 0), image_dev.data_ptr(), weight_dev.data_ptr(), n_pix,
+                                     model_dev.data_ptr(), B, logl_dev.data_ptr(), _stream(stream)))
+    return logl_dev
 
 
 def lensed_set_profiling(h, on):
