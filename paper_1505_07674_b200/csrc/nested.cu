@@ -593,7 +593,8 @@ extern "C" lensed_status lensed_ns_run(lensed_handle *h, const float *prior_lo, 
     long long rounds_launched = 0;
     const int check_every = 4;
     for (;;) {
-        for (int r = 0; r < check_every; ++r, ++rounds_launched) {
+        // never a round beyond max_rounds: the convergence check every few rounds must not overshoot it
+        for (int r = 0; r < check_every && rounds_launched < opt->max_rounds; ++r, ++rounds_launched) {
             ns_bound_kernel<<<1, 256, 0, st>>>(pb, d_U, d_m, d_G, d_s, d_state);
             ns_propose_kernel<<<(K + 127) / 128, 128, 0, st>>>(pb, d_m, d_G, d_s, d_Uc, d_theta_c, d_state);
             NS_CU(cudaGetLastError());
@@ -619,7 +620,9 @@ extern "C" lensed_status lensed_ns_run(lensed_handle *h, const float *prior_lo, 
     res->information = host.info;
     res->ln_z_err = sqrt(fmax(host.info, 0.0) / N);
     res->n_rounds = n_rounds;
-    res->n_likelihood = (long long)N + rounds_launched * K;
+    // rounds the sampler used: batches launched after convergence within a group of check_every are
+    // discarded by the ns_* kernels and not counted
+    res->n_likelihood = (long long)N + n_rounds * K;
     res->n_dead = n_dead;
     res->n_samples = host.n_written;
     res->converged = converged;

@@ -77,12 +77,11 @@ def test_three_rounds_agree_point_by_point_with_the_oracle_driver(L):
     prob = Problem(cfg)
     lo, hi = _tiny_priors(cfg)
     kw = dict(n_live=64, batch=48, tol=1e-9, enlarge=1.25, seed=2024, max_rounds=3)
+    # max_rounds = 3 is not a multiple of the driver's convergence-check interval (4): it must stop at 3
     ref = ns.run(lambda t: prob.oracle_loglike(t.astype(np.float32), want_model=False), lo, hi, **kw)
-    # the driver checks convergence every 4 rounds: ask for 4 and compare with 4 oracle rounds
-    kw4 = dict(kw, max_rounds=4)
-    ref = ns.run(lambda t: prob.oracle_loglike(t.astype(np.float32), want_model=False), lo, hi, **kw4)
-    got = _gpu_run(L, prob, lo, hi, 4096, **kw4)
-    assert got["n_rounds"] == 4 and ref["n_rounds"] == 4 and not got["converged"]
+    got = _gpu_run(L, prob, lo, hi, 4096, **kw)
+    assert got["n_rounds"] == 3 and ref["n_rounds"] == 3 and not got["converged"]
+    assert got["n_likelihood"] == ref["n_likelihood"] == 64 + 3 * 48
     assert got["n_dead"] == ref["n_dead"] and got["n_samples"] == len(ref["logl"])
     nd = ref["n_dead"]
     assert np.array_equal(got["samples"][:nd], ref["samples"][:nd].astype(np.float32))       # deaths, in order
@@ -119,7 +118,8 @@ def test_tiny_config_evidence_and_posterior_match_the_oracle_driver_and_recover_
     lo, hi = _tiny_priors(cfg)
     kw = dict(n_live=300, batch=256, tol=1e-3, enlarge=1.2, seed=7)
     got = _gpu_run(L, prob, lo, hi, 60000, **kw)
-    ref = ns.run(lambda t: prob.oracle_loglike(t.astype(np.float32), want_model=False), lo, hi, **kw)
+    # a different seed for the oracle driver: "within 3 sigma" then compares two independent runs
+    ref = ns.run(lambda t: prob.oracle_loglike(t.astype(np.float32), want_model=False), lo, hi, **dict(kw, seed=1007))
     assert got["converged"] and ref["converged"]
     err = math.hypot(got["ln_z_err"], ref["ln_z_err"])
     assert abs(got["ln_z"] - ref["ln_z"]) < 3.0 * err, (got["ln_z"], ref["ln_z"], err)
@@ -165,7 +165,8 @@ def test_shrunk_hst_case_with_an_image_plane_prior(L):
         return out.astype(np.float32).astype(np.float64)
 
     got = _gpu_run(L, prob, lo, hi, 40000, image_plane_sources=src, **kw)
-    ref = ns.run(lambda th: prob.oracle_loglike(th.astype(np.float32), want_model=False), lo, hi, transform=transform, **kw)
+    ref = ns.run(lambda th: prob.oracle_loglike(th.astype(np.float32), want_model=False), lo, hi, transform=transform,
+                 **dict(kw, seed=1011))                     # independent of the GPU run's seed
     assert got["converged"] and ref["converged"]
     err = math.hypot(got["ln_z_err"], ref["ln_z_err"])
     assert abs(got["ln_z"] - ref["ln_z"]) < 3.0 * err, (got["ln_z"], ref["ln_z"], err)
@@ -230,3 +231,50 @@ def test_bad_arguments_are_rejected(L):
             L.lensed_ns_run(h, lo, lo)                                          # nothing free
     finally:
         L.lensed_destroy(h)
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_evidence_of_a_sky_only_model_equals_its_closed_form(L, seed):
+    """A pin of the GPU sampler that does not go through oracle/nested_oracle.py (which follows the
+    kernel's structure).  With the model list ("sky",) eq. 17 is a parabola in the
+    one parameter: logL(level) = -1/2 [A (level - mu)^2 + C] with A = sum w, mu = sum w d / A,
+    C = sum w (d - mu)^2, so under a uniform prior on [lo, hi]
+        Z = exp(-C/2) sqrt(2 pi / A) [Phi((hi - mu) sqrt A) - Phi((lo - mu) sqrt A)] / (hi - lo)
+    and, the prior being many posterior widths wide, H = <ln L> - ln Z = -C/2 - 1/2 - ln Z.
+    (tol = 0.02, not smaller: lensed_loglike returns FP32, so in one dimension the live points reach
+    the plateau where every logL rounds to the same float -- |level - mu| < ~0.003 posterior widths
+    here -- before a remaining-evidence fraction of 1e-4 is reached, and a draw that only ties the
+    threshold is never accepted.  The live points' share is added at the end either way.)"""
+    import torch
+    rng = np.random.default_rng(40 + seed)
+    H, W, sigma, level = 12, 10, 0.05, 1.3
+    d = (level + sigma * rng.standard_normal((H, W))).astype(np.float32)
+    w = np.full((H, W), 1.0 / sigma ** 2, dtype=np.float32)
+    A = float(w.astype(np.float64).sum())
+    mu = float((w.astype(np.float64) * d).sum() / A)
+    C = float((w.astype(np.float64) * (d - mu) ** 2).sum())
+    s = 1.0 / math.sqrt(A)
+    lo = np.array([mu - 25.0 * s], dtype=np.float32)
+    hi = np.array([mu + 15.0 * s], dtype=np.float32)
+    phi = lambda x: 0.5 * (1.0 + math.erf(x / math.sqrt(2.0)))
+    ln_z = -0.5 * C + math.log(math.sqrt(2.0 * math.pi / A) * (phi((hi[0] - mu) / s) - phi((lo[0] - mu) / s)) / float(hi[0] - lo[0]))
+    info = -0.5 * C - 0.5 - ln_z
+    cap = 40000
+    samples = torch.zeros((cap, 1), dtype=torch.float32, device="cuda")
+    logl = torch.zeros(cap, dtype=torch.float32, device="cuda")
+    logw = torch.zeros(cap, dtype=torch.float32, device="cuda")
+    h = L.lensed_create(d, w, None, None, synth.get_config(0).quad, synth.kind_ids(("sky",)), 0.05, 0.0)
+    try:
+        res = L.lensed_ns_run(h, lo, hi, n_live=400, batch=128, tol=0.02, enlarge=1.2, seed=seed, max_rounds=2000,
+                              samples_dev=samples, logl_dev=logl, logw_dev=logw)
+    finally:
+        L.lensed_destroy(h)
+    assert res["converged"], res
+    assert abs(res["ln_z"] - ln_z) < 3.0 * res["ln_z_err"], (res["ln_z"], ln_z, res["ln_z_err"])
+    assert res["information"] == pytest.approx(info, rel=0.15)
+    n = res["n_samples"]
+    wgt = np.exp(logw[:n].cpu().numpy().astype(np.float64))
+    x = samples[:n, 0].cpu().numpy().astype(np.float64)
+    mean = (wgt * x).sum() / wgt.sum()
+    sd = math.sqrt((wgt * (x - mean) ** 2).sum() / wgt.sum())
+    assert abs(mean - mu) < 0.25 * s and sd == pytest.approx(s, rel=0.15)
