@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(kMaxModels * kPrepVec) prep_kernel(Program pro
     int kind = -1;
     double p[7];
     bool valid = true;
-    double sersic_c = 0.0, sersic_n = 0.0;          // source Sersic: threshold constants (below)
+    double sersic_c = 0.0, sersic_n = 0.0, sersic_b = 0.0;   // source Sersic: threshold constants (below)
     if (active) {
         kind = prog.kind[m];
         const float *pf = a.params + (size_t)b * prog.P + prog.par_off[m];
@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(kMaxModels * kPrepVec) prep_kernel(Program pro
             double s, c;
             sincos(p[6] * (kPi / 180.0), &s, &c);
             put64(e, p[0] / a.scale + a.cxh, p[1] / a.scale + a.cyh, c, s, q, rs, 1.0 / n, bn, ln_i0);
-            if (kind == K_SRC_SERSIC && n > 1.0) { sersic_c = n * sqrt(q) * rs / bn; sersic_n = n; }
+            if (kind == K_SRC_SERSIC && n > 1.0) { sersic_c = n * sqrt(q) * rs / bn; sersic_n = n; sersic_b = bn; }
             // Foreground expansion (trace_static.cuh): the pixel integral of exp(h(s)), s = (R/r_S)^2,
             // from its Taylor expansion to fourth order in the rule offsets is accurate to
             // 0.016 tau^6 (measured over n in [0.5, 8], q in [0.2, 1], r_S in [2, 60] px for the sub4,
@@ -246,7 +246,13 @@ __global__ void __launch_bounds__(kMaxModels * kPrepVec) prep_kernel(Program pro
         for (int i = 0; i < prog.n_models; ++i) defl += s_defl[lv][i];     // list order: deterministic
         const double G = a.refine_gain * 200.0 / fmax((double)defl, 25.0);
         const double cc = G * sersic_c;
-        d[11] = (float)fmin(pow(cc, -2.0 * sersic_n / (sersic_n - 1.0)), 1e30);
+        // ... and never beyond the scaled radius where the profile has fallen to exp(-24) of its centre,
+        // b_n R'^(1/n) = 24: just above n = 1 the exponent runs away, and with cc < 1 (a compact source,
+        // r_S below ~0.3 px) T2 would reach the clamp and EVERY traced pixel of the vector be re-traced in
+        // FP64 -- one such prior draw then dominates the step.  Out there the component is below FP32
+        // resolution of its own peak, so its rounding noise cannot be seen in any pixel that counts.
+        const double cap = pow(24.0 / sersic_b, 2.0 * sersic_n);
+        d[11] = (float)fmin(fmin(pow(cc, -2.0 * sersic_n / (sersic_n - 1.0)), cap), 1e30);
     }
     if (m == 0) {
         float *der = a.derived + (size_t)b * prog.D;
