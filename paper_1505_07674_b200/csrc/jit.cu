@@ -76,7 +76,9 @@ const Nvrtc &nvrtc()
 struct Driver {
     PFN_cuModuleLoadData_v2000 ModuleLoadData = nullptr;
     PFN_cuModuleGetFunction_v2000 ModuleGetFunction = nullptr;
+    PFN_cuModuleUnload_v2000 ModuleUnload = nullptr;
     PFN_cuFuncSetAttribute_v9000 FuncSetAttribute = nullptr;
+    PFN_cuFuncGetAttribute_v2020 FuncGetAttribute = nullptr;
     PFN_cuLaunchKernel_v4000 LaunchKernel = nullptr;
     bool ok = false;
 };
@@ -92,22 +94,28 @@ const Driver &driver()
                    qr == cudaDriverEntryPointSuccess;
         };
         d.ok = get("cuModuleLoadData", (void **)&d.ModuleLoadData) && get("cuModuleGetFunction", (void **)&d.ModuleGetFunction) &&
-               get("cuFuncSetAttribute", (void **)&d.FuncSetAttribute) && get("cuLaunchKernel", (void **)&d.LaunchKernel);
+               get("cuModuleUnload", (void **)&d.ModuleUnload) && get("cuFuncSetAttribute", (void **)&d.FuncSetAttribute) &&
+               get("cuFuncGetAttribute", (void **)&d.FuncGetAttribute) && get("cuLaunchKernel", (void **)&d.LaunchKernel);
     });
     return d;
 }
 
 }  // namespace
 
+// Immutable once jit_get has published it: clones of a handle launch it from several threads.
 struct JitTracer {
     CUfunction fn = nullptr;
     int np = 0;
-    size_t smem_set = 48 * 1024;
+    size_t smem_max = 48 * 1024;      // dynamic shared memory a launch may ask for (set once, in jit_get)
 };
 
 namespace {
+struct CacheEntry {
+    JitTracer *tracer = nullptr;      // NULL: this signature failed in this process ...
+    std::string why;                  // ... for this reason (reported to every later handle too)
+};
 std::mutex g_mutex;
-std::map<std::string, JitTracer *> g_cache;      // key: device, counts, points per pass, blocks per SM
+std::map<std::string, CacheEntry> g_cache;       // key: device, counts, points per pass, blocks per SM
 }  // namespace
 
 // Which lists are specialised at run time: at most one shear (TraceSig), and few enough positioned
@@ -174,10 +182,13 @@ const JitTracer *jit_get(const int (&c)[K_COUNT], int np, int device, std::strin
              c[K_SRC_SERSIC], c[K_SRC_GAUSS], c[K_FG_SERSIC], c[K_FG_GAUSS], np, minb);
     std::lock_guard<std::mutex> lock(g_mutex);
     auto it = g_cache.find(key);
-    if (it != g_cache.end()) return it->second;
+    if (it != g_cache.end()) {
+        if (!it->second.tracer && why) *why = it->second.why;
+        return it->second.tracer;
+    }
     auto fail = [&](const std::string &msg) -> const JitTracer * {
         if (why) *why = msg;
-        g_cache[key] = nullptr;                  // do not try again in this process
+        g_cache[key] = CacheEntry{nullptr, msg};     // do not try again in this process; keep the reason
         return nullptr;
     };
     const Driver &drv = driver();
@@ -192,28 +203,36 @@ const JitTracer *jit_get(const int (&c)[K_COUNT], int np, int device, std::strin
     CUmodule mod = nullptr;
     CUfunction fn = nullptr;
     if (drv.ModuleLoadData(&mod, cubin.data()) != CUDA_SUCCESS) return fail("cuModuleLoadData failed");
-    if (drv.ModuleGetFunction(&fn, mod, name.c_str()) != CUDA_SUCCESS) return fail("cuModuleGetFunction failed");
+    if (drv.ModuleGetFunction(&fn, mod, name.c_str()) != CUDA_SUCCESS) {
+        drv.ModuleUnload(mod);
+        return fail("cuModuleGetFunction failed");
+    }
+    // the dynamic shared memory any launch may need, allowed once and here (under g_mutex): everything the
+    // device lets a block opt in to beyond the kernel's own static arrays.  jit_launch only reads it.
+    int optin = 0, fixed = 0;
+    if (cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device) != cudaSuccess ||
+        drv.FuncGetAttribute(&fixed, CU_FUNC_ATTRIBUTE_SHARED_SIZE_BYTES, fn) != CUDA_SUCCESS || optin - fixed < 48 * 1024 ||
+        drv.FuncSetAttribute(fn, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, optin - fixed) != CUDA_SUCCESS) {
+        drv.ModuleUnload(mod);
+        return fail("cuFuncSetAttribute(max dynamic shared memory) failed");
+    }
     JitTracer *t = new JitTracer;
     t->fn = fn;
     t->np = np;
-    g_cache[key] = t;                            // the module stays loaded for the life of the process
+    t->smem_max = (size_t)(optin - fixed);
+    g_cache[key] = CacheEntry{t, std::string()};     // the module stays loaded for the life of the process
     return t;
 }
 
 // same launch as trace_block.cuh launch_trace_kernel, through the driver API
-cudaError_t jit_launch(const JitTracer *t0, const Program &prog, const TraceArgs &a0, int nvec, cudaStream_t st)
+cudaError_t jit_launch(const JitTracer *t, const Program &prog, const TraceArgs &a0, int nvec, cudaStream_t st)
 {
-    JitTracer *t = const_cast<JitTracer *>(t0);
     const Driver &drv = driver();
     TraceArgs a = a0;
     a.quad = a0.quad_pp;
     a.nq_pad = a0.nq_pp;
     const size_t smem = trace_smem_bytes(prog, a.nq_pad);
-    if (smem > t->smem_set) {
-        if (drv.FuncSetAttribute(t->fn, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)smem) != CUDA_SUCCESS)
-            return cudaErrorInvalidValue;
-        t->smem_set = smem;
-    }
+    if (smem > t->smem_max) return cudaErrorInvalidValue;
     Program p = prog;
     void *params[2] = {&p, &a};
     const unsigned gx = (unsigned)((a.npix + a.pix_per_block - 1) / a.pix_per_block);
