@@ -48,3 +48,49 @@ def pixel_errors(model_gpu, model_ref):
 
 def logl_errors(logl_gpu, logl_ref):
     return np.abs(np.asarray(logl_gpu, dtype=np.float64) - logl_ref) / np.maximum(np.abs(logl_ref), 1e-300)
+
+
+# ---------------------------------------------------------------------------- parameter domain
+# Hand-written expectations for the parameter domain, shared by the CPU pin of the oracle
+# (test_oracle_pins.py) and the GPU test (test_parity_gpu.py): neither side's code wrote them.
+# SURVEY.md section 8(b) "Errors" fixes: q outside (0, 1], r <= 0 (Sersic), sigma <= 0, n <= 0 and
+# non-finite values are outside the domain.  DESIGN.md section 2 "Domain" adds this build's two
+# readings: 0.02 <= n <= 20, and r = 0 allowed for the lenses (a lens of zero mass deflects nothing).
+DOMAIN_BASE = {
+    "sis": [0.01, -0.02, 0.3], "point": [0.01, -0.02, 0.05], "sie": [0.01, -0.02, 0.3, 0.7, 30.0],
+    "shear": [0.03, -0.02],
+    "src_sersic": [0.02, 0.01, 0.1, -1.0, 1.5, 0.7, 40.0], "fg_sersic": [0.02, 0.01, 0.1, -1.0, 1.5, 0.7, 40.0],
+    "src_gauss": [0.02, 0.01, 0.08, -1.0, 0.7, 40.0], "fg_gauss": [0.02, 0.01, 0.08, -1.0, 0.7, 40.0],
+    "sky": [0.1],
+}
+_DOMAIN_EDGES = {                      # kind -> (slot, value, inside the domain?)
+    "sis": [(2, -1e-3, False), (2, 0.0, True)],
+    "point": [(2, -1e-3, False), (2, 0.0, True)],
+    "sie": [(2, -1e-3, False), (2, 0.0, True), (3, 0.0, False), (3, -0.5, False), (3, 1e-3, True), (3, 1.0, True),
+            (3, 1.0001, False)],
+    "shear": [(0, 5.0, True), (1, -5.0, True)],
+    "src_sersic": [(2, 0.0, False), (2, -0.1, False), (2, 1e-3, True), (4, 0.0, False), (4, 0.0199, False), (4, 0.0201, True),
+                   (4, 20.0, True), (4, 20.01, False), (5, 0.0, False), (5, 1.0, True), (5, 1.0001, False)],
+    "src_gauss": [(2, 0.0, False), (2, -0.1, False), (2, 1e-3, True), (4, 0.0, False), (4, 1.0, True), (4, 1.0001, False)],
+    "sky": [(0, -3.0, True)],
+}
+_DOMAIN_EDGES["fg_sersic"] = _DOMAIN_EDGES["src_sersic"]
+_DOMAIN_EDGES["fg_gauss"] = _DOMAIN_EDGES["src_gauss"]
+
+
+def domain_cases():
+    """-> [(models, params float32, valid)]: for every kind one vector just inside and one just
+    outside every bound, and NaN / +inf / -inf in every slot.  A lens comes with a Gaussian source
+    behind it so that there is something to render."""
+    out = []
+    for kind, base in DOMAIN_BASE.items():
+        lens = kind in ("sis", "point", "sie", "shear")
+        models = (kind, "src_gauss") if lens else (kind,)
+        tail = DOMAIN_BASE["src_gauss"] if lens else []
+        rows = list(_DOMAIN_EDGES[kind]) + [(s, v, False) for s in range(len(base)) for v in (np.nan, np.inf, -np.inf)]
+        rows.append((0, base[0], True))                          # the base vector itself
+        for slot, value, valid in rows:
+            p = np.array(list(base) + list(tail), dtype=np.float32)
+            p[slot] = value
+            out.append((models, p, valid))
+    return out

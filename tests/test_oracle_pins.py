@@ -488,6 +488,27 @@ def test_invalid_vector_gives_minus_infinity_and_nan_image():
     assert np.isfinite(model[0]).all() and np.isnan(model[1]).all()
 
 
+def test_parameter_domain_bound_by_bound_against_hand_written_expectations():
+    """params_valid, every kind and every bound: a vector just inside is rendered (finite logL and
+    image), one just outside -- or with NaN / inf in any slot -- gives logL = -inf and a NaN image.
+    The expectations are written out by hand in tests/cases.py (SURVEY.md section 8(b) "Errors";
+    DESIGN.md section 2 "Domain" for 0.02 <= n <= 20 and r = 0 allowed for lenses)."""
+    from paper_1505_07674_b200 import synth
+    from tests.cases import domain_cases
+    H, W, s = 10, 12, 0.05
+    quad = synth.get_config(0).quad
+    d, w = np.zeros((H, W)), np.ones((H, W))
+    cases = domain_cases()
+    assert sum(v for _, _, v in cases) >= 25 and sum(not v for _, _, v in cases) >= 130
+    for models, p, valid in cases:
+        logl, model = orc.loglike(H, W, s, d, w, None, None, quad, synth.kind_ids(models), p[None], want_model=True)
+        what = (models, p.tolist())
+        if valid:
+            assert np.isfinite(logl[0]) and np.isfinite(model[0]).all(), what
+        else:
+            assert logl[0] == -np.inf and np.isnan(model[0]).all(), what
+
+
 # -------------------------------------------------------------------- whole pipeline
 def test_rotation_by_90_degrees_and_mirror_of_the_whole_pipeline():
     # square image, symmetric rule, PSF rotated/mirrored along: the model image rotates/mirrors
