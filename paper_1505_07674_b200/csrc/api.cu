@@ -1,7 +1,8 @@
-// api.cu -- the C ABI of include/lensed.h: handle, argument checks, create-time tables
+// api.cu -- the C ABI of include/lensed.h and include/lensed_tune.h: handle, argument checks, create-time tables
 // (traced-pixel list, active tiles, flipped PSF, padded rule), batch chunking and launches.
 // Host logic only; every step of the path runs in prep.cu / trace.cu / conv.cu.
 #include "../../include/lensed.h"
+#include "../../include/lensed_tune.h"
 #include "lensed_internal.h"
 #include "jit.h"
 
@@ -958,6 +959,27 @@ lensed_status lensed_set_fg_expansion(lensed_handle *h, double tau)
     if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
     if (tau != tau || tau > 0.5) return fail(h, LENSED_EINVAL, "tau = %g outside [0, 0.5]", tau);
     h->fgx_tau = tau > 0.0 ? tau : 0.0;
+    return LENSED_OK;
+}
+
+namespace {
+__global__ void fill_kernel(float *p, size_t n, float value)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = value;
+}
+}  // namespace
+
+lensed_status lensed_debug_fill_frames(lensed_handle *h, float value)
+{
+    if (!h) return fail(nullptr, LENSED_EINVAL, "null handle");
+    if (!isfinite(value)) return fail(h, LENSED_EINVAL, "value must be finite (0 x NaN would leak through the zero taps)");
+    CU(h, cudaSetDevice(h->device));
+    CU(h, cudaDeviceSynchronize());
+    if (h->d_L && h->cap_L) {
+        fill_kernel<<<1024, 256>>>(h->d_L, h->cap_L, value);
+        CU(h, cudaGetLastError());
+        CU(h, cudaDeviceSynchronize());
+    }
     return LENSED_OK;
 }
 

@@ -25,6 +25,7 @@
 // candidate, try, stream), restated here from the published algorithm; the CPU oracle states
 // it again on its side, so both draw the same numbers.
 #include "../../include/lensed.h"
+#include "../../include/lensed_tune.h"
 #include "lensed_internal.h"
 
 #include <math.h>

@@ -21,7 +21,7 @@ LENS_SIS, LENS_SIE, LENS_POINT, LENS_SHEAR = 0, 1, 2, 3
 SRC_SERSIC, SRC_GAUSS, FG_SERSIC, FG_GAUSS, FG_SKY = 4, 5, 6, 7, 8
 PHASES = ("prep", "trace", "refine", "conv", "final")
 
-# every symbol include/lensed.h declares: (restype, argtypes)
+# every symbol include/lensed.h and include/lensed_tune.h declare: (restype, argtypes)
 _c, _i, _d, _p, _ll = ctypes.c_char_p, ctypes.c_int, ctypes.c_double, ctypes.c_void_p, ctypes.c_longlong
 SYMBOLS = {
     "lensed_create": (_i, [_i, _i, _d, _p, _p, _p, _p, _i, _i, _p, _i, _p, _i, _d, _i, _p]),
@@ -44,6 +44,7 @@ SYMBOLS = {
     "lensed_set_refine": (_i, [_p, _d]),
     "lensed_set_fg_expansion": (_i, [_p, _d]),
     "lensed_get_refined": (_i, [_p, _p]),
+    "lensed_debug_fill_frames": (_i, [_p, ctypes.c_float]),
     "lensed_set_chunk_bytes": (_i, [_p, _ll]),
     "lensed_frame_bytes": (_ll, [_p]),
     "lensed_set_conv_shape": (_i, [_p, _i]),
@@ -278,6 +279,11 @@ def lensed_get_refined(h):
     n = ctypes.c_longlong()
     _check(lib().lensed_get_refined(h, ctypes.byref(n)), h)
     return n.value
+
+
+def lensed_debug_fill_frames(h, value):
+    """overwrite every cell of the handle's scratch frames (lensed_tune.h): uninitialised-read check"""
+    _check(lib().lensed_debug_fill_frames(h, float(value)), h)
 
 
 def lensed_set_chunk_bytes(h, nbytes):

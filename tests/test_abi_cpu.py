@@ -14,9 +14,27 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _declared():
-    text = open(os.path.join(ROOT, "include", "lensed.h")).read()
+    return _declared_in("lensed.h") | _declared_in("lensed_tune.h")
+
+
+def _declared_in(header):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return set(re.findall(r"\b(lensed_[a-z_]+)\s*\(", text))
+
+
+def test_the_method_header_holds_the_method_and_the_tuning_header_the_rest():
+    """include/lensed.h: the calls that follow the paper's statement of the problem; every
+    measurement, tuning and test hook is declared in include/lensed_tune.h instead."""
+    method, tune = _declared_in("lensed.h"), _declared_in("lensed_tune.h")
+    assert not method & tune
+    assert method == {"lensed_create", "lensed_clone", "lensed_num_params", "lensed_num_traced", "lensed_num_pixels",
+                      "lensed_render", "lensed_loglike", "lensed_render_host", "lensed_loglike_host", "lensed_deflect",
+                      "lensed_image_plane_prior", "lensed_estimate_weights", "lensed_set_error_rule", "lensed_render_error",
+                      "lensed_ns_run", "lensed_chisq_static", "lensed_last_error", "lensed_destroy"}
+    assert all("debug" not in n and "_set_" not in n.replace("lensed_set_error_rule", "") for n in method)
+    assert {"lensed_set_profiling", "lensed_debug_force_global_taps", "lensed_fma_peak", "lensed_issue_probe",
+            "lensed_ns_philox", "lensed_set_conv_shape", "lensed_set_static_tracer"} <= tune
 
 
 def test_library_exports_every_declared_symbol_and_binding_covers_them():

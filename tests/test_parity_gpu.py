@@ -446,6 +446,37 @@ def test_quadrature_error_map_of_the_gauss_kronrod_rule(L, n_kronrod):
             np.abs(err[b] - ref) / bound).max()
 
 
+@pytest.mark.parametrize("index,H,W", [(2, 75, 93), (1, 72, 66), (3, 70, 80)])
+def test_frame_cells_the_tracer_never_writes_reach_no_result(L, index, H, W):
+    """Stand-in for an uninitialised-read checker (compute-sanitizer is closed on this pool).  The
+    padded frames of the unconvolved images hold cells no kernel writes: pad cells no border pixel
+    clamps to and, on a masked image, pixels outside the traced set.  The convolution reads some of
+    them under structurally zero taps or for outputs it discards (conv.cu "Input").  Overwriting
+    EVERY cell of the frames between two calls (lensed_debug_fill_frames, include/lensed_tune.h)
+    must not change one bit of logL or of the rendered images, in any convolution shape."""
+    cfg = synth.shrunk(synth.get_config(index), H, W, 5)
+    prob = Problem(cfg)
+    params = cfg.batch(5)
+    h = prob.create()
+    try:
+        for shape in (3, 2, 1, 0):
+            try:
+                L.lensed_set_conv_shape(h, shape)
+            except L.LensedError as e:
+                assert e.status == L.EUNSUPPORTED
+                continue
+            ref = _gpu_eval(L, h, params, H, W)
+            for value in (1e30, -7.5):
+                L.lensed_debug_fill_frames(h, value)
+                logl = _gpu_eval(L, h, params, H, W, render=False)[0]
+                assert np.array_equal(logl, ref[0]), (shape, value)
+                L.lensed_debug_fill_frames(h, value)
+                model = _gpu_eval(L, h, params, H, W)[1]
+                assert np.array_equal(model, ref[1]), (shape, value)
+    finally:
+        L.lensed_destroy(h)
+
+
 def test_full_constant_tap_pool_falls_back_to_global_memory_taps(L):
     """The PSF taps of the live handles share 60 KB of constant memory (include/lensed.h).  Two
     63x63 PSFs (32.5 KB each) do not fit together: the second handle keeps its taps in global
