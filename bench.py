@@ -53,6 +53,32 @@ def flops_per_ray(models):
     return FLOPS_RAY_POS + FLOPS_QUAD + sum(FLOPS_MODEL[m] for m in models)
 
 
+# "if the build uses a cheaper algorithm ... it counts that algorithm's flops".  The
+# specialised tracers take a foreground Sersic's pixel integral from its moment expansion
+# (DESIGN.md section 5): 25-70 flops per PIXEL instead of 17 per RAY, for all but the few pixels
+# around the profile's centre.  The count of the algorithm that runs charges the expansion's
+# fourth-order cost for every pixel, spread over the pixel's rays.  The pixels that still take the
+# per-ray sum do more work than that, so this is a LOWER bound on the work required and on the
+# fraction; the bench line's `frac` of a tracer-dominant config uses it.
+FG_EXPANSION_FLOPS_PER_PIXEL = 70
+
+
+def rule_is_symmetric(quad):
+    """first and third moments of the rule vanish (the condition api.cu puts on the expansion)"""
+    q = np.asarray(quad, dtype=np.float64).reshape(-1, 3)
+    x, y, w = q[:, 0], q[:, 1], q[:, 2] / q[:, 2].sum()
+    m = [w @ x, w @ y, w @ x ** 3, w @ (x * x * y), w @ (x * y * y), w @ y ** 3]
+    return bool(max(abs(v) for v in m[:2]) < 1e-7 and max(abs(v) for v in m[2:]) < 1e-8)
+
+
+def flops_per_ray_run(models, n_quad, expansion):
+    """flops per ray of the algorithm in use: as flops_per_ray, foreground Sersics by expansion"""
+    if not expansion:
+        return float(flops_per_ray(models))
+    n_fg = sum(1 for m in models if m == "fg_sersic")
+    return flops_per_ray(models) - n_fg * FLOPS_MODEL["fg_sersic"] + n_fg * FG_EXPANSION_FLOPS_PER_PIXEL / n_quad
+
+
 def flops_per_conv_pixel(cfg):
     taps = 1 if cfg.psf is None else cfg.psf.size
     return 2 * taps + 3
@@ -193,6 +219,10 @@ class Bench:
             lensed.lensed_set_conv_shape(self.h, lensed.CONV_SHAPES.index(args.conv_shape))
         self.tracer_kind = ("interpreter", "static", "jit")[lensed.lensed_get_static_tracer(self.h)]
         self.conv_shape = lensed.CONV_SHAPES[lensed.lensed_get_conv_shape(self.h)]
+        # the foreground expansion runs in the specialised tracers on rules without odd moments
+        self.fg_expansion = self.tracer_kind != "interpreter" and rule_is_symmetric(cfg.quad)
+        self.flops_ray = flops_per_ray(cfg.models)                                          # SURVEY.md 8(d)'s count
+        self.flops_ray_run = flops_per_ray_run(cfg.models, len(cfg.quad), self.fg_expansion)   # the algorithm in use
         self.n_traced = cfg.n_traced()                       # m_d, the required set
         assert self.n_traced <= lensed.lensed_num_traced(self.h)
         self.n_counted = int(cfg.H * cfg.W if cfg.mask is None else cfg.mask.sum())
@@ -261,7 +291,7 @@ class Bench:
     def flop_model(self, steps, phase_n):
         """algorithmic flops of ONE launch of the tracer / the convolution, averaged over its launches"""
         cfg = self.cfg
-        return {"trace": flops_per_ray(cfg.models) * len(cfg.quad) * self.n_traced * self.B * steps / max(phase_n["trace"], 1),
+        return {"trace": self.flops_ray_run * len(cfg.quad) * self.n_traced * self.B * steps / max(phase_n["trace"], 1),
                 "conv": flops_per_conv_pixel(cfg) * self.n_counted * self.B * steps / max(phase_n["conv"], 1)}
 
     def kernels(self, steps, phase_ms, phase_n):
@@ -289,9 +319,48 @@ class Bench:
                 "rays_per_s": value * self.n_traced * len(cfg.quad), "ms_per_step": sum(ms) / steps, "steps": steps,
                 "tracer": self.tracer_kind, "conv_shape": self.conv_shape,
                 "trace_ms": k["trace"]["ms_per_step"], "trace_frac": k["trace"]["frac"],
+                "trace_frac_survey_count": k["trace"]["frac"] * self.flops_ray / self.flops_ray_run if k["trace"]["frac"] else None,
+                "flops_per_ray": self.flops_ray, "flops_per_ray_run": self.flops_ray_run,
                 "conv_ms": k["conv"]["ms_per_step"], "conv_frac": k["conv"]["frac"],
                 "other_ms": sum(k[p]["ms_per_step"] for p in ("prep", "refine", "final")),
                 "whole_step_frac": whole / NOMINAL_FP32_TFLOPS}
+
+
+def parity_sample(lensed, torch, bench, logl_dev, n):
+    """SURVEY.md section 4 "max and 99.999th-percentile pixel error", at the scale the bench runs: n vectors
+    spread evenly over the timed batch, logL (the values the timed region produced) and rendered pixels
+    against the CPU oracle as checker, in chunks of 32 vectors.  Also the FP64-refined pixels per vector,
+    so that the refinement threshold is looked at once at full batch size."""
+    from oracle import lensed_oracle as orc
+    cfg = bench.cfg
+    idx = np.unique(np.linspace(0, bench.B - 1, min(n, bench.B)).astype(np.int64))
+    kinds = synth.kind_ids(cfg.models)
+    logl_g = logl_dev.cpu().numpy()[idx].astype(np.float64)
+    el, ep, pix_all = [], [], []
+    model = torch.empty((32, cfg.H, cfg.W), dtype=torch.float32, device=bench.dev)
+    for c0 in range(0, len(idx), 32):
+        sel = idx[c0:c0 + 32]
+        p = bench.params[sel]
+        lo, mo = orc.loglike(cfg.H, cfg.W, cfg.scale, bench.image, bench.weight, cfg.mask, cfg.psf, cfg.quad, kinds, p,
+                             zp=cfg.zp, want_model=True)
+        lensed.lensed_render(bench.h, torch.from_numpy(p).to(bench.dev), model[:len(sel)])
+        torch.cuda.synchronize()
+        mg = model[:len(sel)].cpu().numpy().astype(np.float64)
+        el.extend(np.abs(logl_g[c0:c0 + 32] - lo) / np.maximum(np.abs(lo), 1e-300))
+        for g, r in zip(mg, mo):
+            big = np.abs(r) > 1e-3 * np.abs(r).max()
+            e = np.abs(g[big] - r[big]) / np.abs(r[big])
+            ep.append(e.max())
+            pix_all.append(e)
+    el, ep, pix_all = np.array(el), np.array(ep), np.concatenate(pix_all)
+    lensed.lensed_reset_profile(bench.h)
+    lensed.lensed_loglike(bench.h, bench.p_dev, bench.logl)
+    refined = lensed.lensed_get_refined(bench.h)
+    return {"vectors": int(len(idx)), "logl_tol": 1e-5, "pixel_tol": 1e-4,
+            "logl_err_max": float(el.max()), "logl_err_p999": float(np.quantile(el, 0.999)), "logl_over_tol": int((el > 1e-5).sum()),
+            "pixel_err_max": float(ep.max()), "pixel_err_p99999": float(np.quantile(pix_all, 0.99999)),
+            "pixels_checked": int(pix_all.size), "vectors_with_a_pixel_over_tol": int((ep > 1e-4).sum()),
+            "refined_pixels_per_vector": refined / bench.B}
 
 
 def nested_row(lensed, torch, local, rounds=40, n_live=1024, batch=1024):
@@ -346,6 +415,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--conv-shape", default="auto", choices=("auto", "wide", "narrow", "strip", "half"),
                     help="convolution shape (include/lensed.h); auto = what lensed_create picks")
+    ap.add_argument("--parity-sample", type=int, default=0, metavar="N",
+                    help="extra, outside the timed region: N vectors spread over the batch against the CPU oracle "
+                         "(logL and rendered pixels), max and 99.9th-percentile error; Euclid: ~0.06 s of oracle per vector")
     ap.add_argument("--interpreter", action="store_true",
                     help="run the interpreting tracer instead of the compile-time specialised one")
     args = ap.parse_args()
@@ -434,10 +506,25 @@ def main():
                 "frac_of_measured_ffma": achieved / measured_ffma if measured_ffma else None,
                 "whole_step_tflops": (per_launch["trace"] * phase_n["trace"] + per_launch["conv"] * phase_n["conv"])
                 / (total_ms * 1e-3) / 1e12 if world == 1 else None,
-                "flops_per_ray": flops_per_ray(cfg.models), "flops_per_conv_pixel": flops_per_conv_pixel(cfg),
+                "flops_per_ray": bench.flops_ray, "flops_per_ray_run": bench.flops_ray_run,
+                "flop_count": "flops_per_ray_run: SURVEY 8(d)'s per-ray counts with each foreground Sersic charged its "
+                              "moment expansion (70 flops per pixel / n_quad per ray) where the specialised tracer uses it -- "
+                              "a lower bound on the work required; every tflops / frac here uses it",
+                "fg_expansion": bench.fg_expansion,
+                "flops_per_conv_pixel": flops_per_conv_pixel(cfg),
                 "kernels": kern}
+    if kern["trace"]["frac"]:
+        roofline["trace_frac"] = kern["trace"]["frac"]
+        roofline["trace_frac_survey_count"] = kern["trace"]["frac"] * bench.flops_ray / bench.flops_ray_run
     if roofline["whole_step_tflops"]:
         roofline["whole_step_frac"] = roofline["whole_step_tflops"] / NOMINAL_FP32_TFLOPS
+    if traffic:
+        # algorithmic bytes of the dominant kernel per launch: the convolution reads each padded frame once (4 B per
+        # pixel; d, w and the taps are amortised over the batch), the tracer writes it once
+        alg = 4.0 * cfg.H * cfg.W * B * args.steps / max(phase_n[dom], 1)
+        roofline["traffic_over_algorithmic_bytes"] = traffic / alg
+        roofline["traffic_note"] = ("not measured in this run: dram bytes per vector of the committed ncu capture (traffic_source), "
+                                    "scaled to this launch; above 1 = halo re-reads across tiles, harmless on an ALU-bound kernel")
 
     # -------------------------------------------------------------- batch sweep (config 4 only)
     sweep = None
@@ -462,6 +549,12 @@ def main():
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": "%d of the %d vectors, full image, %.1f s" % (n, B, dt)}
     gpu_launches = int(sum(phase_n.values()))
+    parity = None
+    if rank == 0 and world == 1 and args.parity_sample > 0:
+        try:
+            parity = parity_sample(lensed, torch, bench, logl, args.parity_sample)
+        except Exception as ex:                              # noqa: BLE001 -- an extra: the bench line stands without it
+            parity = {"error": str(ex)[:200]}
     bench.close()
 
     # ------------------------------- the other configs and the sampler row (short, rank 0, N = 1)
@@ -500,12 +593,14 @@ def main():
             "gpu_launches": gpu_launches,
             "clocks": clock_info, "roofline": roofline, "cpu_baseline": cpu,
         }
+        if parity is not None:
+            out["parity_sample"] = parity
         if sweep is not None:
             out["sweep"] = sweep
         if per_config is not None:
             out["per_config"] = per_config
             out["nested_sampling"] = nested
-        print(json.dumps(out))
+        print(json.dumps(out, default=lambda o: o.item() if hasattr(o, "item") else str(o)))   # numpy scalars
     if world > 1:
         dist.destroy_process_group()
 
