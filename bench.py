@@ -411,7 +411,7 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="vectors per GPU per step (0 = the config's)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the batch sweep of the Euclid config")
     ap.add_argument("--no-extras", action="store_true",
-                    help="skip the per-config rows (configs 0-3, 5) and the nested-sampling row")
+                    help="skip the per-config rows (configs 0-3, 5, 6) and the nested-sampling row")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--conv-shape", default="auto", choices=("auto", "wide", "narrow", "strip", "half"),
                     help="convolution shape (include/lensed.h); auto = what lensed_create picks")
@@ -561,7 +561,7 @@ def main():
     per_config = nested = None
     if args.config == DEFAULT_CONFIG and not args.no_extras and world == 1 and not args.batch:
         per_config = []
-        for c, steps in ((0, 20), (1, 20), (2, 10), (3, 5), (5, 10)):
+        for c, steps in ((0, 20), (1, 20), (2, 10), (3, 5), (5, 10), (6, 10)):
             try:
                 b = Bench(lensed, torch, c, synth.get_config(c).B, local, rank, args)
                 row = b.summary(steps, 3, flush)
