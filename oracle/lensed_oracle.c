@@ -29,7 +29,10 @@
  * light_constants / light_profile); oracle_source_position against the lens
  * equation solved by inspection (SIS image positions), the additivity of
  * deflections and grad(psi); oracle_estimate_weights against hand values and
- * the unit mean of w (d - mu)^2 on seeded Poisson counts.  Parity unpinned:
+ * the unit mean of w (d - mu)^2 on seeded Poisson counts; params_valid bound
+ * by bound against the hand-written table of tests/cases.py (domain_cases:
+ * every kind, one vector just inside and one just outside every bound, NaN /
+ * inf in every slot).  Parity unpinned:
  * absolute pixel values of any figure of the paper (it prints none).
  *
  * Build: gcc -O2 -std=c99 -fopenmp -fPIC -shared lensed_oracle.c -o liblensed_oracle.so -lm

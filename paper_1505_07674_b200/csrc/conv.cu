@@ -413,7 +413,7 @@ __global__ void __maxnreg__(176) conv_kernel(const __grid_constant__ ConvArgs a,
 // uniform datapath (LDCU + UR operands, 305 instructions per loop body); with 255, or with a
 // minimum block count in __launch_bounds__, it moves them to vector registers (LDC + 24-28 MOV,
 // 327 instructions, 14 % slower).
-// // What the block shapes above
+// What the block shapes above
 // lose at their barriers -- the tile prologue (wait for the copy), the epilogue (chi-square
 // reduction) and the ramps of the chunk loops, during which a block's warps all leave the FMA pipe
 // together -- a warp here loses alone, while the other warp of its scheduler keeps the pipe busy.
